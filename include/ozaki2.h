@@ -1,0 +1,141 @@
+/*
+ * ozaki2.h -- C ABI of the B200-native Ozaki-scheme-II DGEMM library (libozaki2.so).
+ *
+ * The library emulates C = alpha * A B + beta * C in FP64 on the INT8 tensor cores of one
+ * B200 (sm_100a), following "Improved Scaling for Fast Mode of Ozaki Scheme II"
+ * (PAPER.md, cited as P:<line>): Steps 1-4 of section 2.2 with the three ways
+ * of choosing the scaling vectors mu, nu of section 2.3 / section 4.
+ *
+ * Conventions for every entry point
+ *   - plain pointers and sizes only; "device pointer" = memory of the current CUDA device,
+ *     "host pointer" = ordinary host memory.  Nothing is allocated or freed for the caller.
+ *   - matrices are column-major (BLAS "NN"): A is m x k with leading dimension lda >= max(1,m),
+ *     B is k x n with ldb >= max(1,k), C is m x n with ldc >= max(1,m).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
+ *     that take a stream only enqueue work: no host synchronisation, no allocation.
+ *   - return value: 0 on success; -i if the i-th argument (1-based, as written in the
+ *     prototype) is invalid; OZAKI2_ERR_WORKSPACE if the workspace is missing or too small;
+ *     OZAKI2_ERR_DEVICE if the device is not sm_100; a positive value is a cudaError_t from a
+ *     launch or copy.  Nothing throws across this boundary.
+ *   - non-finite inputs are not detected: a row of A / column of B holding Inf or NaN gives
+ *     unspecified values in that row / column of C (never a hang or a fault).
+ */
+#ifndef OZAKI2_H
+#define OZAKI2_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* scaling_mode */
+#define OZAKI2_MODE_ACCURATE 0 /* accurate mode: auxiliary INT8 GEMM, eq. (4)-(9)      */
+#define OZAKI2_MODE_FAST 1     /* original fast mode: Algorithm 1, eq. (11)(12)        */
+#define OZAKI2_MODE_PROP 2     /* revised fast mode: Algorithm 2, eq. (17)(18)         */
+
+#define OZAKI2_MIN_MODULI 2
+#define OZAKI2_MAX_MODULI 20           /* prefix of eq. (14)                           */
+#define OZAKI2_MAX_K (1 << 17)         /* INT32 accumulator bound                          */
+
+#define OZAKI2_ERR_WORKSPACE (-100)
+#define OZAKI2_ERR_DEVICE (-101)
+
+/*
+ * The hot path.  C := alpha * (A B)~ + beta * C, where (A B)~ is the Ozaki-II emulation with
+ * `num_moduli` moduli (the first num_moduli of eq. (14)) and scaling mode `scaling_mode`:
+ *   S1  mu_i = 2^e_i, nu_j = 2^f_j from row / column statistics
+ *   S2  A' = trunc(diag(mu) A), B' = trunc(B diag(nu)); INT8 residues rmod(., p_l)
+ *   S3  U_l = (rmod(A',p_l) rmod(B',p_l)) mod p_l on the INT8 tensor cores, l = 1..N    (eq. 2)
+ *   S4  C'' = rmod(sum_l P_l q_l U_l, P)                                          (eq. 2, 3)
+ *   S5  C = diag(mu)^-1 C'' diag(nu)^-1, then alpha / beta
+ * A, B, C: device pointers, 8-byte aligned; C must not overlap A or B.  C is read only if
+ * beta != 0.  alpha, beta by value.  Quick returns: m == 0 or n == 0 does nothing; k == 0 or
+ * alpha == 0 gives C := beta * C (zeros if beta == 0).  k <= OZAKI2_MAX_K.
+ * Needs a workspace of ozaki2_workspace_bytes(m, n, k, num_moduli, scaling_mode) bytes
+ * registered with ozaki2_set_workspace for the current device.  Asynchronous on `stream`.
+ */
+int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
+                 const double *B, int64_t ldb, double beta, double *C, int64_t ldc,
+                 int num_moduli, int scaling_mode, void *stream);
+
+/* Bytes of device workspace ozaki2_dgemm needs for this problem (0 for an invalid one). */
+size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
+
+/*
+ * Register a caller-owned device buffer (256-byte aligned) as the workspace of the current
+ * device; it must stay valid until replaced.  (NULL, 0) unregisters.  Not stream ordered: do
+ * not replace it while calls that use it are in flight.
+ */
+int ozaki2_set_workspace(void *device_ptr, size_t bytes);
+
+/*
+ * The same call with HOST buffers: copies A and B to the device, runs ozaki2_dgemm, copies C
+ * back (and C in first if beta != 0), all on `stream`, then synchronises the stream.
+ * `device_scratch` is a caller-owned device buffer of at least
+ * ozaki2_host_scratch_bytes(m, n, k) bytes that receives the device copies of A, B, C.
+ * Host buffers should be page-locked for the copies to run at link speed.
+ */
+int ozaki2_dgemm_host(int64_t m, int64_t n, int64_t k, double alpha, const double *A_host, int64_t lda,
+                      const double *B_host, int64_t ldb, double beta, double *C_host, int64_t ldc,
+                      int num_moduli, int scaling_mode, void *device_scratch, size_t scratch_bytes,
+                      void *stream);
+size_t ozaki2_host_scratch_bytes(int64_t m, int64_t n, int64_t k);
+
+/* Text for a return value of this library. */
+const char *ozaki2_status_string(int status);
+
+/* ------------------------------------------------------------------------------------------
+ * Parity and profiling surface.  ozaki2_dgemm_stages runs exactly the kernels of ozaki2_dgemm
+ * and, in addition, copies the intermediate results of each stage into the caller's device
+ * buffers in CANONICAL layouts (independent of the internal pitches).  Every pointer may be
+ * NULL (= not wanted).
+ * ---------------------------------------------------------------------------------------- */
+typedef struct ozaki2_stage_outputs {
+    int32_t *e;          /* [m]        log2 mu_i                                              */
+    int32_t *f;          /* [n]        log2 nu_j                                              */
+    int32_t *rowmax;     /* [m]        max_j cbar_ij, accurate mode only          */
+    int32_t *colmax;     /* [n]        max_i cbar_ij, accurate mode only                      */
+    int8_t *resA;        /* [N][m][k]  symmetric INT8 residues of A', k fastest               */
+    int8_t *resB;        /* [N][n][k]  symmetric INT8 residues of B', k fastest               */
+    uint8_t *U;          /* [N][n][m]  (resA_l resB_l^T) mod p_l in [0,p_l), m fastest        */
+    uint64_t *Cpp;       /* [n][m][4]  C'' as 256-bit two's-complement words, little-endian   */
+    float *stage_ms;     /* HOST pointer, [5]: elapsed ms of S1, S2, S3, S4+S5, total; filling
+                            it synchronises the stream (profiling only)                       */
+} ozaki2_stage_outputs;
+
+int ozaki2_dgemm_stages(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
+                        const double *B, int64_t ldb, double beta, double *C, int64_t ldc,
+                        int num_moduli, int scaling_mode, void *stream, const ozaki2_stage_outputs *out);
+
+/*
+ * Constants of Step 1 for `num_moduli` moduli, written to HOST arrays (any may be NULL):
+ * p[N], q[N] (q_l = P_l^-1 mod p_l), P_words[4] and w_words[N][4] (w_l = P_l q_l,
+ * eq. (2)) as little-endian 64-bit words, and the FP32 constants P'_prop = P'_accu
+ * (P:141-143), P'_fast, delta (eq. (6)).
+ */
+int ozaki2_get_constants(int num_moduli, int32_t *p, int32_t *q, uint64_t *P_words, uint64_t *w_words,
+                         float *Pprop, float *Pfast, float *delta);
+
+/* y[t] = LOG2F(x[t]) for x[t] in [1,2]: the library's stand-in for __log2f (R3),
+ * evaluated on the device.  x, y: device pointers. */
+int ozaki2_debug_log2f(const float *x, float *y, int64_t count, void *stream);
+
+/* out[t] = in[t] mod p_l in [0,p_l) for any INT32 in[t], computed by the same routine as the
+ * epilogue of the residue GEMM.  in, out: device pointers. */
+int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64_t count, void *stream);
+
+/* One INT8 product resA_l resB_l^T mod p_l for canonical planes (same layouts as above) on the
+ * tensor-core kernel (use_tensor_cores != 0) or on a plain CUDA-core check kernel (== 0) that
+ * ozaki2_dgemm never uses.  Both need no workspace. */
+int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA,
+                              const int8_t *resB, uint8_t *U, int use_tensor_cores, void *stream);
+
+/* Library build information: "ozaki2 <version> sm_100a ..." */
+const char *ozaki2_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OZAKI2_H */

@@ -1,0 +1,493 @@
+// oz2_api.cu -- the C ABI of libozaki2 (include/ozaki2.h): argument checks, Step-1 constants,
+// workspace carving and the launch sequence S1..S5 on the caller's stream.  No host synchronisation and no
+// allocation on the ozaki2_dgemm path.
+#include "../../include/ozaki2.h"
+#include "oz2_common.cuh"
+
+#include <math.h>
+#include <stdio.h>
+#include <mutex>
+#include <string.h>
+#include <vector>
+
+namespace {
+
+const int kModuli[OZ2_MAX_MODULI] = OZ2_MODULI_LIST;
+
+// ---------------------------------------------------------------------------------------------
+// small non-negative big integers, little-endian 32-bit limbs (host only, Step 1)
+// ---------------------------------------------------------------------------------------------
+typedef std::vector<uint32_t> Big;
+
+Big big_from(uint32_t v) { return Big(1, v); }
+
+void big_mul_small(Big &a, uint32_t f)
+{
+    uint64_t carry = 0;
+    for (size_t t = 0; t < a.size(); t++) {
+        uint64_t s = (uint64_t)a[t] * f + carry;
+        a[t] = (uint32_t)s;
+        carry = s >> 32;
+    }
+    if (carry) a.push_back((uint32_t)carry);
+}
+
+uint32_t big_mod_small(const Big &a, uint32_t p)
+{
+    uint64_t r = 0;
+    for (size_t t = a.size(); t-- > 0;) r = ((r << 32) | a[t]) % p;
+    return (uint32_t)r;
+}
+
+Big big_half(const Big &a)
+{
+    Big r(a.size());
+    for (size_t t = 0; t < a.size(); t++) r[t] = (a[t] >> 1) | (t + 1 < a.size() ? a[t + 1] << 31 : 0u);
+    return r;
+}
+
+long double big_to_ld(const Big &a)
+{
+    long double r = 0.0L;
+    for (size_t t = a.size(); t-- > 0;) r = r * 4294967296.0L + (long double)a[t];
+    return r;
+}
+
+void big_store(const Big &a, uint32_t *dst, int words)
+{
+    for (int t = 0; t < words; t++) dst[t] = t < (int)a.size() ? a[t] : 0u;
+}
+
+float f32_round_down(long double x)
+{
+    float f = (float)x;
+    if ((long double)f > x) f = nextafterf(f, -INFINITY);
+    return f;
+}
+float f32_round_up(long double x)
+{
+    float f = (float)x;
+    if ((long double)f < x) f = nextafterf(f, INFINITY);
+    return f;
+}
+
+int words_of_P_host(int N) { return N <= 4 ? 1 : N <= 8 ? 2 : N <= 12 ? 3 : N <= 16 ? 4 : 5; }
+
+struct HostConsts {
+    Oz2HostTables tab;
+    int q[OZ2_MAX_MODULI + 1][OZ2_MAX_MODULI];
+    Big P[OZ2_MAX_MODULI + 1];
+    Big w[OZ2_MAX_MODULI + 1][OZ2_MAX_MODULI];
+};
+
+void build_host_consts(HostConsts &H)
+{
+    memset(&H.tab, 0, sizeof(H.tab));
+    // ---- per-modulus tables
+    for (int l = 0; l < OZ2_MAX_MODULI; l++) {
+        Oz2ModTab &t = H.tab.mod[l];
+        const uint32_t p = (uint32_t)kModuli[l];
+        t.p = p;
+        t.magic = (uint32_t)(0x100000000ull / p) + 1u;
+        t.half = (p - 1) / 2;
+        uint32_t pw = 1 % p;                               // 256^i mod p
+        for (int i = 0; i < 12; i++) {
+            t.wb[i / 4] |= pw << (8 * (i % 4));
+            pw = (pw * 256u) % p;
+        }
+        t.conv_bias = 0;
+        t.w16 = 65536u % p;
+        t.epi_bias = ((32768u * t.w16 + p - 1) / p) * p;   // multiple of p, >= 2^15 w16
+    }
+    // ---- per-N tables
+    for (int N = OZAKI2_MIN_MODULI; N <= OZ2_MAX_MODULI; N++) {
+        Oz2CrtTab &c = H.tab.crt[N];
+        Big P = big_from(1);
+        for (int l = 0; l < N; l++) big_mul_small(P, (uint32_t)kModuli[l]);
+        H.P[N] = P;
+        const int nw = words_of_P_host(N);
+        c.nw = nw;
+        big_store(P, c.P, OZ2_MAX_WORDS);
+        big_store(big_half(P), c.Phalf, OZ2_MAX_WORDS);
+        for (int l = 0; l < N; l++) {
+            Big Pl = big_from(1);
+            for (int j = 0; j < N; j++)
+                if (j != l) big_mul_small(Pl, (uint32_t)kModuli[j]);
+            const uint32_t p = (uint32_t)kModuli[l];
+            const uint32_t r = big_mod_small(Pl, p);
+            uint32_t q = 0;
+            for (uint32_t x = 1; x < p; x++)
+                if ((r * x) % p == 1u) { q = x; break; }
+            H.q[N][l] = (int)q;
+            big_mul_small(Pl, q);                           // w_l = P_l q_l
+            H.w[N][l] = Pl;
+            big_store(Pl, c.w[l], OZ2_MAX_WORDS);
+        }
+        const long double Pld = big_to_ld(P);
+        c.invP = (double)(ldexpl(1.0L, 32 * (nw - 1)) / Pld);
+        Big Pm1 = P;
+        Pm1[0] -= 1;                                        // P is a multiple of 256: no borrow
+        const long double l2 = log2l(big_to_ld(Pm1));
+        c.Pprop = f32_round_down(l2 / 2.0L - 0.5L);         // P:326-328 (= P'_accu)
+        c.Pfast = f32_round_down(l2 / 2.0L - 1.5L);
+        c.delta = f32_round_up(0.5L / (1.0L - ldexpl(1.0L, -22)));   // eq. (6)
+    }
+}
+
+HostConsts &host_consts()
+{
+    static HostConsts H;
+    static std::once_flag once;
+    std::call_once(once, [] { build_host_consts(H); });
+    return H;
+}
+
+// ---------------------------------------------------------------------------------------------
+// per-device state
+// ---------------------------------------------------------------------------------------------
+constexpr int kMaxDevices = 64;
+struct DeviceState {
+    bool tables_ready = false;
+    bool checked = false;
+    bool is_sm100 = false;
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+};
+DeviceState g_dev[kMaxDevices];
+std::mutex g_mu;
+
+int ensure_device(DeviceState **out)
+{
+    int dev = 0;
+    OZ2_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return OZAKI2_ERR_DEVICE;
+    std::lock_guard<std::mutex> lk(g_mu);
+    DeviceState &d = g_dev[dev];
+    if (!d.checked) {
+        int major = 0;
+        OZ2_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        d.is_sm100 = (major == 10);
+        d.checked = true;
+    }
+    if (!d.is_sm100) return OZAKI2_ERR_DEVICE;
+    if (!d.tables_ready) {
+        const Oz2HostTables &t = host_consts().tab;
+        int rc;
+        if ((rc = oz2_scale_upload_tables(t))) return rc;
+        if ((rc = oz2_convert_upload_tables(t))) return rc;
+        if ((rc = oz2_gemm_upload_tables(t))) return rc;
+        if ((rc = oz2_crt_upload_tables(t))) return rc;
+        d.tables_ready = true;
+    }
+    *out = &d;
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// workspace layout
+// ---------------------------------------------------------------------------------------------
+struct Layout {
+    int64_t kp, mp;
+    size_t off_e, off_f, off_amax, off_ssq, off_EA, off_EB, off_rowmax, off_colmax, off_RA, off_RB, off_U, off_Abar,
+        off_Bbar, total;
+};
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+Layout make_layout(int64_t m, int64_t n, int64_t k, int N, int mode)
+{
+    Layout L;
+    L.kp = oz2_round_up(k > 0 ? k : 1, 128);
+    L.mp = oz2_round_up(m > 0 ? m : 1, 16);
+    size_t o = 0;
+    L.off_e = o;      o = align_up(o + 4 * (size_t)m);
+    L.off_f = o;      o = align_up(o + 4 * (size_t)n);
+    L.off_amax = o;   o = align_up(o + 8 * (size_t)m);
+    L.off_ssq = o;    o = align_up(o + 8 * (size_t)m);
+    L.off_EA = o;     o = align_up(o + 4 * (size_t)m);
+    L.off_EB = o;     o = align_up(o + 4 * (size_t)n);
+    L.off_rowmax = o; o = align_up(o + 4 * (size_t)m);
+    L.off_colmax = o; o = align_up(o + 4 * (size_t)n);
+    L.off_RA = o;     o = align_up(o + (size_t)N * m * L.kp);
+    L.off_RB = o;     o = align_up(o + (size_t)N * n * L.kp);
+    L.off_U = o;      o = align_up(o + (size_t)N * n * L.mp);
+    L.off_Abar = o;
+    L.off_Bbar = o;
+    if (mode == OZAKI2_MODE_ACCURATE) {
+        o = align_up(o + (size_t)m * L.kp);
+        L.off_Bbar = o;
+        o = align_up(o + (size_t)n * L.kp);
+    }
+    L.total = o;
+    return L;
+}
+
+// widths: fast / prop  <= floor(P'_prop) + 1 bits, accurate <= floor(P'_accu) + 7 bits; two dp4a words hold 64
+bool needs_wide_words(int N, int mode)
+{
+    const float Pp = host_consts().tab.crt[N].Pprop;
+    const int width = (int)floorf(Pp) + (mode == OZAKI2_MODE_ACCURATE ? 7 : 1);
+    return width > 64;
+}
+
+int check_args(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B, int64_t ldb,
+               const double *C, int64_t ldc, int N, int mode)
+{
+    if (m < 0) return -1;
+    if (n < 0) return -2;
+    if (k < 0 || k > OZAKI2_MAX_K) return -3;
+    if (m > 0 && k > 0 && !A) return -5;
+    if (lda < (m > 1 ? m : 1)) return -6;
+    if (n > 0 && k > 0 && !B) return -7;
+    if (ldb < (k > 1 ? k : 1)) return -8;
+    if (m > 0 && n > 0 && !C) return -10;
+    if (ldc < (m > 1 ? m : 1)) return -11;
+    if (N < OZAKI2_MIN_MODULI || N > OZAKI2_MAX_MODULI) return -12;
+    if (mode != OZAKI2_MODE_ACCURATE && mode != OZAKI2_MODE_FAST && mode != OZAKI2_MODE_PROP) return -13;
+    if (m > 0x7FFFFFFFll - 1024 || n > 0x7FFFFFFFll - 1024) return m > n ? -1 : -2;
+    return 0;
+}
+
+__global__ void k_scale_c(int64_t m, int64_t n, double beta, double *C, int64_t ldc)
+{
+    int64_t i = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
+    int64_t j = blockIdx.x;
+    if (i < m) {
+        double *p = C + i + j * ldc;
+        *p = beta == 0.0 ? 0.0 : beta * *p;
+    }
+}
+
+} // namespace
+
+// =============================================================================================
+// the path
+// =============================================================================================
+static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
+                    int64_t ldb, double beta, double *C, int64_t ldc, int N, int mode, cudaStream_t st,
+                    const ozaki2_stage_outputs *out)
+{
+    int rc = check_args(m, n, k, A, lda, B, ldb, C, ldc, N, mode);
+    if (rc) return rc;
+    if (m == 0 || n == 0) return 0;
+    DeviceState *dev = nullptr;
+    if ((rc = ensure_device(&dev))) return rc;
+    if (k == 0 || alpha == 0.0) {
+        // C := beta C (zeros if beta == 0, BLAS rule)
+        if (!(beta == 1.0)) {
+            k_scale_c<<<dim3((unsigned)n, (unsigned)((m + 255) / 256)), 256, 0, st>>>(m, n, beta, C, ldc);
+            OZ2_CUDA_TRY(cudaGetLastError());
+        }
+        return 0;
+    }
+    const Layout L = make_layout(m, n, k, N, mode);
+    if (!dev->ws || dev->ws_bytes < L.total) return OZAKI2_ERR_WORKSPACE;
+    uint8_t *ws = static_cast<uint8_t *>(dev->ws);
+    int32_t *e = reinterpret_cast<int32_t *>(ws + L.off_e), *f = reinterpret_cast<int32_t *>(ws + L.off_f);
+    unsigned long long *amax = reinterpret_cast<unsigned long long *>(ws + L.off_amax);
+    unsigned long long *ssq = reinterpret_cast<unsigned long long *>(ws + L.off_ssq);
+    int32_t *EA = reinterpret_cast<int32_t *>(ws + L.off_EA), *EB = reinterpret_cast<int32_t *>(ws + L.off_EB);
+    int32_t *rowmax = reinterpret_cast<int32_t *>(ws + L.off_rowmax), *colmax = reinterpret_cast<int32_t *>(ws + L.off_colmax);
+    int8_t *RA = reinterpret_cast<int8_t *>(ws + L.off_RA), *RB = reinterpret_cast<int8_t *>(ws + L.off_RB);
+    uint8_t *U = ws + L.off_U;
+
+    cudaEvent_t ev[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };
+    const bool timing = out && out->stage_ms;
+    if (timing) {
+        for (int t = 0; t < 5; t++) OZ2_CUDA_TRY(cudaEventCreate(&ev[t]));
+        OZ2_CUDA_TRY(cudaEventRecord(ev[0], st));
+    }
+    // ---- S1 scaling
+    if (mode == OZAKI2_MODE_ACCURATE) {
+        int8_t *Abar = reinterpret_cast<int8_t *>(ws + L.off_Abar), *Bbar = reinterpret_cast<int8_t *>(ws + L.off_Bbar);
+        if ((rc = oz2_launch_scale_accu_prepare(m, n, k, A, lda, B, ldb, amax, EA, EB, Abar, Bbar, L.kp, rowmax, colmax, st))) return rc;
+        if ((rc = oz2_launch_gemm_tc(1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
+        if ((rc = oz2_launch_scale_accu_finish(N, m, n, EA, EB, rowmax, colmax, e, f, st))) return rc;
+    } else {
+        if ((rc = oz2_launch_scale_fastprop(mode, N, m, n, k, A, lda, B, ldb, amax, ssq, e, f, st))) return rc;
+    }
+    if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[1], st));
+    // ---- S2 conversion
+    const int wide = needs_wide_words(N, mode) ? 1 : 0;
+    if ((rc = oz2_launch_convert(0, N, wide, m, k, A, lda, e, RA, L.kp, st))) return rc;
+    if ((rc = oz2_launch_convert(1, N, wide, n, k, B, ldb, f, RB, L.kp, st))) return rc;
+    if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[2], st));
+    // ---- S3 residue GEMMs
+    if ((rc = oz2_launch_gemm_tc(N, 0, m, n, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
+    if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[3], st));
+    // ---- S4 + S5
+    if ((rc = oz2_launch_crt(N, m, n, U, L.mp, e, f, alpha, beta, C, ldc, out ? out->Cpp : nullptr, st))) return rc;
+    if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[4], st));
+
+    if (out) {
+        if (out->e) OZ2_CUDA_TRY(cudaMemcpyAsync(out->e, e, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
+        if (out->f) OZ2_CUDA_TRY(cudaMemcpyAsync(out->f, f, 4 * (size_t)n, cudaMemcpyDeviceToDevice, st));
+        if (mode == OZAKI2_MODE_ACCURATE) {
+            if (out->rowmax) OZ2_CUDA_TRY(cudaMemcpyAsync(out->rowmax, rowmax, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
+            if (out->colmax) OZ2_CUDA_TRY(cudaMemcpyAsync(out->colmax, colmax, 4 * (size_t)n, cudaMemcpyDeviceToDevice, st));
+        }
+        // pitched internal planes -> canonical dense layouts
+        if (out->resA)
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(out->resA, (size_t)k, RA, (size_t)L.kp, (size_t)k, (size_t)N * m, cudaMemcpyDeviceToDevice, st));
+        if (out->resB)
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(out->resB, (size_t)k, RB, (size_t)L.kp, (size_t)k, (size_t)N * n, cudaMemcpyDeviceToDevice, st));
+        if (out->U)
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(out->U, (size_t)m, U, (size_t)L.mp, (size_t)m, (size_t)N * n, cudaMemcpyDeviceToDevice, st));
+        if (timing) {
+            OZ2_CUDA_TRY(cudaStreamSynchronize(st));
+            for (int t = 0; t < 4; t++) OZ2_CUDA_TRY(cudaEventElapsedTime(out->stage_ms + t, ev[t], ev[t + 1]));
+            OZ2_CUDA_TRY(cudaEventElapsedTime(out->stage_ms + 4, ev[0], ev[4]));
+            for (int t = 0; t < 5; t++) cudaEventDestroy(ev[t]);
+        }
+    }
+    return 0;
+}
+
+extern "C" {
+
+int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
+                 int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream)
+{
+    return run_path(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+                    static_cast<cudaStream_t>(stream), nullptr);
+}
+
+int ozaki2_dgemm_stages(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
+                        int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream,
+                        const ozaki2_stage_outputs *out)
+{
+    return run_path(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+                    static_cast<cudaStream_t>(stream), out);
+}
+
+size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode)
+{
+    if (m < 0 || n < 0 || k < 0 || k > OZAKI2_MAX_K) return 0;
+    if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return 0;
+    if (scaling_mode < 0 || scaling_mode > 2) return 0;
+    return make_layout(m, n, k, num_moduli, scaling_mode).total;
+}
+
+int ozaki2_set_workspace(void *device_ptr, size_t bytes)
+{
+    int dev = 0;
+    OZ2_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return OZAKI2_ERR_DEVICE;
+    if (device_ptr && (reinterpret_cast<uintptr_t>(device_ptr) & 255)) return -1;
+    if (!device_ptr && bytes) return -2;
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_dev[dev].ws = device_ptr;
+    g_dev[dev].ws_bytes = device_ptr ? bytes : 0;
+    return 0;
+}
+
+size_t ozaki2_host_scratch_bytes(int64_t m, int64_t n, int64_t k)
+{
+    if (m < 0 || n < 0 || k < 0) return 0;
+    return align_up(8 * (size_t)m * k) + align_up(8 * (size_t)k * n) + align_up(8 * (size_t)m * n);
+}
+
+int ozaki2_dgemm_host(int64_t m, int64_t n, int64_t k, double alpha, const double *A_host, int64_t lda,
+                      const double *B_host, int64_t ldb, double beta, double *C_host, int64_t ldc, int num_moduli,
+                      int scaling_mode, void *device_scratch, size_t scratch_bytes, void *stream)
+{
+    int rc = check_args(m, n, k, A_host, lda, B_host, ldb, C_host, ldc, num_moduli, scaling_mode);
+    if (rc) return rc;
+    if (m == 0 || n == 0) return 0;
+    if (!device_scratch || scratch_bytes < ozaki2_host_scratch_bytes(m, n, k)) return -15;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    uint8_t *base = static_cast<uint8_t *>(device_scratch);
+    double *dA = reinterpret_cast<double *>(base);
+    double *dB = reinterpret_cast<double *>(base + align_up(8 * (size_t)m * k));
+    double *dC = reinterpret_cast<double *>(base + align_up(8 * (size_t)m * k) + align_up(8 * (size_t)k * n));
+    if (k > 0) {
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, 8 * (size_t)m, A_host, 8 * (size_t)lda, 8 * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, st));
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB, 8 * (size_t)k, B_host, 8 * (size_t)ldb, 8 * (size_t)k, (size_t)n, cudaMemcpyHostToDevice, st));
+    }
+    if (beta != 0.0)
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC, 8 * (size_t)m, C_host, 8 * (size_t)ldc, 8 * (size_t)m, (size_t)n, cudaMemcpyHostToDevice, st));
+    rc = run_path(m, n, k, alpha, dA, m > 1 ? m : 1, dB, k > 1 ? k : 1, beta, dC, m > 1 ? m : 1, num_moduli, scaling_mode, st, nullptr);
+    if (rc) return rc;
+    OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host, 8 * (size_t)ldc, dC, 8 * (size_t)m, 8 * (size_t)m, (size_t)n, cudaMemcpyDeviceToHost, st));
+    OZ2_CUDA_TRY(cudaStreamSynchronize(st));
+    return 0;
+}
+
+const char *ozaki2_status_string(int status)
+{
+    static const char *arg_names[] = { "",      "m",   "n",    "k", "alpha",      "A",           "lda",   "B",
+                                       "ldb",   "beta", "C",   "ldc", "num_moduli", "scaling_mode", "stream", "scratch" };
+    static thread_local char buf[96];
+    if (status == 0) return "success";
+    if (status == OZAKI2_ERR_WORKSPACE) return "workspace missing or too small (ozaki2_set_workspace)";
+    if (status == OZAKI2_ERR_DEVICE) return "current device is not sm_100 (B200)";
+    if (status < 0 && status >= -15) {
+        snprintf(buf, sizeof buf, "invalid argument %d (%s)", -status, arg_names[-status]);
+        return buf;
+    }
+    if (status > 0) return cudaGetErrorString(static_cast<cudaError_t>(status));
+    return "unknown status";
+}
+
+int ozaki2_get_constants(int num_moduli, int32_t *p, int32_t *q, uint64_t *P_words, uint64_t *w_words, float *Pprop,
+                         float *Pfast, float *delta)
+{
+    if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return -1;
+    HostConsts &H = host_consts();
+    const int N = num_moduli;
+    auto pack = [](const Big &b, uint64_t *dst) {
+        for (int t = 0; t < 4; t++) {
+            uint64_t lo = 2 * t < (int)b.size() ? b[2 * t] : 0, hi = 2 * t + 1 < (int)b.size() ? b[2 * t + 1] : 0;
+            dst[t] = lo | (hi << 32);
+        }
+    };
+    for (int l = 0; l < N; l++) {
+        if (p) p[l] = kModuli[l];
+        if (q) q[l] = H.q[N][l];
+        if (w_words) pack(H.w[N][l], w_words + 4 * l);
+    }
+    if (P_words) pack(H.P[N], P_words);
+    if (Pprop) *Pprop = H.tab.crt[N].Pprop;
+    if (Pfast) *Pfast = H.tab.crt[N].Pfast;
+    if (delta) *delta = H.tab.crt[N].delta;
+    return 0;
+}
+
+int ozaki2_debug_log2f(const float *x, float *y, int64_t count, void *stream)
+{
+    DeviceState *dev = nullptr;
+    int rc = ensure_device(&dev);
+    if (rc) return rc;
+    if (count < 0) return -3;
+    return oz2_launch_log2f(x, y, count, static_cast<cudaStream_t>(stream));
+}
+
+int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64_t count, void *stream)
+{
+    DeviceState *dev = nullptr;
+    int rc = ensure_device(&dev);
+    if (rc) return rc;
+    if (modulus_index < 0 || modulus_index >= OZ2_MAX_MODULI) return -1;
+    if (count < 0) return -4;
+    return oz2_launch_mod_p(modulus_index, in, out, count, static_cast<cudaStream_t>(stream));
+}
+
+int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA, const int8_t *resB,
+                              uint8_t *U, int use_tensor_cores, void *stream)
+{
+    DeviceState *dev = nullptr;
+    int rc = ensure_device(&dev);
+    if (rc) return rc;
+    if (num_moduli < 1 || num_moduli > OZAKI2_MAX_MODULI) return -1;
+    if (m < 0) return -2;
+    if (n < 0) return -3;
+    if (k <= 0 || k % 128 != 0 || k > OZAKI2_MAX_K) return -4;      // canonical planes are used in place: pitch = k
+    if (m % 16 != 0) return -2;                                     // U pitch = m
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (use_tensor_cores) return oz2_launch_gemm_tc(num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
+    return oz2_launch_gemm_check(num_moduli, m, n, k, resA, resB, k, U, m, st);
+}
+
+const char *ozaki2_version(void) { return "ozaki2 0.1 sm_100a tcgen05.kind::i8 (arxiv/paper_2606_29129)"; }
+
+} // extern "C"

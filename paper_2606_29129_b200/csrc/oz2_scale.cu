@@ -1,0 +1,374 @@
+// oz2_scale.cu -- S1: the scaling vectors mu_i = 2^e_i (rows of A), nu_j = 2^f_j (columns of B).
+//
+//   mode 2  revised fast mode, Algorithm 2, eq. (17)(18)
+//   mode 1  original fast mode, Algorithm 1, eq. (11)(12)
+//   mode 0  accurate mode, eq. (4)-(9): max exponents, Abar/Bbar = ceil(mu'|a|);
+//           the auxiliary INT8 GEMM itself runs in oz2_gemm.cu with a row/column-max epilogue.
+//
+// Readings: R2 the sum of squares is the exact integer sum_h ceil(2^44 (v_h / 2^E)^2) -- order
+// independent, so it can be accumulated with integer atomics; R3 __log2f is replaced by the correctly
+// rounded RN_32(log2 x); R10/R11 directed roundings and the normalised form of Algorithm 2.
+//
+// Kernels are HBM-bound streaming reductions: A is column-major, so a warp reads 32 consecutive rows of one
+// column (coalesced) and every thread keeps the statistics of its own row; a column of B is contiguous and is
+// reduced by one block with warp shuffles.
+#include "oz2_common.cuh"
+
+namespace {
+
+__constant__ Oz2CrtTab c_crt[OZ2_MAX_MODULI + 1];
+
+constexpr int ROWS_PER_BLOCK = 128;   // consecutive rows of A per block (1 KB contiguous per column)
+constexpr int KSLICES = 2;            // h-interleaved slices inside a block
+constexpr int COL_THREADS = 256;
+constexpr int32_t OZ2_E_ZERO = INT32_MIN;   // marks an all-zero row / column in the E arrays of accurate mode
+
+__device__ __forceinline__ unsigned long long abs_bits(double v)
+{
+    return (unsigned long long)__double_as_longlong(v) & 0x7FFFFFFFFFFFFFFFull;
+}
+
+// floor(log2 v) for the positive finite double with bit pattern `b` (true value for subnormals)
+__device__ __forceinline__ int floor_log2_bits(unsigned long long b)
+{
+    int be = (int)(b >> 52);
+    if (be) return be - 1023;
+    return (63 - __clzll((long long)b)) - 1074;
+}
+
+// |v| = M 2^q, M < 2^53 integer
+__device__ __forceinline__ void decompose(unsigned long long b, unsigned long long &M, int &q)
+{
+    int be = (int)(b >> 52);
+    unsigned long long mant = b & 0x000FFFFFFFFFFFFFull;
+    M = be ? (mant | 0x0010000000000000ull) : mant;
+    q = (be ? be : 1) - 1075;
+}
+
+// T = ceil(2^44 (v / 2^E)^2) for |v| < 2^(E+1): exact.  (reading R2)
+__device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int E)
+{
+    if (b == 0) return 0;
+    unsigned long long M;
+    int q;
+    decompose(b, M, q);
+    // 2^44 (v/2^E)^2 = M^2 2^-s, s = 2 (E - q) - 44 >= 60.  With M5 = M << 5: M5^2 = M^2 2^10, so
+    // floor(M^2 2^-s) = floor(hi64(M5^2) 2^-(s - 54)), and the dropped bits are non-zero iff 2 ctz(M) < s.
+    int s = 2 * (E - q) - 44;
+    unsigned long long M5 = M << 5;
+    unsigned long long hi = __umul64hi(M5, M5);
+    int r = s - 54;                                   // >= 6
+    unsigned long long fl = r < 64 ? (hi >> r) : 0ull;
+    int tz = __ffsll((long long)M) - 1;
+    return fl + ((2 * tz < s) ? 1ull : 0ull);
+}
+
+// LOG2F(x) = RN_32(log2 x) for float x in [1,2] (reading R3): FP64 log2 (<= 1 ulp), rounded once.
+__device__ __forceinline__ float log2f_rn(float x) { return __double2float_rn(log2((double)x)); }
+
+// Algorithm 2 (mode 2) / Algorithm 1 (mode 1) on the statistics (E, S) of one row or column.
+__device__ int exponent_fastprop(int mode, const Oz2CrtTab &c, unsigned long long amax, unsigned long long S)
+{
+    if (amax == 0) return 0;                                            // reading R4
+    int E = floor_log2_bits(amax);
+    float F = __ull2float_ru(S);                                        // "rounding-up"
+    int fb = __float_as_int(F);
+    int shat = ((fb >> 23) - 127) - 44;                                 // floor(log2 F) - 44
+    float x = __int_as_float((fb & 0x007FFFFF) | 0x3F800000);           // F / 2^floor(log2 F) in [1,2)
+    float L = log2f_rn(x);
+    if (mode == 2) {
+        float t = __fmaf_ru(0.5f, L, 1.1920928955078125e-07f);          // single_up(0.5 __log2f(.) + 2 u32)
+        float w = __fsub_rd(c.Pprop, 0.5f * (float)shat);               // single_down(P'_prop - 0.5 s)
+        float d = __fsub_rd(w, t);
+        return (int)floorf(d) - E;
+    } else {
+        int s = shat + 2 * E;                                           // floor(log2 a_norm), raw sum
+        float inner = __fadd_ru(L, (float)s);
+        float t = __fmul_ru(c.delta, inner);                            // single_up(delta (__log2f(.) + s))
+        float d = __fsub_rd(c.Pfast, fmaxf(t, 1.0f));
+        return (int)floorf(d) - E;
+    }
+}
+
+// eq. (8)/(9) with reading G3: e = (5 - E) + floor(P'_accu - delta log2~(max cbar)); log2~ of eq. (7)
+__device__ int exponent_accurate(const Oz2CrtTab &c, int E, int M)
+{
+    if (M < 1) M = 1;
+    float F = __uint2float_ru((unsigned)M);
+    int fb = __float_as_int(F);
+    int s = (fb >> 23) - 127;
+    float x = __int_as_float((fb & 0x007FFFFF) | 0x3F800000);
+    float L = log2f_rn(x);
+    float lg = __fadd_ru(L, (float)s);
+    float prod = __fmul_ru(c.delta, lg);
+    float d = __fsub_rd(c.Pprop, prod);
+    return (5 - E) + (int)floorf(d);
+}
+
+// ---------------------------------------------------------------------------------------------
+// rows of A
+// ---------------------------------------------------------------------------------------------
+template <int PASS> // 0: max |a|   1: sum of squared, normalised terms
+__global__ void __launch_bounds__(ROWS_PER_BLOCK *KSLICES)
+k1_rows(int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, int64_t kchunk,
+        unsigned long long *__restrict__ amax, unsigned long long *__restrict__ ssq)
+{
+    int64_t i = (int64_t)blockIdx.x * ROWS_PER_BLOCK + threadIdx.x;
+    int64_t h0 = (int64_t)blockIdx.y * kchunk;
+    int64_t h1 = h0 + kchunk < k ? h0 + kchunk : k;
+    if (i >= m) return;
+    const double *p = A + i;
+    unsigned long long acc = 0;
+    int E = 0;
+    if (PASS == 1) {
+        unsigned long long mx = amax[i];
+        if (mx == 0) return;
+        E = floor_log2_bits(mx);
+    }
+    int64_t h = h0 + threadIdx.y;
+    for (; h + 7 * KSLICES < h1; h += 8 * KSLICES) {
+        double v[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) v[u] = __ldg(p + (h + u * KSLICES) * lda);
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            unsigned long long b = abs_bits(v[u]);
+            if (PASS == 0) acc = b > acc ? b : acc;
+            else acc += sq_term(b, E);
+        }
+    }
+    for (; h < h1; h += KSLICES) {
+        unsigned long long b = abs_bits(__ldg(p + h * lda));
+        if (PASS == 0) acc = b > acc ? b : acc;
+        else acc += sq_term(b, E);
+    }
+    if (PASS == 0) { if (acc) atomicMax(amax + i, acc); }
+    else if (acc) atomicAdd(ssq + i, acc);
+}
+
+__global__ void k1_rows_finalize(int mode, int N, int64_t m, const unsigned long long *__restrict__ amax,
+                                 const unsigned long long *__restrict__ ssq, int32_t *__restrict__ e)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) e[i] = exponent_fastprop(mode, c_crt[N], amax[i], ssq[i]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// columns of B: one block per column
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long block_reduce(unsigned long long v, bool is_max, unsigned long long *sm)
+{
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+        unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = is_max ? (w > v ? w : v) : v + w;
+    }
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) sm[warp] = v;
+    __syncthreads();
+    unsigned long long r = sm[0];
+    for (int w = 1; w < COL_THREADS / 32; w++) r = is_max ? (sm[w] > r ? sm[w] : r) : r + sm[w];
+    return r;
+}
+
+// MODE 1/2: f[j]; MODE 0 (accurate prepare): EB[j] only
+template <bool ACCU>
+__global__ void __launch_bounds__(COL_THREADS)
+k1_cols(int mode, int N, int64_t k, const double *__restrict__ B, int64_t ldb, int32_t *__restrict__ f,
+        int32_t *__restrict__ EB)
+{
+    __shared__ unsigned long long sm[COL_THREADS / 32];
+    const double *col = B + (int64_t)blockIdx.x * ldb;
+    bool vec = ((((uintptr_t)col) & 15) == 0);
+    unsigned long long mx = 0;
+    int64_t kv = vec ? (k & ~(int64_t)1) : 0;
+    for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {
+        double2 v = __ldg(reinterpret_cast<const double2 *>(col + h));
+        unsigned long long b0 = abs_bits(v.x), b1 = abs_bits(v.y);
+        mx = b0 > mx ? b0 : mx;
+        mx = b1 > mx ? b1 : mx;
+    }
+    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) {
+        unsigned long long b = abs_bits(__ldg(col + h));
+        mx = b > mx ? b : mx;
+    }
+    mx = block_reduce(mx, true, sm);
+    if (ACCU) {
+        if (threadIdx.x == 0) EB[blockIdx.x] = mx ? floor_log2_bits(mx) : OZ2_E_ZERO;
+        return;
+    }
+    if (mx == 0) {
+        if (threadIdx.x == 0) f[blockIdx.x] = 0;
+        return;
+    }
+    int E = floor_log2_bits(mx);
+    unsigned long long acc = 0;
+    for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {      // second read: L2 hits
+        double2 v = __ldg(reinterpret_cast<const double2 *>(col + h));
+        acc += sq_term(abs_bits(v.x), E) + sq_term(abs_bits(v.y), E);
+    }
+    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits(__ldg(col + h)), E);
+    acc = block_reduce(acc, false, sm);
+    if (threadIdx.x == 0) f[blockIdx.x] = exponent_fastprop(mode, c_crt[N], mx, acc);
+}
+
+// ---------------------------------------------------------------------------------------------
+// accurate mode: Abar, Bbar as INT8, K-major, pitch kp (zero padded)
+// ---------------------------------------------------------------------------------------------
+// ceil(|a| 2^(5-E)) in [0, 64]
+__device__ __forceinline__ int ceil_scaled(unsigned long long b, int E)
+{
+    if (b == 0) return 0;
+    unsigned long long M;
+    int q;
+    decompose(b, M, q);
+    int r = -(q + 5 - E);                 // value = M 2^-r < 64, r >= 47
+    if (r >= 64) return 1;
+    unsigned long long fl = M >> r;
+    return (int)fl + ((M & ((1ull << r) - 1)) != 0);
+}
+
+__global__ void k1_rows_E(int64_t m, const unsigned long long *__restrict__ amax, int32_t *__restrict__ EA)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < m) EA[i] = amax[i] ? floor_log2_bits(amax[i]) : OZ2_E_ZERO;
+}
+
+// thread = one row, 16 consecutive h per iteration -> one 16-byte store
+__global__ void __launch_bounds__(128)
+k1_abar_rows(int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, const int32_t *__restrict__ EA,
+             int8_t *__restrict__ Abar, int64_t kp)
+{
+    int64_t i = (int64_t)blockIdx.x * 128 + threadIdx.x;
+    if (i >= m) return;
+    int E = EA[i];
+    for (int64_t h0 = (int64_t)blockIdx.y * 16; h0 < kp; h0 += (int64_t)gridDim.y * 16) {
+        uint32_t w[4] = { 0, 0, 0, 0 };
+#pragma unroll
+        for (int u = 0; u < 16; u++) {
+            int64_t h = h0 + u;
+            int v = h < k ? ceil_scaled(abs_bits(__ldg(A + i + h * lda)), E) : 0;
+            w[u >> 2] |= (uint32_t)v << (8 * (u & 3));
+        }
+        *reinterpret_cast<uint4 *>(Abar + i * kp + h0) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+
+// thread = 4 consecutive h of one column -> one 4-byte store, coalesced
+__global__ void __launch_bounds__(256)
+k1_bbar_cols(int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, const int32_t *__restrict__ EB,
+             int8_t *__restrict__ Bbar, int64_t kp)
+{
+    int64_t j = blockIdx.x;
+    int E = EB[j];
+    const double *col = B + j * ldb;
+    for (int64_t h0 = 4 * ((int64_t)blockIdx.y * 256 + threadIdx.x); h0 < kp; h0 += 4 * 256 * (int64_t)gridDim.y) {
+        uint32_t w = 0;
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            int64_t h = h0 + u;
+            int v = h < k ? ceil_scaled(abs_bits(__ldg(col + h)), E) : 0;
+            w |= (uint32_t)v << (8 * u);
+        }
+        *reinterpret_cast<uint32_t *>(Bbar + j * kp + h0) = w;
+    }
+}
+
+__global__ void k1_accu_finalize(int N, int64_t cnt, const int32_t *__restrict__ E, const int32_t *__restrict__ mx,
+                                 int32_t *__restrict__ out)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cnt) return;
+    // a zero row / column (E == OZ2_E_ZERO) gets exponent 0 (reading R4)
+    out[i] = E[i] == OZ2_E_ZERO ? 0 : exponent_accurate(c_crt[N], E[i], mx[i]);
+}
+
+__global__ void k_log2f(const float *__restrict__ x, float *__restrict__ y, int64_t count)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < count) y[t] = log2f_rn(x[t]);
+}
+
+int rows_grid_y(int64_t m, int64_t k, int64_t *kchunk)
+{
+    int64_t bx = (m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK;
+    int64_t want = (148 * 8 + bx - 1) / bx;               // >= 8 blocks per SM overall
+    int64_t maxy = (k + 16 * KSLICES - 1) / (16 * KSLICES);
+    if (want > maxy) want = maxy;
+    if (want < 1) want = 1;
+    if (want > 65535) want = 65535;
+    int64_t kc = (k + want - 1) / want;
+    kc = oz2_round_up(kc, 8 * KSLICES);
+    *kchunk = kc;
+    return (int)((k + kc - 1) / kc);
+}
+
+} // namespace
+
+int oz2_scale_upload_tables(const Oz2HostTables &t)
+{
+    OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_crt, t.crt, sizeof(t.crt)));
+    return 0;
+}
+
+int oz2_launch_scale_fastprop(int mode, int N, int64_t m, int64_t n, int64_t k, const double *A, int64_t lda,
+                              const double *B, int64_t ldb, unsigned long long *amaxA, unsigned long long *ssqA,
+                              int32_t *e, int32_t *f, cudaStream_t st)
+{
+    OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
+    OZ2_CUDA_TRY(cudaMemsetAsync(ssqA, 0, sizeof(unsigned long long) * (size_t)m, st));
+    int64_t kchunk;
+    int gy = rows_grid_y(m, k, &kchunk);
+    dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
+    k1_rows<0><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
+    k1_rows<1><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
+    k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e);
+    k1_cols<false><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, B, ldb, f, nullptr);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B,
+                                  int64_t ldb, unsigned long long *amaxA, int32_t *EA, int32_t *EB, int8_t *Abar,
+                                  int8_t *Bbar, int64_t kp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
+{
+    OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
+    OZ2_CUDA_TRY(cudaMemsetAsync(rowmax, 0, sizeof(int32_t) * (size_t)m, st));
+    OZ2_CUDA_TRY(cudaMemsetAsync(colmax, 0, sizeof(int32_t) * (size_t)n, st));
+    int64_t kchunk;
+    int gy = rows_grid_y(m, k, &kchunk);
+    dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
+    k1_rows<0><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, nullptr);
+    k1_rows_E<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(m, amaxA, EA);
+    k1_cols<true><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, B, ldb, nullptr, EB);
+    int64_t chunks = kp / 16;
+    int64_t bx = (m + 127) / 128;
+    int64_t gyy = (148 * 16 + bx - 1) / bx;
+    if (gyy > chunks) gyy = chunks;
+    if (gyy > 65535) gyy = 65535;
+    if (gyy < 1) gyy = 1;
+    k1_abar_rows<<<dim3((unsigned)bx, (unsigned)gyy), 128, 0, st>>>(m, k, A, lda, EA, Abar, kp);
+    int64_t gx = (kp / 4 + 255) / 256;
+    if (gx > 64) gx = 64;
+    k1_bbar_cols<<<dim3((unsigned)n, (unsigned)gx), 256, 0, st>>>(n, k, B, ldb, EB, Bbar, kp);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA, const int32_t *EB,
+                                 const int32_t *rowmax, const int32_t *colmax, int32_t *e, int32_t *f, cudaStream_t st)
+{
+    k1_accu_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(N, m, EA, rowmax, e);
+    k1_accu_finalize<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, n, EB, colmax, f);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+int oz2_launch_log2f(const float *x, float *y, int64_t count, cudaStream_t st)
+{
+    if (count <= 0) return 0;
+    k_log2f<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(x, y, count);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    return 0;
+}
