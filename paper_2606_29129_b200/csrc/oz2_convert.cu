@@ -28,13 +28,18 @@ __device__ __forceinline__ void scaled_words(double a, int ex, uint32_t (&w)[NB]
     unsigned long long M = be ? (mant | 0x0010000000000000ull) : mant;
     int sh = (be ? be : 1) - 1075 + ex;          // |a| 2^ex = M 2^sh
     uint32_t m0 = (uint32_t)M, m1 = (uint32_t)(M >> 32);
-    if (sh >= 0) {
-        // left shift by 0..31 (the row's largest element has 53 + sh <= 84 bits); larger shifts cannot occur
-        // for finite inputs because every |a| is below 2 * max|row|
-        int s = sh & 31;
-        w[0] = m0 << s;
-        w[1] = __funnelshift_l(m0, m1, s);
-        if (NB == 3) w[2] = __funnelshift_l(m1, 0u, s);
+    if (sh >= 0 && be != 0) {
+        // normal number: left shift by 0..31 (the row's largest element has 53 + sh <= 84 bits, every other
+        // |a| is below twice the largest)
+        w[0] = m0 << sh;
+        w[1] = __funnelshift_l(m0, m1, sh);
+        if (NB == 3) w[2] = __funnelshift_l(m1, 0u, sh);
+    } else if (sh >= 0) {
+        // subnormal number with a short mantissa: the shift can reach 83
+        unsigned long long lo = sh < 64 ? (M << sh) : 0ull;
+        w[0] = (uint32_t)lo;
+        w[1] = (uint32_t)(lo >> 32);
+        if (NB == 3) w[2] = sh == 0 ? 0u : (sh < 64 ? (uint32_t)(M >> (64 - sh)) : (uint32_t)(M << (sh - 64)));
     } else {
         int r = -sh;
         unsigned long long v = r < 64 ? (M >> r) : 0ull;      // dropping magnitude bits = toward zero
@@ -75,7 +80,9 @@ k2_rows(int N, int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, 
     if (i >= m) return;
     const int ex = e[i];
     const int64_t plane_stride = m * kp;
-    for (int64_t h0 = (int64_t)blockIdx.y * 16; h0 < kp; h0 += (int64_t)gridDim.y * 16) {
+    const int64_t chunk = oz2_round_up((kp / 16 + gridDim.y - 1) / gridDim.y, 8) * 16;   // multiple of 128 bytes
+    const int64_t hbeg = (int64_t)blockIdx.y * chunk, hend = hbeg + chunk < kp ? hbeg + chunk : kp;
+    for (int64_t h0 = hbeg; h0 < hend; h0 += 16) {
         uint32_t w[16][NB];
         uint32_t negmask = 0;
 #pragma unroll

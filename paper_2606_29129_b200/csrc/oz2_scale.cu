@@ -52,15 +52,28 @@ __device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int 
     unsigned long long M;
     int q;
     decompose(b, M, q);
-    // 2^44 (v/2^E)^2 = M^2 2^-s, s = 2 (E - q) - 44 >= 60.  With M5 = M << 5: M5^2 = M^2 2^10, so
-    // floor(M^2 2^-s) = floor(hi64(M5^2) 2^-(s - 54)), and the dropped bits are non-zero iff 2 ctz(M) < s.
+    // 2^44 (v/2^E)^2 = M^2 2^-s with s = 2 (E - q) - 44.
     int s = 2 * (E - q) - 44;
-    unsigned long long M5 = M << 5;
-    unsigned long long hi = __umul64hi(M5, M5);
-    int r = s - 54;                                   // >= 6
-    unsigned long long fl = r < 64 ? (hi >> r) : 0ull;
-    int tz = __ffsll((long long)M) - 1;
-    return fl + ((2 * tz < s) ? 1ull : 0ull);
+    if (M >> 52) {
+        // normal number: s >= 60.  With M5 = M << 5: M5^2 = M^2 2^10, so floor(M^2 2^-s) =
+        // floor(hi64(M5^2) 2^-(s - 54)), and the dropped bits are non-zero iff 2 ctz(M) < s.
+        unsigned long long M5 = M << 5;
+        unsigned long long hi = __umul64hi(M5, M5);
+        int r = s - 54;                               // >= 6
+        unsigned long long fl = r < 64 ? (hi >> r) : 0ull;
+        int tz = __ffsll((long long)M) - 1;
+        return fl + ((2 * tz < s) ? 1ull : 0ull);
+    }
+    // subnormal input (M < 2^52): s can be anything, also negative; use the full 128-bit square
+    unsigned long long lo = M * M, hi = __umul64hi(M, M);
+    if (s <= 0) return lo << (-s);                    // exact, the value is at most 2^46
+    if (s < 64) return ((hi << (64 - s)) | (lo >> s)) + ((lo & ((1ull << s) - 1)) ? 1ull : 0ull);
+    if (s < 128) {
+        int r = s - 64;
+        unsigned long long rem = (r ? (hi & ((1ull << r) - 1)) : 0ull) | lo;
+        return (hi >> r) + (rem ? 1ull : 0ull);
+    }
+    return 1ull;
 }
 
 // LOG2F(x) = RN_32(log2 x) for float x in [1,2] (reading R3): FP64 log2 (<= 1 ulp), rounded once.
@@ -223,7 +236,8 @@ __device__ __forceinline__ int ceil_scaled(unsigned long long b, int E)
     unsigned long long M;
     int q;
     decompose(b, M, q);
-    int r = -(q + 5 - E);                 // value = M 2^-r < 64, r >= 47
+    int r = -(q + 5 - E);                 // value = M 2^-r < 64; r >= 47 for normal numbers
+    if (r <= 0) return (int)(M << (-r));  // subnormal with a small mantissa: exact
     if (r >= 64) return 1;
     unsigned long long fl = M >> r;
     return (int)fl + ((M & ((1ull << r) - 1)) != 0);

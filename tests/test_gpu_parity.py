@@ -1,0 +1,226 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs, element by element.
+
+Bar (BASELINE.json north_star): bit-exact on every integer stage -- scaling exponents, INT8 residues,
+per-modulus products mod p_l, the recovered integer C'' -- and max elementwise relative difference
+<= 2^-50 on the final FP64 C.  With alpha = 1, beta = 0 the final C is in fact required bit-identical here
+(C = RN(C'') 2^-(e+f) has a single rounding on both sides).
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import ozaki2_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+TOL_C = 2.0 ** -50
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_29129_b200 as pkg
+    pkg.lib()                       # fails loudly if libozaki2.so is missing
+    return pkg
+
+
+def gpu_stages(B, A, Bm, N, mode, **kw):
+    import torch
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    want = ["e", "f", "resA", "resB", "U", "Cpp"] + (["rowmax", "colmax"] if mode == 0 else [])
+    out = B.dgemm_stages(Ad, Bd, N, mode, want=want, **kw)
+    torch.cuda.synchronize()
+    res = {k: (v.cpu().numpy() if hasattr(v, "cpu") else v) for k, v in out.items()}
+    res["C"] = np.asfortranarray(res["C"].T)
+    res["Cpp"] = res["Cpp"].view(np.uint64)
+    return res
+
+
+def assert_stage_parity(g, o, mode, tag=""):
+    assert np.array_equal(g["e"], o["e"]), f"{tag} e"
+    assert np.array_equal(g["f"], o["f"]), f"{tag} f"
+    if mode == 0:
+        assert np.array_equal(g["rowmax"].astype(np.int64), o["rowmax"]), f"{tag} rowmax"
+        assert np.array_equal(g["colmax"].astype(np.int64), o["colmax"]), f"{tag} colmax"
+    assert np.array_equal(g["resA"], o["RA"]), f"{tag} resA"
+    assert np.array_equal(g["resB"], o["RB"]), f"{tag} resB"
+    assert np.array_equal(g["U"], o["U"]), f"{tag} U"
+    assert np.array_equal(g["Cpp"], o["Cpp"]), f"{tag} C''"
+    assert np.array_equal(g["C"], o["C"]), f"{tag} C"
+    nz = o["C"] != 0
+    if nz.any():
+        assert np.max(np.abs(g["C"][nz] - o["C"][nz]) / np.abs(o["C"][nz])) <= TOL_C
+
+
+# --------------------------------------------------------------------------------------------- config 0
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_config0_128_all_stages(B, mode):
+    A, Bm = W.config_matrices(0)
+    N = 14
+    o = O.stages(A, Bm, N, mode, want_exact=True)
+    g = gpu_stages(B, A, Bm, N, mode)
+    assert_stage_parity(g, o, mode, f"cfg0 mode{mode}")
+    # and against the exact __int128-style product: C'' == A'B' whenever |A'B'| < P/2 (always here)
+    assert o["counts"]["wrong"] == 0
+    assert np.array_equal(g["Cpp"], o["Z"])
+
+
+# --------------------------------------------------------------------------------------------- ragged shapes, all N
+@pytest.mark.parametrize("m,n,k,N,mode", [
+    (200, 77, 333, 14, 2), (1, 1, 1, 2, 2), (129, 257, 127, 9, 1), (37, 300, 1000, 16, 0), (130, 40, 129, 17, 2),
+    (64, 513, 260, 20, 0), (255, 255, 4097, 20, 2), (16, 16, 16, 3, 1), (300, 5, 31, 15, 0), (5, 300, 2049, 8, 2),
+    (260, 260, 100, 12, 2), (128, 256, 128, 4, 2), (131, 100, 777, 5, 0), (100, 131, 64, 18, 1), (77, 77, 77, 13, 2),
+    (33, 65, 640, 6, 2), (90, 70, 50, 7, 1), (70, 90, 150, 10, 0), (50, 60, 70, 11, 2), (61, 67, 71, 19, 0),
+])
+def test_ragged_shapes_and_every_moduli_count(B, m, n, k, N, mode):
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 1000 + m + n + k + N)
+    o = O.stages(A, Bm, N, mode)
+    g = gpu_stages(B, A, Bm, N, mode)
+    assert_stage_parity(g, o, mode, f"{m}x{n}x{k} N{N} mode{mode}")
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("N", [14, 20])
+def test_wide_exponent_inputs_zero_rows_subnormals(B, mode, N):
+    A, Bm = W.wide_exponent_matrices(140, 70, 200, seed=7 + N)
+    A[3, :] = np.ldexp(1.0, -1074)
+    A[4, :5] = 5e-324
+    o = O.stages(A, Bm, N, mode)
+    g = gpu_stages(B, A, Bm, N, mode)
+    assert_stage_parity(g, o, mode, f"wide N{N} mode{mode}")
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_structured_inputs(B, mode):
+    for A, Bm in (W.all_ones_scaled(130, 60, 256, 2.0 ** -4), W.small_integer_matrices(50, 40, 300, 8, 5),
+                  (np.asfortranarray(np.eye(64)), W.eq15_matrices(64, 32, 64, 2.0, 3)[1])):
+        o = O.stages(A, Bm, 20, mode)
+        g = gpu_stages(B, A, Bm, 20, mode)
+        assert_stage_parity(g, o, mode, "structured")
+
+
+# --------------------------------------------------------------------------------------------- alpha / beta, lda
+def test_alpha_beta_and_leading_dimensions(B):
+    import torch
+    m, n, k, N = 70, 50, 90, 14
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 77)
+    lda, ldb, ldc = m + 3, k + 5, m + 7
+    Ap = np.zeros((lda, k), order="F"); Ap[:m] = A
+    Bp = np.zeros((ldb, n), order="F"); Bp[:k] = Bm
+    rng = np.random.Generator(np.random.PCG64(3))
+    Cin = np.asfortranarray(rng.standard_normal((ldc, n)))
+    Ad, Bd, Cd = B.colmajor_to_device(Ap), B.colmajor_to_device(Bp), B.colmajor_to_device(Cin)
+    B.ensure_workspace(m, n, k, N, 2)
+    for alpha, beta in ((0.7, -1.3), (1.0, 0.0), (-2.0, 1.0), (0.0, 0.5), (0.0, 0.0)):
+        Cd.copy_(B.colmajor_to_device(Cin))
+        rc = B.ozaki2_dgemm(m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, 2)
+        assert rc == 0
+        torch.cuda.synchronize()
+        got = B.device_to_colmajor(Cd)
+        if alpha == 0.0:
+            want = np.zeros((m, n)) if beta == 0.0 else beta * Cin[:m]
+        else:
+            want = O.dgemm(A, Bm, N, 2, alpha=alpha, beta=beta, C_in=Cin[:m].copy())
+        assert np.array_equal(got[:m], want), (alpha, beta)
+        assert np.array_equal(got[m:], Cin[m:])               # rows beyond m untouched
+    # beta == 0 must overwrite NaNs (BLAS rule)
+    Cd.fill_(float("nan"))
+    assert B.ozaki2_dgemm(m, n, k, 1.0, Ad, lda, Bd, ldb, 0.0, Cd, ldc, N, 2) == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(B.device_to_colmajor(Cd)[:m], O.dgemm(A, Bm, N, 2))
+
+
+def test_workspace_errors(B):
+    import torch
+    A, Bm = W.eq15_matrices(64, 64, 64, 0.5, 1)
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    Cd = torch.empty((64, 64), dtype=torch.float64, device="cuda")
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    assert B.ozaki2_set_workspace(small, small.numel()) == 0
+    assert B.ozaki2_dgemm(64, 64, 64, 1.0, Ad, 64, Bd, 64, 0.0, Cd, 64, 14, 2) == B.OZAKI2_ERR_WORKSPACE
+    assert B.ozaki2_set_workspace(None, 0) == 0
+    assert B.ozaki2_dgemm(64, 64, 64, 1.0, Ad, 64, Bd, 64, 0.0, Cd, 64, 14, 2) == B.OZAKI2_ERR_WORKSPACE
+    B.ensure_workspace(64, 64, 64, 14, 2)
+    assert B.ozaki2_dgemm(64, 64, 64, 1.0, Ad, 64, Bd, 64, 0.0, Cd, 64, 14, 2) == 0
+    torch.cuda.synchronize()
+
+
+def test_host_buffer_entry_point(B):
+    import torch
+    m, n, k, N = 96, 80, 200, 15
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 5)
+    B.ensure_workspace(m, n, k, N, 2)
+    nbytes = B.ozaki2_host_scratch_bytes(m, n, k)
+    scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    Ch = np.zeros((m, n), order="F")
+    rc = B.ozaki2_dgemm_host(m, n, k, 1.0, A, m, Bm, k, 0.0, Ch, m, N, 2, scratch, nbytes)
+    assert rc == 0
+    assert np.array_equal(Ch, O.dgemm(A, Bm, N, 2))
+
+
+# --------------------------------------------------------------------------------------------- primitives
+def test_log2f_exhaustive_equals_oracle(B):
+    import torch
+    bits = np.arange(0x3F800000, 0x40000000 + 1, dtype=np.uint32)
+    x = bits.view(np.float32)
+    xd = torch.from_numpy(x.copy()).cuda()
+    yd = torch.empty_like(xd)
+    assert B.ozaki2_debug_log2f(xd, yd, x.size) == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(yd.cpu().numpy(), O.log2f_array(x))
+
+
+def test_epilogue_mod_p_all_moduli(B):
+    import torch
+    rng = np.random.Generator(np.random.PCG64(9))
+    v = np.concatenate([rng.integers(-2 ** 31, 2 ** 31, size=1 << 22, dtype=np.int64),
+                        np.array([-2 ** 31, 2 ** 31 - 1, -1, 0, 1, 2 ** 16, -2 ** 16, 2 ** 16 - 1, 65535 * 32768], np.int64),
+                        np.arange(-70000, 70000, dtype=np.int64)]).astype(np.int32)
+    vd = torch.from_numpy(v).cuda()
+    od = torch.empty(v.size, dtype=torch.uint8, device="cuda")
+    p = O.constants(20)["p"]
+    for l in range(20):
+        assert B.ozaki2_debug_mod_p(l, vd, od, v.size) == 0
+        torch.cuda.synchronize()
+        assert np.array_equal(od.cpu().numpy(), (v.astype(np.int64) % p[l]).astype(np.uint8)), l
+
+
+@pytest.mark.parametrize("m,n,k,N", [(128, 256, 128, 1), (256, 512, 1024, 3), (384, 272, 2048, 20), (16, 8, 128, 2)])
+def test_residue_gemm_tensor_core_vs_oracle_and_check_kernel(B, m, n, k, N):
+    import torch
+    rng = np.random.Generator(np.random.PCG64(k + N))
+    p = O.constants(20)["p"][:N]
+    RA = np.stack([rng.integers(-(q // 2), (q - 1) // 2 + 1, size=(m, k)) for q in p]).astype(np.int8)
+    RB = np.stack([rng.integers(-(q // 2), (q - 1) // 2 + 1, size=(n, k)) for q in p]).astype(np.int8)
+    want, _ = O.products(max(N, 2), RA if N > 1 else np.concatenate([RA, RA]), RB if N > 1 else np.concatenate([RB, RB]))
+    want = want[:N]
+    RAd, RBd = torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda()
+    for tc in (1, 0):
+        Ud = torch.zeros((N, n, m), dtype=torch.uint8, device="cuda")
+        assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, tc) == 0
+        torch.cuda.synchronize()
+        assert np.array_equal(Ud.cpu().numpy(), want), f"tensor_cores={tc}"
+
+
+def test_int32_accumulator_wraps_at_k_2pow17(B):
+    # reading R6: p = 256 residues of -128 over k = 2^17 give 2^31, which must WRAP (256 | 2^32), not saturate;
+    # the odd moduli stay below 2^31.
+    import torch
+    m, n, k, N = 128, 256, 1 << 17, 2
+    RA = np.zeros((N, m, k), np.int8)
+    RB = np.zeros((N, n, k), np.int8)
+    RA[0] = -128; RB[0] = -128
+    RA[1] = 127; RB[1] = 127
+    RA[0, 5, :7] = 3                      # make one row differ so that the result is not constant
+    want, maxR = O.products(N, RA[:, :8], RB[:, :8])
+    assert maxR == 2 ** 31
+    RAd, RBd = torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda()
+    Ud = torch.zeros((N, n, m), dtype=torch.uint8, device="cuda")
+    assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, 1) == 0
+    torch.cuda.synchronize()
+    got = Ud.cpu().numpy()
+    assert np.array_equal(got[:, :8, :8], want)
+    assert np.all(got[1] == (127 * 127 * k) % 255)
