@@ -103,6 +103,9 @@ typedef struct ozaki2_stage_outputs {
     uint64_t *Cpp;       /* [n][m][4]  C'' as 256-bit two's-complement words, little-endian   */
     float *stage_ms;     /* HOST pointer, [5]: elapsed ms of S1, S2, S3, S4+S5, total; filling
                             it synchronises the stream (profiling only)                       */
+    void **stage_events; /* HOST array of 5 caller-owned cudaEvent_t (timing enabled): recorded on
+                            `stream` before S1 and after S1, S2, S3, S4+S5.  No synchronisation:
+                            the caller reads them with cudaEventElapsedTime after its own sync  */
 } ozaki2_stage_outputs;
 
 int ozaki2_dgemm_stages(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
@@ -131,6 +134,10 @@ int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64
  * ozaki2_dgemm never uses.  Both need no workspace. */
 int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA,
                               const int8_t *resB, uint8_t *U, int use_tensor_cores, void *stream);
+
+/* Number of kernels this library has launched in this process so far (all devices, all entry
+ * points; memsets and copies are not counted). */
+uint64_t ozaki2_kernel_launches(void);
 
 /* Library build information: "ozaki2 <version> sm_100a ..." */
 const char *ozaki2_version(void);

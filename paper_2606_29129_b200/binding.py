@@ -30,7 +30,7 @@ class Ozaki2Error(RuntimeError):
 class ozaki2_stage_outputs(C.Structure):
     _fields_ = [("e", C.c_void_p), ("f", C.c_void_p), ("rowmax", C.c_void_p), ("colmax", C.c_void_p),
                 ("resA", C.c_void_p), ("resB", C.c_void_p), ("U", C.c_void_p), ("Cpp", C.c_void_p),
-                ("stage_ms", C.POINTER(C.c_float))]
+                ("stage_ms", C.POINTER(C.c_float)), ("stage_events", C.POINTER(C.c_void_p))]
 
 
 def lib() -> C.CDLL:
@@ -67,6 +67,8 @@ def lib() -> C.CDLL:
         L.ozaki2_debug_residue_gemm.argtypes = [ci, i64, i64, i64, vp, vp, vp, ci, vp]
         L.ozaki2_debug_residue_gemm.restype = ci
         L.ozaki2_version.restype = C.c_char_p
+        L.ozaki2_kernel_launches.argtypes = []
+        L.ozaki2_kernel_launches.restype = C.c_uint64
         _lib = L
     return _lib
 
@@ -97,6 +99,10 @@ def ozaki2_status_string(status: int) -> str:
 
 def ozaki2_version() -> str:
     return lib().ozaki2_version().decode()
+
+
+def ozaki2_kernel_launches() -> int:
+    return int(lib().ozaki2_kernel_launches())
 
 
 def ozaki2_workspace_bytes(m, n, k, num_moduli, scaling_mode) -> int:
@@ -209,6 +215,16 @@ def dgemm(A_dev, B_dev, num_moduli, scaling_mode=OZAKI2_MODE_PROP, alpha=1.0, be
     if rc:
         raise Ozaki2Error(rc, "ozaki2_dgemm")
     return C_dev
+
+
+def dgemm_with_stage_events(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, events, stream=None) -> int:
+    """ozaki2_dgemm_stages with nothing but `stage_events`: the same kernels as ozaki2_dgemm, plus five
+    cudaEventRecord calls.  `events`: five torch.cuda.Event(enable_timing=True) that have been recorded once
+    (torch creates the CUDA event lazily).  No synchronisation."""
+    out = ozaki2_stage_outputs()
+    arr = (C.c_void_p * 5)(*[ev.cuda_event for ev in events])
+    out.stage_events = C.cast(arr, C.POINTER(C.c_void_p))
+    return ozaki2_dgemm_stages(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream, out)
 
 
 def dgemm_stages(A_dev, B_dev, num_moduli, scaling_mode, alpha=1.0, beta=0.0, C_dev=None, want=("e", "f", "resA", "resB", "U", "Cpp"),

@@ -6,9 +6,13 @@
 
 #include <math.h>
 #include <stdio.h>
+#include <atomic>
 #include <mutex>
 #include <string.h>
 #include <vector>
+
+static std::atomic<uint64_t> g_launches{0};
+void oz2_count_launches(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
 
 namespace {
 
@@ -276,6 +280,7 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
         // C := beta C (zeros if beta == 0, BLAS rule)
         if (!(beta == 1.0)) {
             k_scale_c<<<dim3((unsigned)n, (unsigned)((m + 255) / 256)), 256, 0, st>>>(m, n, beta, C, ldc);
+            oz2_count_launches(1);
             OZ2_CUDA_TRY(cudaGetLastError());
         }
         return 0;
@@ -293,10 +298,12 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
 
     cudaEvent_t ev[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };
     const bool timing = out && out->stage_ms;
+    cudaEvent_t *uev = out && out->stage_events ? reinterpret_cast<cudaEvent_t *>(out->stage_events) : nullptr;
     if (timing) {
         for (int t = 0; t < 5; t++) OZ2_CUDA_TRY(cudaEventCreate(&ev[t]));
         OZ2_CUDA_TRY(cudaEventRecord(ev[0], st));
     }
+    if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[0], st));
     // ---- S1 scaling
     if (mode == OZAKI2_MODE_ACCURATE) {
         int8_t *Abar = reinterpret_cast<int8_t *>(ws + L.off_Abar), *Bbar = reinterpret_cast<int8_t *>(ws + L.off_Bbar);
@@ -307,17 +314,21 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
         if ((rc = oz2_launch_scale_fastprop(mode, N, m, n, k, A, lda, B, ldb, amax, ssq, e, f, st))) return rc;
     }
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[1], st));
+    if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[1], st));
     // ---- S2 conversion
     const int wide = needs_wide_words(N, mode) ? 1 : 0;
     if ((rc = oz2_launch_convert(0, N, wide, m, k, A, lda, e, RA, L.kp, st))) return rc;
     if ((rc = oz2_launch_convert(1, N, wide, n, k, B, ldb, f, RB, L.kp, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[2], st));
+    if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[2], st));
     // ---- S3 residue GEMMs
     if ((rc = oz2_launch_gemm_tc(N, 0, m, n, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[3], st));
+    if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[3], st));
     // ---- S4 + S5
     if ((rc = oz2_launch_crt(N, m, n, U, L.mp, e, f, alpha, beta, C, ldc, out ? out->Cpp : nullptr, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[4], st));
+    if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[4], st));
 
     if (out) {
         if (out->e) OZ2_CUDA_TRY(cudaMemcpyAsync(out->e, e, 4 * (size_t)m, cudaMemcpyDeviceToDevice, st));
@@ -487,6 +498,8 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
     if (use_tensor_cores) return oz2_launch_gemm_tc(num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
     return oz2_launch_gemm_check(num_moduli, m, n, k, resA, resB, k, U, m, st);
 }
+
+uint64_t ozaki2_kernel_launches(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char *ozaki2_version(void) { return "ozaki2 0.1 sm_100a tcgen05.kind::i8 (arxiv/paper_2606_29129)"; }
 

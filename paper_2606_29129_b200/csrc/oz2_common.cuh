@@ -77,6 +77,9 @@ int oz2_launch_mod_p(int l, const int32_t *in, uint8_t *out, int64_t count, cuda
 int oz2_launch_crt(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f,
                    double alpha, double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st);
 
+// kernel-launch accounting behind ozaki2_kernel_launches()
+void oz2_count_launches(int n);
+
 #define OZ2_CUDA_TRY(expr)                                   \
     do {                                                     \
         cudaError_t _e = (expr);                             \

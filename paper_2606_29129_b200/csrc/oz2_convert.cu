@@ -199,6 +199,7 @@ int oz2_launch_convert(int op, int N, int wide, int64_t rows, int64_t k, const d
         if (wide) k2_cols<3><<<(unsigned)gx, 128, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
         else k2_cols<2><<<(unsigned)gx, 128, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
     }
+    oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }

@@ -203,6 +203,7 @@ int launch_n(int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *
     dim3 grid((unsigned)n, (unsigned)((m + 511) / 512));
     if (Cpp) k4_crt<N, true><<<grid, 128, 0, st>>>(m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp);
     else k4_crt<N, false><<<grid, 128, 0, st>>>(m, n, U, mp, e, f, alpha, beta, C, ldc, nullptr);
+    oz2_count_launches(1);
     return (int)cudaGetLastError();
 }
 

@@ -380,6 +380,7 @@ int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t 
     else
         k3_residue_gemm<false><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
                                                                     U, mp, nullptr, nullptr);
+    oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -391,6 +392,7 @@ int oz2_launch_gemm_check(int nplanes, int64_t m, int64_t n, int64_t k, const in
     if (m <= 0 || n <= 0 || nplanes <= 0) return 0;
     dim3 grid((unsigned)((m + 31) / 32), (unsigned)((n + 7) / 8), (unsigned)nplanes);
     k3_check<<<grid, 256, 0, st>>>(nplanes, (int)m, (int)n, kp, RA, RB, U, mp);
+    oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -399,6 +401,7 @@ int oz2_launch_mod_p(int l, const int32_t *in, uint8_t *out, int64_t count, cuda
 {
     if (count <= 0) return 0;
     k_mod_p<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(l, in, out, count);
+    oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }

@@ -339,6 +339,7 @@ int oz2_launch_scale_fastprop(int mode, int N, int64_t m, int64_t n, int64_t k, 
     k1_rows<1><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
     k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e);
     k1_cols<false><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, B, ldb, f, nullptr);
+    oz2_count_launches(4);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -366,6 +367,7 @@ int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double 
     int64_t gx = (kp / 4 + 255) / 256;
     if (gx > 64) gx = 64;
     k1_bbar_cols<<<dim3((unsigned)n, (unsigned)gx), 256, 0, st>>>(n, k, B, ldb, EB, Bbar, kp);
+    oz2_count_launches(5);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -375,6 +377,7 @@ int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA,
 {
     k1_accu_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(N, m, EA, rowmax, e);
     k1_accu_finalize<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, n, EB, colmax, f);
+    oz2_count_launches(2);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
@@ -383,6 +386,7 @@ int oz2_launch_log2f(const float *x, float *y, int64_t count, cudaStream_t st)
 {
     if (count <= 0) return 0;
     k_log2f<<<(unsigned)((count + 255) / 256), 256, 0, st>>>(x, y, count);
+    oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
