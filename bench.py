@@ -38,8 +38,8 @@ INT8_OVER_BF16 = 2.0                # guide's nominal ratio 4.5 / 2.25 PFLOP/s
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--moduli", type=int, default=16, help="number of moduli N (BASELINE configs[2]: 14..18)")
     ap.add_argument("--mode", type=int, default=2, help="0 accurate, 1 original fast, 2 revised fast (headline)")
@@ -65,12 +65,12 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
-        self.index, self.proc, self.lines = index, None, []
+        self.index, self.proc, self.lines, self.window = index, None, [], [0.0, float("inf")]
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._pump, daemon=True)
             self.thread.start()
@@ -79,7 +79,7 @@ class ClockSampler:
 
     def _pump(self):
         for line in self.proc.stdout:
-            self.lines.append(line)
+            self.lines.append((time.time(), line))
 
     def stop(self):
         if self.proc is None:
@@ -92,7 +92,9 @@ class ClockSampler:
         self.thread.join(timeout=5)
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.lines:
+        inside = [ln for ts, ln in self.lines if self.window[0] <= ts <= self.window[1]]
+        # a timed region shorter than the sampling period: fall back to every sample taken since start()
+        for line in (inside if inside else [ln for _, ln in self.lines]):
             f = [x.strip() for x in line.split(",")]
             if len(f) < 7:
                 continue
@@ -110,9 +112,9 @@ class ClockSampler:
 
 
 def cpu_slab_shape(m, n, k):
-    """Bounded sample of the workload for the oracle: 256 rows of A against 2048 columns of B at the full k
-    (about 10-30 s on 8 cores at k = 8192)."""
-    return min(m, 256), min(n, 2048), k
+    """Bounded sample of the workload for the oracle: 512 rows of A against 4096 columns of B at the full k
+    (about 15 s on the GPU box's 16 host threads at k = 8192, N = 16)."""
+    return min(m, 512), min(n, 4096), k
 
 
 def time_oracle_slab(A, B, N, mode, shape):
@@ -217,15 +219,19 @@ def main():
         for ev in row:
             ev.record(stream)
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
     sampler = ClockSampler(local)
-    sampler.start()
+    sampler.start()                       # nvidia-smi takes a moment to come up: started before the last warm-ups
+    for _ in range(2):
+        step()
+    barrier()
     launches0 = pkg.ozaki2_kernel_launches()
+    sampler.window[0] = time.time()
     t0.record(stream)
     for s in range(K):
         step(evs[s])
     t1.record(stream)
     barrier()
+    sampler.window[1] = time.time()
     launches = pkg.ozaki2_kernel_launches() - launches0
     clocks = sampler.stop()
     total_ms = t0.elapsed_time(t1)

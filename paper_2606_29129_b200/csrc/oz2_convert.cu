@@ -1,171 +1,223 @@
 // oz2_convert.cu -- S2: A' = trunc(diag(mu) A), B' = trunc(B diag(nu)) (Step 2) and the symmetric
 // INT8 residues rmod(., p_l) for all N moduli in ONE pass over A and B.
 //
-// The scaled integers (up to 84 bits, never materialised in memory) live in registers as NB 32-bit words
-// (magnitude) plus a sign.  The residue modulo an odd p is taken from the base-256 digits:
-//     |a'| = sum_i d_i 256^i   =>   |a'| mod p = (sum_i d_i (256^i mod p)) mod p,
-// i.e. NB dp4a instructions against packed byte weights, one mulhi-based exact reduction that lands directly
-// in the symmetric range, then the sign.  p = 256 is the low byte in two's complement (reading R5).
+// Arithmetic.  The scaled integer a' (up to 84 bits, never written to memory) lives in registers as NB 32-bit
+// words in two's complement.  With d_i the base-256 digits of that bit pattern,
+//     a' = sum_i d_i 256^i - [a' < 0] 2^(32 NB),
+// so for an odd modulus p
+//     x = sum_i d_i (256^i mod p) + [a' < 0] ((-2^(32 NB)) mod p)        (NB dp4a, x < 2^20)
+// is congruent to a' and non-negative, and  r = x - p round(x / p)  with  round(x / p) = umulhi(x + h, magic),
+// h = (p - 1) / 2, is the symmetric residue in [-h, h] directly (the quotient is exact for x < 2^24).
+// p = 256: the low byte of the two's-complement pattern (reading R5).
 //
-// Layout written: planes[l][row][kp], k fastest (K-major for the tensor-core GEMM), kp = round_up(k, 128),
-// padding zero filled.  A is column-major, so the A path maps one thread to one row (coalesced loads along
-// the rows of a column) and stores 16 bytes per modulus; B's columns are already K-major: a warp walks 512
-// consecutive h of one column with fully coalesced 4-byte stores per modulus.
+// Data movement (the stage is bound by HBM traffic 8 + N bytes per element and by ~7 integer instructions per
+// element and modulus).  Planes are [l][row][kp], k fastest (K-major for the tensor-core GEMM),
+// kp = round_up(k, 128), zero padded.  Work unit everywhere: a "quad" = 4 consecutive h of one row, held by one
+// lane, so that a warp stores 128 contiguous bytes per row and modulus.
+//   * B is column-major = already K-major: a warp streams 256 consecutive h of one column with 16-byte loads.
+//   * A is column-major = M-major: a CTA stages a 32-row x 128-h tile through shared memory (coalesced 256-byte
+//     reads along the rows, transposed on the way in), then every warp converts whole rows of the tile.
+// The same two movers serve accurate mode's Abar / Bbar = ceil(mu' |.|), one plane.
 #include "oz2_common.cuh"
 
 namespace {
 
-__constant__ Oz2ModTab c_mod[OZ2_MAX_MODULI];
+struct ConvTab {
+    uint32_t negp, magic, half, cneg2, cneg3, wb[3];      // negp = 2^32 - p
+};
+__constant__ ConvTab c_conv[OZ2_MAX_MODULI];
 
-// magnitude words of trunc(|a| 2^ex) and the sign of a
+constexpr int TI = 32;             // rows of A per tile
+constexpr int TH = 128;            // h per tile
+constexpr int SROW = TH + 2;       // padded row of the staging tile in doubles (16-byte aligned rows)
+constexpr int CONV_THREADS = 256;
+
+// two's-complement words of trunc(a 2^ex); returns the sign mask (0 or 0xFFFFFFFF)
 template <int NB>
-__device__ __forceinline__ void scaled_words(double a, int ex, uint32_t (&w)[NB], uint32_t &neg)
+__device__ __forceinline__ uint32_t scaled_words(double a, int ex, uint32_t (&w)[NB])
 {
-    unsigned long long b = (unsigned long long)__double_as_longlong(a);
-    neg = (uint32_t)(b >> 63);
-    int be = (int)((b >> 52) & 0x7FF);
-    unsigned long long mant = b & 0x000FFFFFFFFFFFFFull;
-    unsigned long long M = be ? (mant | 0x0010000000000000ull) : mant;
-    int sh = (be ? be : 1) - 1075 + ex;          // |a| 2^ex = M 2^sh
-    uint32_t m0 = (uint32_t)M, m1 = (uint32_t)(M >> 32);
-    if (sh >= 0 && be != 0) {
-        // normal number: left shift by 0..31 (the row's largest element has 53 + sh <= 84 bits, every other
-        // |a| is below twice the largest)
-        w[0] = m0 << sh;
-        w[1] = __funnelshift_l(m0, m1, sh);
-        if (NB == 3) w[2] = __funnelshift_l(m1, 0u, sh);
-    } else if (sh >= 0) {
-        // subnormal number with a short mantissa: the shift can reach 83
-        unsigned long long lo = sh < 64 ? (M << sh) : 0ull;
-        w[0] = (uint32_t)lo;
-        w[1] = (uint32_t)(lo >> 32);
-        if (NB == 3) w[2] = sh == 0 ? 0u : (sh < 64 ? (uint32_t)(M >> (64 - sh)) : (uint32_t)(M << (sh - 64)));
-    } else {
-        int r = -sh;
-        unsigned long long v = r < 64 ? (M >> r) : 0ull;      // dropping magnitude bits = toward zero
+    const unsigned long long b = (unsigned long long)__double_as_longlong(a);
+    const uint32_t hi = (uint32_t)(b >> 32), lo = (uint32_t)b;
+    const uint32_t negm = (uint32_t)((int32_t)hi >> 31);
+    const unsigned long long neg64 = (unsigned long long)(long long)(int32_t)negm;
+    const int be = (int)((hi >> 20) & 0x7FFu);
+    const uint32_t m1 = (hi & 0x000FFFFFu) | (be ? 0x00100000u : 0u), m0 = lo;
+    const unsigned long long M = ((unsigned long long)m1 << 32) | m0;
+    const int sh = (be ? be : 1) - 1075 + ex;          // |a| 2^ex = M 2^sh, M < 2^53
+    if (NB == 2) {
+        // |a'| < 2^63: a non-zero M is shifted left by at most 62
+        unsigned long long v;
+        if (sh >= 0) v = M << (sh > 63 ? 63 : sh);
+        else v = (-sh < 64) ? (M >> (-sh)) : 0ull;      // dropping magnitude bits = toward zero
+        v = (v ^ neg64) - neg64;
         w[0] = (uint32_t)v;
         w[1] = (uint32_t)(v >> 32);
-        if (NB == 3) w[2] = 0u;
+        return v ? negm : 0u;                           // a' = -0 is +0: no 2^64 term
+    } else {
+        uint32_t v0, v1, v2;
+        if (sh >= 0) {
+            // |a'| < 2^95: word shift ws = sh / 32 (<= 2 for a non-zero M), bit shift bs
+            const int s = sh > 95 ? 95 : sh;
+            const int ws = s >> 5, bs = s & 31;
+            const uint32_t t0 = m0 << bs, t1 = __funnelshift_l(m0, m1, bs), t2 = __funnelshift_l(m1, 0u, bs);
+            v0 = ws == 0 ? t0 : 0u;
+            v1 = ws == 0 ? t1 : (ws == 1 ? t0 : 0u);
+            v2 = ws == 0 ? t2 : (ws == 1 ? t1 : t0);
+        } else {
+            const int r = -sh;
+            const unsigned long long v = r < 64 ? (M >> r) : 0ull;
+            v0 = (uint32_t)v;
+            v1 = (uint32_t)(v >> 32);
+            v2 = 0u;
+        }
+        // 96-bit two's-complement negate: (v ^ m) - m
+        const unsigned long long l01 = (((unsigned long long)v1 << 32) | v0) ^ neg64;
+        const unsigned long long s01 = l01 + (negm & 1u);
+        const uint32_t carry = (s01 < l01) ? 1u : 0u;
+        w[0] = (uint32_t)s01;
+        w[1] = (uint32_t)(s01 >> 32);
+        w[2] = (v2 ^ negm) + carry;
+        return (v0 | v1 | v2) ? negm : 0u;
     }
 }
 
-// symmetric residue of +-V modulo the odd modulus described by t
+// One quad: residues of 4 consecutive h for every modulus, one 4-byte store per modulus.
 template <int NB>
-__device__ __forceinline__ int residue_odd(const uint32_t (&w)[NB], uint32_t neg, const Oz2ModTab &t)
+__device__ __forceinline__ void quad_residues(const double (&a)[4], int ex, int N, int8_t *dst, int64_t plane_stride)
 {
-    uint32_t x = __dp4a(w[0], t.wb[0], 0u);
-    x = __dp4a(w[1], t.wb[1], x);
-    if (NB == 3) x = __dp4a(w[2], t.wb[2], x);
-    uint32_t q = __umulhi(x + t.half, t.magic);              // floor((x + h) / p) = round(x / p), exact (x < 2^24)
-    int r = (int)x - (int)(q * t.p);                         // in [-h, h], congruent to |a'|
-    return neg ? -r : r;
+    uint32_t w[4][NB], ng[4];
+#pragma unroll
+    for (int u = 0; u < 4; u++) ng[u] = scaled_words<NB>(a[u], ex, w[u]);
+    // p = 256: low bytes
+    {
+        const uint32_t lo = __byte_perm(w[0][0], w[1][0], 0x0040), hi = __byte_perm(w[2][0], w[3][0], 0x0040);
+        *reinterpret_cast<uint32_t *>(dst) = __byte_perm(lo, hi, 0x5410);
+    }
+    int8_t *out = dst;
+#pragma unroll 2
+    for (int l = 1; l < N; l++) {
+        const uint32_t negp = c_conv[l].negp, magic = c_conv[l].magic, half = c_conv[l].half;
+        const uint32_t cneg = NB == 2 ? c_conv[l].cneg2 : c_conv[l].cneg3;
+        const uint32_t wb0 = c_conv[l].wb[0], wb1 = c_conv[l].wb[1], wb2 = c_conv[l].wb[2];
+        uint32_t r[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            uint32_t x = ng[u] & cneg;
+            x = __dp4a(w[u][0], wb0, x);
+            x = __dp4a(w[u][1], wb1, x);
+            if (NB == 3) x = __dp4a(w[u][2], wb2, x);
+            const uint32_t q = __umulhi(x + half, magic);           // round(x / p), exact
+            r[u] = q * negp + x;                                    // x - q p: symmetric residue, two's complement
+        }
+        const uint32_t lo = __byte_perm(r[0], r[1], 0x0040), hi = __byte_perm(r[2], r[3], 0x0040);
+        out += plane_stride;
+        *reinterpret_cast<uint32_t *>(out) = __byte_perm(lo, hi, 0x5410);
+    }
 }
 
-template <int NB>
-__device__ __forceinline__ int residue_256(const uint32_t (&w)[NB], uint32_t neg)
+// accurate mode: ceil(|a| 2^(5-E)) in [0, 64]
+__device__ __forceinline__ uint32_t ceil_scaled(double a, int E)
 {
-    int b0 = (int)(w[0] & 0xFFu);
-    return (neg ? -b0 : b0) & 0xFF;                          // two's-complement low byte of a'
+    const unsigned long long b = (unsigned long long)__double_as_longlong(a) & 0x7FFFFFFFFFFFFFFFull;
+    if (b == 0) return 0u;
+    const int be = (int)(b >> 52);
+    const unsigned long long mant = b & 0x000FFFFFFFFFFFFFull;
+    const unsigned long long M = be ? (mant | 0x0010000000000000ull) : mant;
+    const int q = (be ? be : 1) - 1075;
+    const int r = -(q + 5 - E);           // value = M 2^-r <= 64; r >= 47 for normal numbers
+    if (r <= 0) return (uint32_t)(M << (-r));
+    if (r >= 64) return 1u;
+    return (uint32_t)(M >> r) + ((M & ((1ull << r) - 1)) != 0 ? 1u : 0u);
+}
+
+__device__ __forceinline__ void quad_bar(const double (&a)[4], int E, int8_t *dst)
+{
+    uint32_t o = 0;
+#pragma unroll
+    for (int u = 0; u < 4; u++) o |= ceil_scaled(a[u], E) << (8 * u);
+    *reinterpret_cast<uint32_t *>(dst) = o;
 }
 
 // ---------------------------------------------------------------------------------------------
-// A path: thread = row i, 16 consecutive h per iteration
+// A path.  MODE 0: residues (NB words)   MODE 1: Abar
 // ---------------------------------------------------------------------------------------------
-template <int NB>
-__global__ void __launch_bounds__(128)
+template <int NB, int MODE>
+__global__ void __launch_bounds__(CONV_THREADS)
 k2_rows(int N, int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, const int32_t *__restrict__ e,
         int8_t *__restrict__ planes, int64_t kp)
 {
-    int64_t i = (int64_t)blockIdx.x * 128 + threadIdx.x;
-    if (i >= m) return;
-    const int ex = e[i];
+    __shared__ __align__(16) double tile[TI * SROW];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t i0 = (int64_t)blockIdx.x * TI, h0 = (int64_t)blockIdx.y * TH;
+    // ---- stage: thread (lane = row, warp = h mod 8), 16 loads in flight, transposed into tile[i][h]
+    {
+        const int64_t i = i0 + lane;
+        const bool iok = i < m;
+        const double *src = A + i + (h0 + warp) * lda;
+        double v[16];
+#pragma unroll
+        for (int s = 0; s < 16; s++) {
+            const int64_t h = h0 + warp + 8 * s;
+            v[s] = (iok && h < k) ? __ldg(src + (int64_t)(8 * s) * lda) : 0.0;
+        }
+#pragma unroll
+        for (int s = 0; s < 16; s++) tile[lane * SROW + warp + 8 * s] = v[s];
+    }
+    __syncthreads();
+    // ---- convert: warp w owns rows 4w .. 4w+3, lane owns the quad h = 4 lane .. 4 lane + 3
     const int64_t plane_stride = m * kp;
-    const int64_t chunk = oz2_round_up((kp / 16 + gridDim.y - 1) / gridDim.y, 8) * 16;   // multiple of 128 bytes
-    const int64_t hbeg = (int64_t)blockIdx.y * chunk, hend = hbeg + chunk < kp ? hbeg + chunk : kp;
-    for (int64_t h0 = hbeg; h0 < hend; h0 += 16) {
-        uint32_t w[16][NB];
-        uint32_t negmask = 0;
-#pragma unroll
-        for (int u = 0; u < 16; u++) {
-            int64_t h = h0 + u;
-            double a = h < k ? __ldg(A + i + h * lda) : 0.0;
-            uint32_t neg;
-            scaled_words<NB>(a, ex, w[u], neg);
-            negmask |= neg << u;
-        }
-        int8_t *dst = planes + i * kp + h0;
-        {   // p = 256
-            uint32_t o[4] = { 0, 0, 0, 0 };
-#pragma unroll
-            for (int u = 0; u < 16; u++) o[u >> 2] |= (uint32_t)residue_256<NB>(w[u], (negmask >> u) & 1u) << (8 * (u & 3));
-            *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
-        }
 #pragma unroll 1
-        for (int l = 1; l < N; l++) {
-            const Oz2ModTab t = c_mod[l];
-            uint32_t o[4] = { 0, 0, 0, 0 };
-#pragma unroll
-            for (int u = 0; u < 16; u++)
-                o[u >> 2] |= ((uint32_t)residue_odd<NB>(w[u], (negmask >> u) & 1u, t) & 0xFFu) << (8 * (u & 3));
-            *reinterpret_cast<uint4 *>(dst + l * plane_stride) = make_uint4(o[0], o[1], o[2], o[3]);
-        }
+    for (int rr = 0; rr < TI / 8; rr++) {
+        const int il = warp * (TI / 8) + rr;
+        const int64_t i = i0 + il;
+        if (i >= m) break;
+        const double2 lo = *reinterpret_cast<const double2 *>(&tile[il * SROW + 4 * lane]);
+        const double2 hi = *reinterpret_cast<const double2 *>(&tile[il * SROW + 4 * lane + 2]);
+        const double a[4] = { lo.x, lo.y, hi.x, hi.y };
+        int8_t *dst = planes + i * kp + h0 + 4 * lane;
+        const int ex = __ldg(e + i);
+        if (MODE == 0) quad_residues<NB>(a, ex, N, dst, plane_stride);
+        else quad_bar(a, ex, dst);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// B path: warp = 512 consecutive h of column j; lane holds h = c*512 + 128 t + 4 lane + {0..3}, t = 0..3
+// B path: warp = 256 consecutive h of column j; lane holds the quads at 4 lane and 128 + 4 lane
 // ---------------------------------------------------------------------------------------------
-template <int NB>
-__global__ void __launch_bounds__(128)
+template <int NB, int MODE>
+__global__ void __launch_bounds__(CONV_THREADS)
 k2_cols(int N, int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, const int32_t *__restrict__ f,
         int8_t *__restrict__ planes, int64_t kp)
 {
     const int lane = threadIdx.x & 31;
-    const int64_t chunks = (kp + 511) / 512;
-    const int64_t items = n * chunks;
+    const int64_t chunks = (kp + 255) / 256;
+    const int64_t item = (int64_t)blockIdx.x * (CONV_THREADS / 32) + (threadIdx.x >> 5);
+    if (item >= n * chunks) return;
+    const int64_t j = item / chunks, c = item - j * chunks;
+    const double *col = B + j * ldb;
+    const int ex = __ldg(f + j);
+    const bool vec = ((((uintptr_t)col) & 15) == 0);
     const int64_t plane_stride = n * kp;
-    for (int64_t it = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5); it < items; it += (int64_t)gridDim.x * 4) {
-        const int64_t j = it / chunks, c = it - j * chunks;
-        const double *col = B + j * ldb;
-        const int ex = f[j];
-        const bool vec = ((((uintptr_t)col) & 15) == 0);
-        uint32_t w[16][NB];
-        uint32_t negmask = 0;
+    double a[2][4];
 #pragma unroll
-        for (int t = 0; t < 4; t++) {
-            int64_t h = c * 512 + 128 * t + 4 * lane;
-            double a[4];
-            if (vec && h + 3 < k) {
-                double2 v0 = __ldg(reinterpret_cast<const double2 *>(col + h));
-                double2 v1 = __ldg(reinterpret_cast<const double2 *>(col + h + 2));
-                a[0] = v0.x; a[1] = v0.y; a[2] = v1.x; a[3] = v1.y;
-            } else {
+    for (int t = 0; t < 2; t++) {
+        const int64_t h = c * 256 + 128 * t + 4 * lane;
+        if (vec && h + 3 < k) {
+            const double2 v0 = __ldg(reinterpret_cast<const double2 *>(col + h));
+            const double2 v1 = __ldg(reinterpret_cast<const double2 *>(col + h + 2));
+            a[t][0] = v0.x; a[t][1] = v0.y; a[t][2] = v1.x; a[t][3] = v1.y;
+        } else {
 #pragma unroll
-                for (int u = 0; u < 4; u++) a[u] = (h + u < k) ? __ldg(col + h + u) : 0.0;
-            }
-#pragma unroll
-            for (int u = 0; u < 4; u++) {
-                uint32_t neg;
-                scaled_words<NB>(a[u], ex, w[4 * t + u], neg);
-                negmask |= neg << (4 * t + u);
-            }
+            for (int u = 0; u < 4; u++) a[t][u] = (h + u < k) ? __ldg(col + h + u) : 0.0;
         }
-        int8_t *dst = planes + j * kp + c * 512 + 4 * lane;
-#pragma unroll 1
-        for (int l = 0; l < N; l++) {
-            const Oz2ModTab tb = c_mod[l];
+    }
 #pragma unroll
-            for (int t = 0; t < 4; t++) {
-                uint32_t o = 0;
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    int r = l == 0 ? residue_256<NB>(w[4 * t + u], (negmask >> (4 * t + u)) & 1u)
-                                   : residue_odd<NB>(w[4 * t + u], (negmask >> (4 * t + u)) & 1u, tb);
-                    o |= ((uint32_t)r & 0xFFu) << (8 * u);
-                }
-                if (c * 512 + 128 * t + 4 * lane < kp)
-                    *reinterpret_cast<uint32_t *>(dst + l * plane_stride + 128 * t) = o;
-            }
+    for (int t = 0; t < 2; t++) {
+        const int64_t h = c * 256 + 128 * t + 4 * lane;
+        if (h < kp) {
+            int8_t *dst = planes + j * kp + h;
+            if (MODE == 0) quad_residues<NB>(a[t], ex, N, dst, plane_stride);
+            else quad_bar(a[t], ex, dst);
         }
     }
 }
@@ -174,30 +226,40 @@ k2_cols(int N, int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, 
 
 int oz2_convert_upload_tables(const Oz2HostTables &t)
 {
-    OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_mod, t.mod, sizeof(t.mod)));
+    ConvTab h[OZ2_MAX_MODULI];
+    for (int l = 0; l < OZ2_MAX_MODULI; l++) {
+        const uint32_t p = t.mod[l].p;
+        h[l].negp = 0u - p;
+        h[l].magic = t.mod[l].magic;
+        h[l].half = t.mod[l].half;
+        const uint32_t two64 = (uint32_t)(((0xFFFFFFFFFFFFFFFFull % p) + 1ull) % p);            // 2^64 mod p
+        const uint32_t two32 = (uint32_t)(0x100000000ull % p);
+        const uint32_t two96 = (uint32_t)(((unsigned long long)two64 * two32) % p);             // 2^96 mod p
+        h[l].cneg2 = (p - two64) % p;
+        h[l].cneg3 = (p - two96) % p;
+        for (int i = 0; i < 3; i++) h[l].wb[i] = t.mod[l].wb[i];
+    }
+    OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_conv, h, sizeof(h)));
     return 0;
 }
 
+// op 0: rows of A, op 1: columns of B.  N >= 1: residue planes [N][rows][kp] with exponents `ex`.  N == 0: the
+// single plane ceil(mu' |.|) of accurate mode; `ex` then holds E = floor(log2 max |.|) per row.
 int oz2_launch_convert(int op, int N, int wide, int64_t rows, int64_t k, const double *X, int64_t ldx,
                        const int32_t *ex, int8_t *planes, int64_t kp, cudaStream_t st)
 {
     if (rows <= 0) return 0;
     if (op == 0) {
-        int64_t bx = (rows + 127) / 128;
-        int64_t gy = (148 * 12 + bx - 1) / bx;
-        int64_t chunks = kp / 16;
-        if (gy > chunks) gy = chunks;
-        if (gy > 65535) gy = 65535;
-        if (gy < 1) gy = 1;
-        dim3 grid((unsigned)bx, (unsigned)gy);
-        if (wide) k2_rows<3><<<grid, 128, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else k2_rows<2><<<grid, 128, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        dim3 grid((unsigned)((rows + TI - 1) / TI), (unsigned)(kp / TH));
+        if (N == 0) k2_rows<2, 1><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else if (wide) k2_rows<3, 0><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else k2_rows<2, 0><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
     } else {
-        int64_t items = rows * ((kp + 511) / 512);
-        int64_t gx = (items + 3) / 4;
-        if (gx > 148 * 32) gx = 148 * 32;
-        if (wide) k2_cols<3><<<(unsigned)gx, 128, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else k2_cols<2><<<(unsigned)gx, 128, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        const int64_t items = rows * ((kp + 255) / 256);
+        const unsigned gx = (unsigned)((items + CONV_THREADS / 32 - 1) / (CONV_THREADS / 32));
+        if (N == 0) k2_cols<2, 1><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else if (wide) k2_cols<3, 0><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else k2_cols<2, 0><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
     }
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());

@@ -227,66 +227,12 @@ k1_cols(int mode, int N, int64_t k, const double *__restrict__ B, int64_t ldb, i
 }
 
 // ---------------------------------------------------------------------------------------------
-// accurate mode: Abar, Bbar as INT8, K-major, pitch kp (zero padded)
+// accurate mode: E per row / column; Abar, Bbar are written by the movers of oz2_convert.cu
 // ---------------------------------------------------------------------------------------------
-// ceil(|a| 2^(5-E)) in [0, 64]
-__device__ __forceinline__ int ceil_scaled(unsigned long long b, int E)
-{
-    if (b == 0) return 0;
-    unsigned long long M;
-    int q;
-    decompose(b, M, q);
-    int r = -(q + 5 - E);                 // value = M 2^-r < 64; r >= 47 for normal numbers
-    if (r <= 0) return (int)(M << (-r));  // subnormal with a small mantissa: exact
-    if (r >= 64) return 1;
-    unsigned long long fl = M >> r;
-    return (int)fl + ((M & ((1ull << r) - 1)) != 0);
-}
-
 __global__ void k1_rows_E(int64_t m, const unsigned long long *__restrict__ amax, int32_t *__restrict__ EA)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < m) EA[i] = amax[i] ? floor_log2_bits(amax[i]) : OZ2_E_ZERO;
-}
-
-// thread = one row, 16 consecutive h per iteration -> one 16-byte store
-__global__ void __launch_bounds__(128)
-k1_abar_rows(int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, const int32_t *__restrict__ EA,
-             int8_t *__restrict__ Abar, int64_t kp)
-{
-    int64_t i = (int64_t)blockIdx.x * 128 + threadIdx.x;
-    if (i >= m) return;
-    int E = EA[i];
-    for (int64_t h0 = (int64_t)blockIdx.y * 16; h0 < kp; h0 += (int64_t)gridDim.y * 16) {
-        uint32_t w[4] = { 0, 0, 0, 0 };
-#pragma unroll
-        for (int u = 0; u < 16; u++) {
-            int64_t h = h0 + u;
-            int v = h < k ? ceil_scaled(abs_bits(__ldg(A + i + h * lda)), E) : 0;
-            w[u >> 2] |= (uint32_t)v << (8 * (u & 3));
-        }
-        *reinterpret_cast<uint4 *>(Abar + i * kp + h0) = make_uint4(w[0], w[1], w[2], w[3]);
-    }
-}
-
-// thread = 4 consecutive h of one column -> one 4-byte store, coalesced
-__global__ void __launch_bounds__(256)
-k1_bbar_cols(int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, const int32_t *__restrict__ EB,
-             int8_t *__restrict__ Bbar, int64_t kp)
-{
-    int64_t j = blockIdx.x;
-    int E = EB[j];
-    const double *col = B + j * ldb;
-    for (int64_t h0 = 4 * ((int64_t)blockIdx.y * 256 + threadIdx.x); h0 < kp; h0 += 4 * 256 * (int64_t)gridDim.y) {
-        uint32_t w = 0;
-#pragma unroll
-        for (int u = 0; u < 4; u++) {
-            int64_t h = h0 + u;
-            int v = h < k ? ceil_scaled(abs_bits(__ldg(col + h)), E) : 0;
-            w |= (uint32_t)v << (8 * u);
-        }
-        *reinterpret_cast<uint32_t *>(Bbar + j * kp + h0) = w;
-    }
 }
 
 __global__ void k1_accu_finalize(int N, int64_t cnt, const int32_t *__restrict__ E, const int32_t *__restrict__ mx,
@@ -357,18 +303,11 @@ int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double 
     k1_rows<0><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, nullptr);
     k1_rows_E<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(m, amaxA, EA);
     k1_cols<true><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, B, ldb, nullptr, EB);
-    int64_t chunks = kp / 16;
-    int64_t bx = (m + 127) / 128;
-    int64_t gyy = (148 * 16 + bx - 1) / bx;
-    if (gyy > chunks) gyy = chunks;
-    if (gyy > 65535) gyy = 65535;
-    if (gyy < 1) gyy = 1;
-    k1_abar_rows<<<dim3((unsigned)bx, (unsigned)gyy), 128, 0, st>>>(m, k, A, lda, EA, Abar, kp);
-    int64_t gx = (kp / 4 + 255) / 256;
-    if (gx > 64) gx = 64;
-    k1_bbar_cols<<<dim3((unsigned)n, (unsigned)gx), 256, 0, st>>>(n, k, B, ldb, EB, Bbar, kp);
-    oz2_count_launches(5);
+    oz2_count_launches(3);
     OZ2_CUDA_TRY(cudaGetLastError());
+    int rc;
+    if ((rc = oz2_launch_convert(0, 0, 0, m, k, A, lda, EA, Abar, kp, st))) return rc;
+    if ((rc = oz2_launch_convert(1, 0, 0, n, k, B, ldb, EB, Bbar, kp, st))) return rc;
     return 0;
 }
 
