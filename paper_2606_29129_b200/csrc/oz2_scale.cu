@@ -46,25 +46,14 @@ __device__ __forceinline__ void decompose(unsigned long long b, unsigned long lo
 }
 
 // T = ceil(2^44 (v / 2^E)^2) for |v| < 2^(E+1): exact.  (reading R2)
-__device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int E)
+// Slow path, any input: exact 128-bit integer square.
+__device__ __noinline__ unsigned long long sq_term_int(unsigned long long b, int E)
 {
-    if (b == 0) return 0;
     unsigned long long M;
     int q;
     decompose(b, M, q);
     // 2^44 (v/2^E)^2 = M^2 2^-s with s = 2 (E - q) - 44.
     int s = 2 * (E - q) - 44;
-    if (M >> 52) {
-        // normal number: s >= 60.  With M5 = M << 5: M5^2 = M^2 2^10, so floor(M^2 2^-s) =
-        // floor(hi64(M5^2) 2^-(s - 54)), and the dropped bits are non-zero iff 2 ctz(M) < s.
-        unsigned long long M5 = M << 5;
-        unsigned long long hi = __umul64hi(M5, M5);
-        int r = s - 54;                               // >= 6
-        unsigned long long fl = r < 64 ? (hi >> r) : 0ull;
-        int tz = __ffsll((long long)M) - 1;
-        return fl + ((2 * tz < s) ? 1ull : 0ull);
-    }
-    // subnormal input (M < 2^52): s can be anything, also negative; use the full 128-bit square
     unsigned long long lo = M * M, hi = __umul64hi(M, M);
     if (s <= 0) return lo << (-s);                    // exact, the value is at most 2^46
     if (s < 64) return ((hi << (64 - s)) | (lo >> s)) + ((lo & ((1ull << s) - 1)) ? 1ull : 0ull);
@@ -74,6 +63,19 @@ __device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int 
         return (hi >> r) + (rem ? 1ull : 0ull);
     }
     return 1ull;
+}
+
+// Fast path: x = |v| 2^(22-E) is an exact exponent shift while it stays a normal number (x < 2^23), x^2 < 2^46 has
+// a quantum <= 2^-7 in FP64, so RU(x x) <= ceil(x^2) (integers below 2^53 are representable) and
+// ceil(RU(x x)) = ceil(x^2) exactly: one DMUL.RU and one F2I.CEIL.
+__device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int E)
+{
+    if (b == 0) return 0;
+    const int be = (int)(b >> 52);
+    const int ne = be + 22 - E;                       // biased exponent of x
+    if (be == 0 || ne < 1) return sq_term_int(b, E);  // subnormal input or subnormal x: rare
+    const double x = __longlong_as_double((long long)(b + ((unsigned long long)(long long)(22 - E) << 52)));
+    return __double2ull_ru(__dmul_ru(x, x));
 }
 
 // LOG2F(x) = RN_32(log2 x) for float x in [1,2] (reading R3): FP64 log2 (<= 1 ulp), rounded once.
