@@ -226,13 +226,12 @@ Layout make_layout(int64_t m, int64_t n, int64_t k, int N, int mode)
     return L;
 }
 
-// widths: fast / prop  <= floor(P'_prop) + 1 bits, accurate <= floor(P'_accu) + 7 bits; two two's-complement words
-// hold |a'| < 2^63
+// widths: fast / prop  <= floor(P'_prop) + 1 bits, accurate <= floor(P'_accu) + 7 bits; two words hold |a'| < 2^64
 bool needs_wide_words(int N, int mode)
 {
     const float Pp = host_consts().tab.crt[N].Pprop;
     const int width = (int)floorf(Pp) + (mode == OZAKI2_MODE_ACCURATE ? 7 : 1);
-    return width > 63;
+    return width > 64;
 }
 
 int check_args(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B, int64_t ldb,

@@ -1,14 +1,16 @@
 // oz2_convert.cu -- S2: A' = trunc(diag(mu) A), B' = trunc(B diag(nu)) (Step 2) and the symmetric
 // INT8 residues rmod(., p_l) for all N moduli in ONE pass over A and B.
 //
-// Arithmetic.  The scaled integer a' (up to 84 bits, never written to memory) lives in registers as NB 32-bit
-// words in two's complement.  With d_i the base-256 digits of that bit pattern,
-//     a' = sum_i d_i 256^i - [a' < 0] 2^(32 NB),
-// so for an odd modulus p
-//     x = sum_i d_i (256^i mod p) + [a' < 0] ((-2^(32 NB)) mod p)        (NB dp4a, x < 2^20)
-// is congruent to a' and non-negative, and  r = x - p round(x / p)  with  round(x / p) = umulhi(x + h, magic),
-// h = (p - 1) / 2, is the symmetric residue in [-h, h] directly (the quotient is exact for x < 2^24).
-// p = 256: the low byte of the two's-complement pattern (reading R5).
+// Arithmetic.  |a'| (up to 84 bits, never written to memory) lives in registers as NB 32-bit words.  With d_i the
+// base-256 digits of |a'|, for an odd modulus p
+//     x = sum_i d_i (256^i mod p)                                       (NB dp4a; x < 2^20, congruent to |a'|)
+// and the symmetric residue is r = sign(a') (x - p round(x / p)).  The reduction runs in FP32 on exact small
+// integers, so that it can use both halves of the FMA pipe (integer multiplies only run on one):
+//     the dp4a chain starts from 0x4B000000, the bit pattern of 2^23, so its result read as a float is 2^23 + x;
+//     q = RN(x (1/p)~ + 1.5 2^23) - 1.5 2^23 is round(x / p) exactly: |x (1/p)~ - x/p| < 2^-11, while x / p is at
+//     least 1/(2p) > 2^-9 away from every half-integer (p odd);
+//     x - q p is then exact, and RN(sign (x - q p) + 1.5 2^23) holds r in two's complement in its low byte.
+// p = 256: the low byte of a' in two's complement (reading R5).
 //
 // Data movement (the stage is bound by HBM traffic 8 + N bytes per element and by ~7 integer instructions per
 // element and modulus).  Planes are [l][row][kp], k fastest (K-major for the tensor-core GEMM),
@@ -23,7 +25,9 @@
 namespace {
 
 struct ConvTab {
-    uint32_t negp, magic, half, cneg2, cneg3, wb[3];      // negp = 2^32 - p
+    float invp, negp;          // RN(1 / p), -p
+    uint32_t wb[3];            // byte weights 256^(4t+b) mod p, packed
+    uint32_t pad[3];
 };
 __constant__ ConvTab c_conv[OZ2_MAX_MODULI];
 
@@ -32,86 +36,87 @@ constexpr int TH = 128;            // h per tile
 constexpr int SROW = TH + 2;       // padded row of the staging tile in doubles (16-byte aligned rows)
 constexpr int CONV_THREADS = 256;
 
-// two's-complement words of trunc(a 2^ex); returns the sign mask (0 or 0xFFFFFFFF)
+// magnitude words of trunc(|a| 2^ex); returns the sign mask of a (0 or 0xFFFFFFFF)
 template <int NB>
 __device__ __forceinline__ uint32_t scaled_words(double a, int ex, uint32_t (&w)[NB])
 {
     const unsigned long long b = (unsigned long long)__double_as_longlong(a);
     const uint32_t hi = (uint32_t)(b >> 32), lo = (uint32_t)b;
     const uint32_t negm = (uint32_t)((int32_t)hi >> 31);
-    const unsigned long long neg64 = (unsigned long long)(long long)(int32_t)negm;
     const int be = (int)((hi >> 20) & 0x7FFu);
     const uint32_t m1 = (hi & 0x000FFFFFu) | (be ? 0x00100000u : 0u), m0 = lo;
     const unsigned long long M = ((unsigned long long)m1 << 32) | m0;
     const int sh = (be ? be : 1) - 1075 + ex;          // |a| 2^ex = M 2^sh, M < 2^53
     if (NB == 2) {
-        // |a'| < 2^63: a non-zero M is shifted left by at most 62
+        // |a'| < 2^64: a non-zero M is shifted left by at most 63
         unsigned long long v;
         if (sh >= 0) v = M << (sh > 63 ? 63 : sh);
         else v = (-sh < 64) ? (M >> (-sh)) : 0ull;      // dropping magnitude bits = toward zero
-        v = (v ^ neg64) - neg64;
         w[0] = (uint32_t)v;
         w[1] = (uint32_t)(v >> 32);
-        return v ? negm : 0u;                           // a' = -0 is +0: no 2^64 term
     } else {
-        uint32_t v0, v1, v2;
         if (sh >= 0) {
-            // |a'| < 2^95: word shift ws = sh / 32 (<= 2 for a non-zero M), bit shift bs
+            // |a'| < 2^96: word shift ws = sh / 32 (<= 2 for a non-zero M), bit shift bs
             const int s = sh > 95 ? 95 : sh;
             const int ws = s >> 5, bs = s & 31;
             const uint32_t t0 = m0 << bs, t1 = __funnelshift_l(m0, m1, bs), t2 = __funnelshift_l(m1, 0u, bs);
-            v0 = ws == 0 ? t0 : 0u;
-            v1 = ws == 0 ? t1 : (ws == 1 ? t0 : 0u);
-            v2 = ws == 0 ? t2 : (ws == 1 ? t1 : t0);
+            w[0] = ws == 0 ? t0 : 0u;
+            w[1] = ws == 0 ? t1 : (ws == 1 ? t0 : 0u);
+            w[2] = ws == 0 ? t2 : (ws == 1 ? t1 : t0);
         } else {
             const int r = -sh;
             const unsigned long long v = r < 64 ? (M >> r) : 0ull;
-            v0 = (uint32_t)v;
-            v1 = (uint32_t)(v >> 32);
-            v2 = 0u;
+            w[0] = (uint32_t)v;
+            w[1] = (uint32_t)(v >> 32);
+            w[2] = 0u;
         }
-        // 96-bit two's-complement negate: (v ^ m) - m
-        const unsigned long long l01 = (((unsigned long long)v1 << 32) | v0) ^ neg64;
-        const unsigned long long s01 = l01 + (negm & 1u);
-        const uint32_t carry = (s01 < l01) ? 1u : 0u;
-        w[0] = (uint32_t)s01;
-        w[1] = (uint32_t)(s01 >> 32);
-        w[2] = (v2 ^ negm) + carry;
-        return (v0 | v1 | v2) ? negm : 0u;
     }
+    return negm;
 }
 
-// One quad: residues of 4 consecutive h for every modulus, one 4-byte store per modulus.
+// Two quads at once (8 elements, exponents ex0 / ex1): residues for every modulus, one 4-byte store per quad and
+// modulus.  The per-modulus constants are loaded once for the 8 elements; `ok1` guards the second quad's stores.
 template <int NB>
-__device__ __forceinline__ void quad_residues(const double (&a)[4], int ex, int N, int8_t *dst, int64_t plane_stride)
+__device__ __forceinline__ void oct_residues(const double (&a)[2][4], int ex0, int ex1, int N, int8_t *dst0,
+                                             int64_t dst1_off, bool ok1, int64_t plane_stride)
 {
-    uint32_t w[4][NB], ng[4];
+    constexpr float MAGIC = 12582912.0f;               // 1.5 2^23: RN(y + MAGIC) - MAGIC = round(y) for |y| < 2^22
+    uint32_t w[8][NB];
+    float sg[8];                                       // +1.0f / -1.0f
+    uint32_t b256[8];                                  // a' in two's complement, low word
 #pragma unroll
-    for (int u = 0; u < 4; u++) ng[u] = scaled_words<NB>(a[u], ex, w[u]);
-    // p = 256: low bytes
-    {
-        const uint32_t lo = __byte_perm(w[0][0], w[1][0], 0x0040), hi = __byte_perm(w[2][0], w[3][0], 0x0040);
-        *reinterpret_cast<uint32_t *>(dst) = __byte_perm(lo, hi, 0x5410);
+    for (int u = 0; u < 8; u++) {
+        const uint32_t negm = scaled_words<NB>(a[u >> 2][u & 3], u < 4 ? ex0 : ex1, w[u]);
+        sg[u] = __uint_as_float(0x3F800000u | (negm & 0x80000000u));
+        b256[u] = (w[u][0] ^ negm) - negm;
     }
-    int8_t *out = dst;
-#pragma unroll 2
-    for (int l = 1; l < N; l++) {
-        const uint32_t negp = c_conv[l].negp, magic = c_conv[l].magic, half = c_conv[l].half;
-        const uint32_t cneg = NB == 2 ? c_conv[l].cneg2 : c_conv[l].cneg3;
-        const uint32_t wb0 = c_conv[l].wb[0], wb1 = c_conv[l].wb[1], wb2 = c_conv[l].wb[2];
-        uint32_t r[4];
-#pragma unroll
-        for (int u = 0; u < 4; u++) {
-            uint32_t x = ng[u] & cneg;
-            x = __dp4a(w[u][0], wb0, x);
-            x = __dp4a(w[u][1], wb1, x);
-            if (NB == 3) x = __dp4a(w[u][2], wb2, x);
-            const uint32_t q = __umulhi(x + half, magic);           // round(x / p), exact
-            r[u] = q * negp + x;                                    // x - q p: symmetric residue, two's complement
-        }
-        const uint32_t lo = __byte_perm(r[0], r[1], 0x0040), hi = __byte_perm(r[2], r[3], 0x0040);
-        out += plane_stride;
+    int8_t *out = dst0;
+    {   // p = 256: low bytes
+        const uint32_t lo = __byte_perm(b256[0], b256[1], 0x0040), hi = __byte_perm(b256[2], b256[3], 0x0040);
         *reinterpret_cast<uint32_t *>(out) = __byte_perm(lo, hi, 0x5410);
+        const uint32_t lo1 = __byte_perm(b256[4], b256[5], 0x0040), hi1 = __byte_perm(b256[6], b256[7], 0x0040);
+        if (ok1) *reinterpret_cast<uint32_t *>(out + dst1_off) = __byte_perm(lo1, hi1, 0x5410);
+    }
+#pragma unroll 1
+    for (int l = 1; l < N; l++) {
+        const float invp = c_conv[l].invp, negp = c_conv[l].negp;
+        const uint32_t wb0 = c_conv[l].wb[0], wb1 = c_conv[l].wb[1], wb2 = c_conv[l].wb[2];
+        uint32_t r[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            uint32_t xb = __dp4a(w[u][0], wb0, 0x4B000000u);
+            xb = __dp4a(w[u][1], wb1, xb);
+            if (NB == 3) xb = __dp4a(w[u][2], wb2, xb);
+            const float x = __fadd_rn(__uint_as_float(xb), -8388608.0f);        // exact
+            const float q = __fadd_rn(__fmaf_rn(x, invp, MAGIC), -MAGIC);       // round(x / p), exact
+            const float rm = __fmaf_rn(q, negp, x);                             // x - q p in [-(p-1)/2, (p-1)/2]
+            r[u] = __float_as_uint(__fmaf_rn(rm, sg[u], MAGIC));                // low byte = sign * rm
+        }
+        out += plane_stride;
+        const uint32_t lo = __byte_perm(r[0], r[1], 0x0040), hi = __byte_perm(r[2], r[3], 0x0040);
+        *reinterpret_cast<uint32_t *>(out) = __byte_perm(lo, hi, 0x5410);
+        const uint32_t lo1 = __byte_perm(r[4], r[5], 0x0040), hi1 = __byte_perm(r[6], r[7], 0x0040);
+        if (ok1) *reinterpret_cast<uint32_t *>(out + dst1_off) = __byte_perm(lo1, hi1, 0x5410);
     }
 }
 
@@ -167,17 +172,25 @@ k2_rows(int N, int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, 
     // ---- convert: warp w owns rows 4w .. 4w+3, lane owns the quad h = 4 lane .. 4 lane + 3
     const int64_t plane_stride = m * kp;
 #pragma unroll 1
-    for (int rr = 0; rr < TI / 8; rr++) {
+    for (int rr = 0; rr < TI / 8; rr += 2) {
         const int il = warp * (TI / 8) + rr;
         const int64_t i = i0 + il;
         if (i >= m) break;
-        const double2 lo = *reinterpret_cast<const double2 *>(&tile[il * SROW + 4 * lane]);
-        const double2 hi = *reinterpret_cast<const double2 *>(&tile[il * SROW + 4 * lane + 2]);
-        const double a[4] = { lo.x, lo.y, hi.x, hi.y };
+        const bool ok1 = i + 1 < m;
+        double a[2][4];
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+            const double2 lo = *reinterpret_cast<const double2 *>(&tile[(il + t) * SROW + 4 * lane]);
+            const double2 hi = *reinterpret_cast<const double2 *>(&tile[(il + t) * SROW + 4 * lane + 2]);
+            a[t][0] = lo.x; a[t][1] = lo.y; a[t][2] = hi.x; a[t][3] = hi.y;
+        }
         int8_t *dst = planes + i * kp + h0 + 4 * lane;
-        const int ex = __ldg(e + i);
-        if (MODE == 0) quad_residues<NB>(a, ex, N, dst, plane_stride);
-        else quad_bar(a, ex, dst);
+        const int ex0 = __ldg(e + i), ex1 = ok1 ? __ldg(e + i + 1) : 0;
+        if (MODE == 0) oct_residues<NB>(a, ex0, ex1, N, dst, kp, ok1, plane_stride);
+        else {
+            quad_bar(a[0], ex0, dst);
+            if (ok1) quad_bar(a[1], ex1, dst + kp);
+        }
     }
 }
 
@@ -211,14 +224,13 @@ k2_cols(int N, int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, 
             for (int u = 0; u < 4; u++) a[t][u] = (h + u < k) ? __ldg(col + h + u) : 0.0;
         }
     }
-#pragma unroll
-    for (int t = 0; t < 2; t++) {
-        const int64_t h = c * 256 + 128 * t + 4 * lane;
-        if (h < kp) {
-            int8_t *dst = planes + j * kp + h;
-            if (MODE == 0) quad_residues<NB>(a[t], ex, N, dst, plane_stride);
-            else quad_bar(a[t], ex, dst);
-        }
+    const int64_t h = c * 256 + 4 * lane;           // first quad; kp is a multiple of 128, so it is inside
+    int8_t *dst = planes + j * kp + h;
+    const bool ok1 = h + 128 < kp;
+    if (MODE == 0) oct_residues<NB>(a, ex, ex, N, dst, 128, ok1, plane_stride);
+    else {
+        quad_bar(a[0], ex, dst);
+        if (ok1) quad_bar(a[1], ex, dst + 128);
     }
 }
 
@@ -229,15 +241,9 @@ int oz2_convert_upload_tables(const Oz2HostTables &t)
     ConvTab h[OZ2_MAX_MODULI];
     for (int l = 0; l < OZ2_MAX_MODULI; l++) {
         const uint32_t p = t.mod[l].p;
-        h[l].negp = 0u - p;
-        h[l].magic = t.mod[l].magic;
-        h[l].half = t.mod[l].half;
-        const uint32_t two64 = (uint32_t)(((0xFFFFFFFFFFFFFFFFull % p) + 1ull) % p);            // 2^64 mod p
-        const uint32_t two32 = (uint32_t)(0x100000000ull % p);
-        const uint32_t two96 = (uint32_t)(((unsigned long long)two64 * two32) % p);             // 2^96 mod p
-        h[l].cneg2 = (p - two64) % p;
-        h[l].cneg3 = (p - two96) % p;
-        for (int i = 0; i < 3; i++) h[l].wb[i] = t.mod[l].wb[i];
+        h[l].invp = (float)(1.0 / (double)p);
+        h[l].negp = -(float)p;
+        for (int i = 0; i < 3; i++) { h[l].wb[i] = t.mod[l].wb[i]; h[l].pad[i] = 0; }
     }
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_conv, h, sizeof(h)));
     return 0;
