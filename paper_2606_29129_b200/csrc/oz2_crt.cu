@@ -110,54 +110,47 @@ __device__ __forceinline__ double crt_one(const uint32_t (&u)[N], int esum, uint
             }
         }
     }
-    const bool neg = (r[NW] >> 31) != 0;
+    const uint32_t negm = (uint32_t)((int32_t)r[NW] >> 31);
     if (cpp_out) {
-        uint32_t ext = neg ? 0xFFFFFFFFu : 0u;
         uint32_t w8[8];
 #pragma unroll
-        for (int t = 0; t < 8; t++) w8[t] = t <= NW ? r[t] : ext;
+        for (int t = 0; t < 8; t++) w8[t] = t <= NW ? r[t] : negm;
 #pragma unroll
         for (int t = 0; t < 4; t++) cpp_out[t] = ((unsigned long long)w8[2 * t + 1] << 32) | w8[2 * t];
     }
-    // ---- |C''| as NW words (|C''| <= P/2 < 2^(32 NW))
-    uint32_t a[NW];
-    {
-        unsigned long long cy = neg ? 1ull : 0ull;
-#pragma unroll
-        for (int t = 0; t < NW; t++) {
-            unsigned long long s = (unsigned long long)(neg ? ~r[t] : r[t]) + cy;
-            a[t] = (uint32_t)s;
-            cy = s >> 32;
-        }
-    }
-    // ---- top 64 bits, sticky, position of the leading one
-    int top_i = -1;
-#pragma unroll
-    for (int t = 0; t < NW; t++)
-        if (a[t]) top_i = t;
-    if (top_i < 0) return 0.0;
-    uint32_t x0 = 0, x1 = 0, x2 = 0, rest = 0;                        // words top, top-1, top-2, OR of the rest
-#pragma unroll
-    for (int t = 0; t < NW; t++) {
-        if (t == top_i) x0 = a[t];
-        else if (t == top_i - 1) x1 = a[t];
-        else if (t == top_i - 2) x2 = a[t];
-        else if (t < top_i - 2) rest |= a[t];
-    }
-    int lz = __clz((int)x0);
-    unsigned long long mant = ((unsigned long long)__funnelshift_l(x1, x0, lz) << 32) | __funnelshift_l(x2, x1, lz);
-    uint32_t sticky = ((lz ? (x2 << lz) : x2) | rest) ? 1u : 0u;
-    int pos = 32 * top_i + 31 - lz;                                   // |C''| in [2^pos, 2^(pos+1))
-    int sc = pos - 63 - esum;                                         // result = mant 2^sc
+    // ---- |C''| as three 64-bit pieces X2:X1:X0 (|C''| <= P/2 < 2^(32 NW) <= 2^160), branch-free negate
+    const unsigned long long m64 = (unsigned long long)(long long)(int32_t)negm;
+    auto W = [&](int t) -> uint32_t { return t <= NW ? r[t <= NW ? t : 0] : negm; };   // sign-extended word t
+    const unsigned long long R0 = ((unsigned long long)W(1) << 32) | W(0);
+    const unsigned long long R1 = ((unsigned long long)W(3) << 32) | W(2);
+    const unsigned long long R2 = ((unsigned long long)W(5) << 32) | W(4);
+    // two's-complement negate of the 192-bit value when negative: X = (R ^ m) + (m & 1)
+    const unsigned long long X0 = (R0 ^ m64) + (m64 & 1ull);
+    const unsigned long long c0 = (m64 & 1ull) & (unsigned long long)(X0 == 0ull);
+    const unsigned long long X1 = (R1 ^ m64) + c0;
+    const unsigned long long c1 = c0 & (unsigned long long)(X1 == 0ull);
+    const unsigned long long X2 = (R2 ^ m64) + c1;
+    // ---- leading piece, top 64 bits from the leading one, sticky bit
+    unsigned long long ptop, pmid, plow;
+    int base;
+    if (NW >= 5 && X2 != 0ull) { ptop = X2; pmid = X1; plow = X0; base = 128; }
+    else if (NW >= 3 && X1 != 0ull) { ptop = X1; pmid = X0; plow = 0ull; base = 64; }
+    else { ptop = X0; pmid = 0ull; plow = 0ull; base = 0; }
+    if (ptop == 0ull) return 0.0;
+    const int lz = __clzll((long long)ptop);
+    const unsigned long long mant = (ptop << lz) | ((pmid >> 1) >> (63 - lz));
+    const uint32_t sticky = (((pmid << lz) | plow) != 0ull) ? 1u : 0u;
+    const int pos = base + 63 - lz;                                   // |C''| in [2^pos, 2^(pos+1))
+    const int sc = pos - 63 - esum;                                   // result = mant 2^sc
     double v;
-    int Ex = pos - esum;
+    const int Ex = pos - esum;
     if (Ex >= -1020 && Ex <= 1021) {
-        double d = __ull2double_rn(mant | sticky);                    // the one rounding, ties to even
+        const double d = __ull2double_rn(mant | sticky);              // the one rounding, ties to even
         v = __longlong_as_double(__double_as_longlong(d) + ((long long)sc << 52));
     } else {
         v = round_scaled_slow(mant, sticky, sc);
     }
-    return neg ? -v : v;
+    return __longlong_as_double(__double_as_longlong(v) | (long long)(m64 << 63));
 }
 
 template <int N, bool WANT_CPP>
@@ -180,7 +173,7 @@ k4_crt(int64_t m, int64_t n, const uint8_t *__restrict__ U, int64_t mp, const in
         if (i0 + s >= m) { out[s] = 0.0; continue; }
         uint32_t u[N];
 #pragma unroll
-        for (int l = 0; l < N; l++) u[l] = (packed[l] >> (8 * s)) & 0xFFu;
+        for (int l = 0; l < N; l++) u[l] = __byte_perm(packed[l], 0u, 0x4440 + s);
         uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i0 + s) * 4 : nullptr;
         double cij = crt_one<N>(u, e[i0 + s] + fj, cpp);
         double t = alpha * cij;
