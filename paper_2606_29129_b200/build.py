@@ -25,7 +25,7 @@ def _stale(target, deps):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    headers = [os.path.join(CSRC, "oz2_common.cuh"), os.path.join(HERE, "..", "include", "ozaki2.h")]
+    headers = [os.path.join(CSRC, "oz2_common.cuh"), os.path.join(CSRC, "oz2_tc.cuh"), os.path.join(HERE, "..", "include", "ozaki2.h")]
     jobs = []
     objs = []
     for s in SOURCES:

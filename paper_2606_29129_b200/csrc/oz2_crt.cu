@@ -12,6 +12,8 @@
 // once.  HBM traffic: N bytes in + 8 bytes out per element; the kernel is templated on N so that all weight
 // words are constant-bank operands of fully unrolled multiply-adds.
 #include "oz2_common.cuh"
+#include "oz2_tc.cuh"
+#include <string.h>
 
 namespace {
 
@@ -47,28 +49,11 @@ __device__ __noinline__ double round_scaled_slow(unsigned long long mant, uint32
     return d;
 }
 
-template <int N>
-__device__ __forceinline__ double crt_one(const uint32_t (&u)[N], int esum, uint64_t *cpp_out)
+// C'' = rmod(C', P), RN_64(C'') 2^-esum from the words c[0..NW] of C' = sum_l w_l U_l (c[NW] < 2^13)
+template <int NW>
+__device__ __forceinline__ double crt_from_words(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum,
+                                                 uint64_t *cpp_out)
 {
-    constexpr int NW = words_of_P(N);
-    const Oz2CrtTab &T = c_crt[N];
-    // ---- C' = sum_l w_l U_l, word by word
-    unsigned long long acc[NW];
-#pragma unroll
-    for (int t = 0; t < NW; t++) acc[t] = 0;
-#pragma unroll
-    for (int l = 0; l < N; l++)
-#pragma unroll
-        for (int t = 0; t < NW; t++) acc[t] += (unsigned long long)T.w[l][t] * u[l];
-    uint32_t c[NW + 1];
-    unsigned long long carry = 0;
-#pragma unroll
-    for (int t = 0; t < NW; t++) {
-        unsigned long long s = acc[t] + carry;
-        c[t] = (uint32_t)s;
-        carry = s >> 32;
-    }
-    c[NW] = (uint32_t)carry;                                          // < 2^13
     // ---- Q = round(C' / P), estimated from the top three words
     double top = (double)(long long)(((unsigned long long)c[NW] << 32) | c[NW - 1]);
     if constexpr (NW >= 2) top = fma((double)c[NW - 2], 2.3283064365386963e-10, top);
@@ -153,6 +138,31 @@ __device__ __forceinline__ double crt_one(const uint32_t (&u)[N], int esum, uint
     return __longlong_as_double(__double_as_longlong(v) | (long long)(m64 << 63));
 }
 
+template <int N>
+__device__ __forceinline__ double crt_one(const uint32_t (&u)[N], int esum, uint64_t *cpp_out)
+{
+    constexpr int NW = words_of_P(N);
+    const Oz2CrtTab &T = c_crt[N];
+    // ---- C' = sum_l w_l U_l, word by word
+    unsigned long long acc[NW];
+#pragma unroll
+    for (int t = 0; t < NW; t++) acc[t] = 0;
+#pragma unroll
+    for (int l = 0; l < N; l++)
+#pragma unroll
+        for (int t = 0; t < NW; t++) acc[t] += (unsigned long long)T.w[l][t] * u[l];
+    uint32_t c[NW + 1];
+    unsigned long long carry = 0;
+#pragma unroll
+    for (int t = 0; t < NW; t++) {
+        unsigned long long s = acc[t] + carry;
+        c[t] = (uint32_t)s;
+        carry = s >> 32;
+    }
+    c[NW] = (uint32_t)carry;                                          // < 2^13
+    return crt_from_words<NW>(c, T, esum, cpp_out);
+}
+
 template <int N, bool WANT_CPP>
 __global__ void __launch_bounds__(128)
 k4_crt(int64_t m, int64_t n, const uint8_t *__restrict__ U, int64_t mp, const int32_t *__restrict__ e,
@@ -189,6 +199,152 @@ k4_crt(int64_t m, int64_t n, const uint8_t *__restrict__ U, int64_t mp, const in
     }
 }
 
+// =============================================================================================
+// Tensor-core CRT.  sum_l w_l U_l is itself a small dense contraction: with the weights cut into bytes,
+//     S[i][t] = sum_l U_l[i] * byte_t(w_l),   t = 0 .. 4 NW - 1,      C'[i] = sum_t S[i][t] 256^t,
+// i.e. (128 elements) x (K = moduli, zero padded to 32) x (16 or 32 byte slices): ONE tcgen05.mma kind::i8 per 128
+// elements (unsigned x unsigned, S < 2^21).  A = the U planes as they lie in memory ([l][j][i], i fastest) fetched
+// by TMA as an MN-major SWIZZLE_128B operand (planes >= N are zero filled by the TMA bounds check); B = a constant
+// 0.5 / 1 KB image of the weight bytes in shared memory (K-major, no swizzle).  This replaces 4 NW N wide
+// multiply-adds per element on the integer pipe; the epilogue threads (one element each) only fold the slices
+// into words and run crt_from_words.
+// =============================================================================================
+constexpr int K5_STAGES = 8, K5_NBUF = 8, K5_THREADS = 192;
+constexpr int K5_TILE_I = 128, K5_KPAD = 32;
+constexpr int K5_STAGE_BYTES = K5_TILE_I * K5_KPAD;          // 4 KB
+constexpr int K5_SMEM = K5_STAGES * K5_STAGE_BYTES + 1024 /*B image*/ + 1024 /*alignment*/ + 512 /*barriers*/;
+
+__device__ uint8_t g_wb_image[OZ2_MAX_MODULI + 1][1024];     // per N: B operand image (see upload)
+
+__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr)
+                 : "memory");
+}
+
+template <int NW, bool WANT_CPP>
+__global__ void __launch_bounds__(K5_THREADS)
+k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n, const int32_t *__restrict__ e,
+          const int32_t *__restrict__ f, double alpha, double beta, double *__restrict__ C, int64_t ldc,
+          uint64_t *__restrict__ Cpp)
+{
+    constexpr int NS = NW <= 4 ? 16 : 32;                    // byte slices = MMA N
+    // kind::i8 instruction descriptor: D = S32, A = B = unsigned 8 bit, A MN-major, B K-major, N = NS, M = 128
+    constexpr uint32_t IDESC = (2u << 4) | (1u << 15) | ((uint32_t)(NS >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t *wb = smem + K5_STAGES * K5_STAGE_BYTES;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(wb + 1024);
+    uint64_t *full = bars, *empty = bars + K5_STAGES, *tfull = bars + 2 * K5_STAGES, *tempty = tfull + K5_NBUF;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + K5_NBUF);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
+    const int64_t total = tiles_i * n;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < K5_STAGES; s++) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int b = 0; b < K5_NBUF; b++) { mbar_init(tfull + b, 1); mbar_init(tempty + b, 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapU) : "memory");
+    }
+    // B operand image: generic-proxy writes, then made visible to the async (tensor core) proxy
+    for (int t = threadIdx.x; t < 1024 / 16; t += K5_THREADS)
+        reinterpret_cast<uint4 *>(wb)[t] = reinterpret_cast<const uint4 *>(g_wb_image[N])[t];
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(K5_NBUF * NS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            int s = 0; uint32_t ph = 0;
+            for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+                const int64_t j = t / tiles_i, ib = t - j * tiles_i;
+                mbar_wait(empty + s, ph ^ 1u);
+                mbar_expect_tx(full + s, K5_STAGE_BYTES);
+                tma_load_3d(&mapU, full + s, smem + s * K5_STAGE_BYTES, (int)(ib * K5_TILE_I), (int)j, 0);
+                if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            int s = 0, b = 0; uint32_t ph = 0, bph = 0;
+            // B: K-major, no swizzle: core matrices 8 rows x 16 B; K-direction stride (LBO) 128 B, 8-row groups (SBO) 256 B
+            const uint64_t bdesc = (uint64_t)((smem_u32(wb) & 0x3FFFFu) >> 4) | ((uint64_t)(128u >> 4) << 16) |
+                                   ((uint64_t)(256u >> 4) << 32) | (1ull << 46);
+            for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+                mbar_wait(tempty + b, bph ^ 1u);
+                mbar_wait(full + s, ph);
+                tc_fence_after();
+                // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
+                const uint64_t adesc = (uint64_t)((smem_u32(smem + s * K5_STAGE_BYTES) & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) |
+                                       ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
+                tc_mma_i8(tmem_base + (uint32_t)(b * NS), adesc, bdesc, IDESC, 0u);
+                tc_commit(empty + s);
+                tc_commit(tfull + b);
+                if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
+                if (++b == K5_NBUF) { b = 0; bph ^= 1u; }
+            }
+        }
+    } else {
+        const int q = warp & 3;                              // TMEM lane quarter of this warp
+        const Oz2CrtTab &T = c_crt[N];
+        int b = 0; uint32_t bph = 0;
+        for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+            const int64_t j = t / tiles_i, ib = t - j * tiles_i;
+            const int64_t i = ib * K5_TILE_I + q * 32 + lane;
+            mbar_wait(tfull + b, bph);
+            tc_fence_after();
+            uint32_t S[NS];
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * NS);
+            if constexpr (NS == 16) {
+                tc_ld16(taddr, S);
+            } else {
+                uint32_t lo[16], hi[16];
+                tc_ld16(taddr, lo);
+                tc_ld16(taddr + 16u, hi);
+#pragma unroll
+                for (int u = 0; u < 16; u++) { S[u] = lo[u]; S[16 + u] = hi[u]; }
+            }
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty + b);
+            if (++b == K5_NBUF) { b = 0; bph ^= 1u; }
+            if (i < m) {
+                // C' words: V_k = sum_{b<4} S[4k+b] 256^b (< 2^46), then carries
+                uint32_t c[NW + 1];
+                unsigned long long carry = 0;
+#pragma unroll
+                for (int k = 0; k < NW; k++) {
+                    unsigned long long v = (unsigned long long)S[4 * k] + ((unsigned long long)S[4 * k + 1] << 8) +
+                                           ((unsigned long long)S[4 * k + 2] << 16) + ((unsigned long long)S[4 * k + 3] << 24) + carry;
+                    c[k] = (uint32_t)v;
+                    carry = v >> 32;
+                }
+                c[NW] = (uint32_t)carry;
+                uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr;
+                const double cij = crt_from_words<NW>(c, T, __ldg(e + i) + __ldg(f + j), cpp);
+                const double tt = alpha * cij;
+                double *dst = C + i + j * ldc;
+                *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
+            }
+        }
+    }
+    __syncthreads();
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(K5_NBUF * NS) : "memory");
+}
+
 template <int N>
 int launch_n(int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f, double alpha,
              double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
@@ -200,11 +356,53 @@ int launch_n(int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *
     return (int)cudaGetLastError();
 }
 
+template <int NW>
+int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f, double alpha,
+              double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
+{
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return (int)cudaErrorNotSupported;
+    // U planes [N][n][mp] -> 3-D map (i, j, l), box (128, 1, 32): rows i >= mp and planes l >= N are zero filled
+    CUtensorMap map;
+    cuuint64_t dims[3] = { (cuuint64_t)mp, (cuuint64_t)n, (cuuint64_t)N };
+    cuuint64_t strides[2] = { (cuuint64_t)mp, (cuuint64_t)(n * mp) };
+    cuuint32_t box[3] = { (cuuint32_t)K5_TILE_I, 1u, (cuuint32_t)K5_KPAD };
+    cuuint32_t estr[3] = { 1u, 1u, 1u };
+    CUresult r = enc(&map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(U), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    const int64_t tiles = ((m + K5_TILE_I - 1) / K5_TILE_I) * n;
+    const int per_sm = NW <= 4 ? 4 : 2;                   // TMEM: 128 / 256 columns per CTA
+    int64_t grid = (int64_t)sms * per_sm;
+    if (grid > tiles) grid = tiles;
+    if (Cpp) k5_crt_tc<NW, true><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, Cpp);
+    else k5_crt_tc<NW, false><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, nullptr);
+    oz2_count_launches(1);
+    return (int)cudaGetLastError();
+}
+
 } // namespace
 
 int oz2_crt_upload_tables(const Oz2HostTables &t)
 {
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_crt, t.crt, sizeof(t.crt)));
+    // B operand images of k5_crt_tc: element (slice s, modulus l) at (s/8) 256 + (l/16) 128 + (s%8) 16 + (l%16)
+    static uint8_t img[OZ2_MAX_MODULI + 1][1024];
+    memset(img, 0, sizeof(img));
+    for (int N = 2; N <= OZ2_MAX_MODULI; N++)
+        for (int l = 0; l < N; l++)
+            for (int sl = 0; sl < 4 * OZ2_MAX_WORDS && sl < 32; sl++) {
+                const uint8_t byte = (uint8_t)(t.crt[N].w[l][sl / 4] >> (8 * (sl % 4)));
+                img[N][(sl / 8) * 256 + (l / 16) * 128 + (sl % 8) * 16 + (l % 16)] = byte;
+            }
+    OZ2_CUDA_TRY(cudaMemcpyToSymbol(g_wb_image, img, sizeof(img)));
     return 0;
 }
 
@@ -212,12 +410,12 @@ int oz2_launch_crt(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, co
                    double alpha, double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
 {
     if (m <= 0 || n <= 0) return 0;
-    switch (N) {
-#define OZ2_CASE(NN) case NN: return launch_n<NN>(m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
-        OZ2_CASE(2) OZ2_CASE(3) OZ2_CASE(4) OZ2_CASE(5) OZ2_CASE(6) OZ2_CASE(7) OZ2_CASE(8) OZ2_CASE(9)
-        OZ2_CASE(10) OZ2_CASE(11) OZ2_CASE(12) OZ2_CASE(13) OZ2_CASE(14) OZ2_CASE(15) OZ2_CASE(16)
-        OZ2_CASE(17) OZ2_CASE(18) OZ2_CASE(19) OZ2_CASE(20)
-#undef OZ2_CASE
+    if (N < 2 || N > OZ2_MAX_MODULI) return -1;
+    switch (words_of_P(N)) {
+        case 1: return launch_tc<1>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        case 2: return launch_tc<2>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        case 3: return launch_tc<3>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        case 4: return launch_tc<4>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        default: return launch_tc<5>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
     }
-    return -1;
 }
