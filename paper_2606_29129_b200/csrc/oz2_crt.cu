@@ -209,7 +209,7 @@ k4_crt(int64_t m, int64_t n, const uint8_t *__restrict__ U, int64_t mp, const in
 // multiply-adds per element on the integer pipe; the epilogue threads (one element each) only fold the slices
 // into words and run crt_from_words.
 // =============================================================================================
-constexpr int K5_STAGES = 8, K5_NBUF = 8, K5_THREADS = 192;
+constexpr int K5_STAGES = 8, K5_NBUF = 8, K5_THREADS = 320;     // warps: TMA, MMA, 2 sets of 4 epilogue warps
 constexpr int K5_TILE_I = 128, K5_KPAD = 32;
 constexpr int K5_STAGE_BYTES = K5_TILE_I * K5_KPAD;          // 4 KB
 constexpr int K5_SMEM = K5_STAGES * K5_STAGE_BYTES + 1024 /*B image*/ + 1024 /*alignment*/ + 512 /*barriers*/;
@@ -227,7 +227,7 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16])
 }
 
 template <int NW, bool WANT_CPP>
-__global__ void __launch_bounds__(K5_THREADS)
+__global__ void __launch_bounds__(K5_THREADS, 4)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n, const int32_t *__restrict__ e,
           const int32_t *__restrict__ f, double alpha, double beta, double *__restrict__ C, int64_t ldc,
           uint64_t *__restrict__ Cpp)
@@ -245,6 +245,9 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
     const int64_t total = tiles_i * n;
+    // tile t = j * tiles_i + ib, walked with stride gridDim.x without a division per tile
+    const int64_t step_j = (int64_t)gridDim.x / tiles_i, step_i = (int64_t)gridDim.x - step_j * tiles_i;
+    int64_t j = (int64_t)blockIdx.x / tiles_i, ib = (int64_t)blockIdx.x - j * tiles_i;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < K5_STAGES; s++) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
@@ -269,11 +272,12 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
         if (lane == 0) {
             int s = 0; uint32_t ph = 0;
             for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-                const int64_t j = t / tiles_i, ib = t - j * tiles_i;
                 mbar_wait(empty + s, ph ^ 1u);
                 mbar_expect_tx(full + s, K5_STAGE_BYTES);
                 tma_load_3d(&mapU, full + s, smem + s * K5_STAGE_BYTES, (int)(ib * K5_TILE_I), (int)j, 0);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
+                ib += step_i; j += step_j;
+                if (ib >= tiles_i) { ib -= tiles_i; j++; }
             }
         }
     } else if (warp == 1) {
@@ -298,11 +302,19 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
         }
     } else {
         const int q = warp & 3;                              // TMEM lane quarter of this warp
+        const int set = (warp - 2) >> 2;                     // epilogue set 0 / 1 takes every second tile of the CTA
         const Oz2CrtTab &T = c_crt[N];
-        int b = 0; uint32_t bph = 0;
-        for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-            const int64_t j = t / tiles_i, ib = t - j * tiles_i;
+        int b = set; uint32_t bph = 0;
+        {   // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
+            const int64_t t0 = (int64_t)blockIdx.x + (int64_t)set * gridDim.x;
+            j = t0 / tiles_i; ib = t0 - j * tiles_i;
+        }
+        const int64_t step2_j = 2 * (int64_t)gridDim.x / tiles_i, step2_i = 2 * (int64_t)gridDim.x - step2_j * tiles_i;
+        for (int64_t t = (int64_t)blockIdx.x + (int64_t)set * gridDim.x; t < total; t += 2 * (int64_t)gridDim.x) {
             const int64_t i = ib * K5_TILE_I + q * 32 + lane;
+            const int64_t jcur = j;
+            ib += step2_i; j += step2_j;
+            if (ib >= tiles_i) { ib -= tiles_i; j++; }
             mbar_wait(tfull + b, bph);
             tc_fence_after();
             uint32_t S[NS];
@@ -320,7 +332,8 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty + b);
-            if (++b == K5_NBUF) { b = 0; bph ^= 1u; }
+            b += 2;
+            if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
             if (i < m) {
                 // C' words: V_k = sum_{b<4} S[4k+b] 256^b (< 2^46), then carries
                 uint32_t c[NW + 1];
@@ -333,10 +346,10 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
                     carry = v >> 32;
                 }
                 c[NW] = (uint32_t)carry;
-                uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr;
-                const double cij = crt_from_words<NW>(c, T, __ldg(e + i) + __ldg(f + j), cpp);
+                uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)jcur * m + i) * 4 : nullptr;
+                const double cij = crt_from_words<NW>(c, T, __ldg(e + i) + __ldg(f + jcur), cpp);
                 const double tt = alpha * cij;
-                double *dst = C + i + j * ldc;
+                double *dst = C + i + jcur * ldc;
                 *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
             }
         }
