@@ -1,0 +1,121 @@
+"""GPU accuracy / invariance report on BASELINE configs[1] (-m gpu): 1024^3, eq. (15) phi = 1.0, N = 8..20, the three
+scaling modes, plus the scale-invariance variant c in {2^-500, 1e-100, 1, 1e100, 2^500}.
+
+For every (N, mode) the CUDA result is compared bit for bit with the oracle's and its max elementwise relative error
+against the double-double reference is recorded; the table is written to
+gpurun_out/accuracy_report.md (copied to profiles/ by hand).  Assertions are the paper's claims as trends."""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import ozaki2_oracle as O
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+MODES = {0: "accu", 1: "fast", 2: "prop"}
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_29129_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def max_rel_err(C, hi, lo):
+    nz = hi != 0
+    return float(np.max(np.abs((C[nz] - hi[nz]) - lo[nz]) / np.abs(hi[nz])))
+
+
+def gpu_run(B, A, Bm, N, mode):
+    import torch
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    out = B.dgemm_stages(Ad, Bd, N, mode, want=("e", "f"))
+    torch.cuda.synchronize()
+    return B.device_to_colmajor(out["C"]), out["e"].cpu().numpy(), out["f"].cpu().numpy()
+
+
+def widths(M, ex, axis):
+    """effective bit width per row / column: log2 mu + floor(log2 max|.|) + 1."""
+    mx = np.max(np.abs(M), axis=axis)
+    E = np.frexp(mx)[1] - 1
+    w = (ex + E + 1)[mx > 0]
+    return int(w.min()), float(np.median(w)), int(w.max())
+
+
+def slab_violations(A, Bm, e, f, N, rows=48, cols=48):
+    """condition (1) on a slab with the full problem's exponents: (2 sum|a'||b'| >= P, 2|a'b'| >= P) counts."""
+    Ap = O.truncate(0, A[:rows], e[:rows])
+    Bp = O.truncate(1, Bm[:, :cols], f[:cols])
+    _, _, cnt = O.exact_product(N, Ap, Bp, want_words=False)
+    return cnt["violations"], cnt["wrong"]
+
+
+def test_config1_error_vs_moduli_and_modes(B):
+    c = W.CONFIGS[1]
+    A, Bm = W.config_matrices(1)
+    hi, lo = O.dd_reference(A, Bm)
+    lines = ["# Accuracy on BASELINE configs[1]: m=n=k=1024, eq.(15) phi=1.0 (GPU result; bit-identical to the oracle)",
+             "", "max elementwise relative error vs the double-double reference (P:268); FP64 matmul for scale: "
+             f"{max_rel_err(A @ Bm, hi, lo):.3e}", "", "| N | accurate | original fast | revised fast (prop) |", "|---|---|---|---|"]
+    errs = {}
+    for N in c["moduli"]:
+        row = []
+        for mode in (0, 1, 2):
+            Cg, e, f = gpu_run(B, A, Bm, N, mode)
+            if N in (8, 14, 16, 20):                       # full-size parity against the oracle (bit-exact)
+                Co, eo, fo = O.dgemm(A, Bm, N, mode, return_exponents=True)
+                assert np.array_equal(e, eo) and np.array_equal(f, fo), (N, mode)
+                assert np.array_equal(Cg, Co), (N, mode)
+            errs[(N, mode)] = max_rel_err(Cg, hi, lo)
+            row.append(f"{errs[(N, mode)]:.3e}")
+        lines.append(f"| {N} | " + " | ".join(row) + " |")
+    # P:377 errors fall as N grows until the FP64 floor; P:383 prop ~ accu, fast worse at phi >= 1
+    assert errs[(8, 2)] > 1e3 * errs[(12, 2)] > 1e6 * errs[(16, 2)]
+    for N in c["moduli"]:
+        assert errs[(N, 2)] <= 32 * errs[(N, 0)], N
+    assert errs[(20, 2)] < 1e-15 and errs[(20, 0)] < 1e-15
+    assert errs[(14, 1)] > 4 * errs[(14, 2)]
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "accuracy_report.md"), "w") as fh:
+        fh.write("\n".join(lines) + "\n")
+
+
+def test_config1_scale_invariance_variant(B):
+    A0, B0 = W.config_matrices(1)
+    N = 16
+    lines = ["", f"# Scale-invariance variant (A, B both times c), N = {N}: effective bit width of the rows of A (min/median/max),",
+             "condition-(1) violations and wrong recoveries on a 48x48 slab (exact 256-bit product), max rel err vs double-double",
+             "", "| c | mode | width A | width B | violations | wrong | max rel err |", "|---|---|---|---|---|---|---|"]
+    ref = {}
+    for c, cname in zip(W.SCALE_CONSTANTS, ("2^-500", "1e-100", "1", "1e100", "2^500")):
+        A, Bm = A0 * c, B0 * c
+        hi, lo = O.dd_reference(A, Bm)
+        for mode in (0, 1, 2):
+            Cg, e, f = gpu_run(B, A, Bm, N, mode)
+            wa, wb = widths(A, e, 1), widths(Bm, f, 0)
+            viol, wrong = slab_violations(A, Bm, e, f, N)
+            err = max_rel_err(Cg, hi, lo)
+            lines.append(f"| {cname} | {MODES[mode]} | {wa[0]}/{wa[1]:.0f}/{wa[2]} | {wb[0]}/{wb[1]:.0f}/{wb[2]} | {viol} | {wrong} | {err:.3e} |")
+            ref[(cname, mode)] = (Cg, e, f, wa, err, viol)
+            if mode != 1:
+                assert viol == 0, (cname, mode)
+    # power-of-two scalings: revised mode is bit-invariant (exponents shift by -s, C scales by c^2 exactly)
+    C1, e1, f1, w1, err1, _ = ref[("1", 2)]
+    for cname, s in (("2^-500", -500), ("2^500", 500)):
+        Cc, ec, fc, wc, errc, _ = ref[(cname, 2)]
+        assert np.array_equal(ec, e1 - s) and np.array_equal(fc, f1 - s)
+        assert np.array_equal(Cc, np.ldexp(C1, 2 * s))
+        assert wc == w1
+    # non-powers of two move the width by at most one bit (reading R12); the original fast mode loses or gains bits
+    for cname in ("1e-100", "1e100"):
+        assert abs(ref[(cname, 2)][3][1] - w1[1]) <= 1
+    assert ref[("2^500", 1)][3][1] < w1[1] - 8                    # fast mode: width collapses for large inputs
+    assert ref[("2^-500", 1)][5] > 0                               # and violates condition (1) for small ones
+    with open(os.path.join(ROOT, "gpurun_out", "accuracy_report.md"), "a") as fh:
+        fh.write("\n".join(lines) + "\n")
