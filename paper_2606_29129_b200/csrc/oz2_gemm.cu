@@ -10,7 +10,7 @@
 //     INT32 accumulators live in tensor memory (2 x 256 columns, double buffered), they never touch HBM,
 //   * epilogue: 4 warps read the accumulator with tcgen05.ld, reduce mod p_l and write one byte per element,
 //     overlapping the MMAs of the next tile,
-//   * persistent grid (one CTA per SM), static tile order: modulus-major, then groups of 16 M-tiles so that the
+//   * persistent grid (one CTA per SM), static tile order: modulus-major, then groups of 32 M-tiles so that the
 //     148 tiles in flight share A / B panels in L2.
 // INT32 accumulation wraps (never saturates): with reading R6 that keeps k <= 2^17 exact for p = 256.
 #include "oz2_common.cuh"
@@ -30,7 +30,7 @@ constexpr int B_STAGE_BYTES = TILE_N * TILE_K;    // 32 KB
 constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
 constexpr int NUM_THREADS = 192;                  // warp 0: TMA, warp 1: MMA + TMEM alloc, warps 2..5: epilogue
-constexpr int GROUP_M = 16;
+constexpr int GROUP_M = 32;
 
 // tcgen05 instruction descriptor (kind::i8): D = S32, A = B = signed 8 bit, both K-major, N = 256, M = 128
 constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TILE_N >> 3) << 17) |

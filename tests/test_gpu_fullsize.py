@@ -1,0 +1,85 @@
+"""Full-size parity (-m gpu): BASELINE configs 2, 3, 4 in the launch configuration bench.py times (plain ozaki2_dgemm,
+device-resident inputs), checked on sampled rows x columns that the oracle computes one by one.
+
+Given the exponents, every later stage is local to a row of A and a column of B, so the oracle is run on the sampled
+rows / columns with the GPU's exponents and must reproduce the GPU's C bit for bit; the exponents themselves are
+checked against the oracle on the same samples (modes 1, 2: a row's exponent depends on that row only; mode 0: on that
+row of A and ALL of B, which the oracle gets)."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import ozaki2_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_29129_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def sample(count, size, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    idx = set(rng.integers(0, size, size=count).tolist()) | {0, size - 1, size // 2 - 1, 127, 128}
+    return np.array(sorted(i for i in idx if i < size))
+
+
+def oracle_slab_given_exponents(N, As, Bs, e, f):
+    RA, RB = O.residues(0, N, As, e), O.residues(1, N, Bs, f)
+    U, maxR = O.products(N, RA, RB)
+    return O.unscale(O.crt(N, U), e, f), maxR
+
+
+@pytest.mark.parametrize("config,N,modes,nrows,ncols", [
+    (2, 16, (2, 1, 0), 12, 40),          # 8192^3, headline
+    (2, 18, (2,), 12, 40),               # three-word conversion path at full size
+    (3, 20, (2, 0), 8, 24),              # 16384^3, phi = 4, N = 20
+    (4, 16, (2, 0), 8, 24),              # 4096 x 4096 x 65536: INT32 headroom at long k
+])
+def test_fullsize_sampled_parity(B, config, N, modes, nrows, ncols):
+    import torch
+    c = W.CONFIGS[config]
+    m, n, k = c["m"], c["n"], c["k"]
+    A, Bm = W.config_matrices(config)
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    rows, cols = sample(nrows, m, 11 * config + N), sample(ncols, n, 13 * config + N)
+    As, Bs = np.asfortranarray(A[rows, :]), np.asfortranarray(Bm[:, cols])
+    for mode in modes:
+        B.ensure_workspace(m, n, k, N, mode)
+        Cd = torch.empty((n, m), dtype=torch.float64, device="cuda")
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+        for x in ev:
+            x.record()
+        # the same call bench.py times; exponents read back from the workspace copy that dgemm_stages provides
+        out = B.dgemm_stages(Ad, Bd, N, mode, C_dev=Cd, want=("e", "f"))
+        assert B.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode) == 0
+        torch.cuda.synchronize()
+        e, f = out["e"].cpu().numpy(), out["f"].cpu().numpy()
+        Cg = Cd[torch.from_numpy(cols).cuda()][:, torch.from_numpy(rows).cuda()].cpu().numpy().T
+        # exponents on the samples
+        if mode != 0:
+            eo, _ = O.exponents(mode, N, As, Bs[:, :1])
+            _, fo = O.exponents(mode, N, As[:1, :], Bs)
+        else:
+            eo, _ = O.exponents(0, N, As, Bm)              # rows of the sample against ALL columns
+            _, fo = O.exponents(0, N, A, Bs)               # ALL rows against the sampled columns
+        assert np.array_equal(e[rows], eo), (config, N, mode, "e")
+        assert np.array_equal(f[cols], fo), (config, N, mode, "f")
+        Co, maxR = oracle_slab_given_exponents(N, As, Bs, e[rows], f[cols])
+        assert maxR <= 2 ** 31
+        assert np.array_equal(Cg, Co), (config, N, mode, "C")
+        # and the result is a good product: error vs double-double on the sample
+        hi, lo = O.dd_reference(As, Bs)
+        nz = hi != 0
+        err = np.max(np.abs((Cg[nz] - hi[nz]) - lo[nz]) / np.abs(hi[nz]))
+        if mode != 1:
+            assert err < {16: 1e-10, 18: 1e-13, 20: 1e-14}[N], (config, N, mode, err)
+        del Cd, out
+    del Ad, Bd
+    torch.cuda.empty_cache()

@@ -73,7 +73,7 @@ def test_config0_128_all_stages(B, mode):
     (200, 77, 333, 14, 2), (1, 1, 1, 2, 2), (129, 257, 127, 9, 1), (37, 300, 1000, 16, 0), (130, 40, 129, 17, 2),
     (64, 513, 260, 20, 0), (255, 255, 4097, 20, 2), (16, 16, 16, 3, 1), (300, 5, 31, 15, 0), (5, 300, 2049, 8, 2),
     (260, 260, 100, 12, 2), (128, 256, 128, 4, 2), (131, 100, 777, 5, 0), (100, 131, 64, 18, 1), (77, 77, 77, 13, 2),
-    (33, 65, 640, 6, 2), (90, 70, 50, 7, 1), (70, 90, 150, 10, 0), (50, 60, 70, 11, 2), (61, 67, 71, 19, 0),
+    (33, 65, 640, 6, 2), (90, 70, 50, 7, 1), (48, 40, 131072, 14, 2), (40, 24, 131072, 20, 0), (70, 90, 150, 10, 0), (50, 60, 70, 11, 2), (61, 67, 71, 19, 0),
 ])
 def test_ragged_shapes_and_every_moduli_count(B, m, n, k, N, mode):
     A, Bm = W.eq15_matrices(m, n, k, 1.0, 1000 + m + n + k + N)
