@@ -209,72 +209,109 @@ k4_crt(int64_t m, int64_t n, const uint8_t *__restrict__ U, int64_t mp, const in
 // multiply-adds per element on the integer pipe; the epilogue threads (one element each) only fold the slices
 // into words and run crt_from_words.
 // =============================================================================================
-constexpr int K5_STAGES = 8, K5_NBUF = 8, K5_THREADS = 320;     // warps: TMA, MMA, 2 sets of 4 epilogue warps
-constexpr int K5_TILE_I = 128, K5_KPAD = 32;
-constexpr int K5_STAGE_BYTES = K5_TILE_I * K5_KPAD;          // 4 KB
+constexpr int K5_STAGES = 4, K5_NBUF = 4, K5_THREADS = 320;     // warps: TMA, MMA, 2 sets of 4 epilogue warps
+constexpr int K5_TILE_I = 256, K5_KPAD = 32;                    // one pipeline step = 2 MMAs of 128 elements
+constexpr int K5_STAGE_BYTES = K5_TILE_I * K5_KPAD;             // 8 KB
 constexpr int K5_SMEM = K5_STAGES * K5_STAGE_BYTES + 1024 /*B image*/ + 1024 /*alignment*/ + 512 /*barriers*/;
 
-__device__ uint8_t g_wb_image[OZ2_MAX_MODULI + 1][1024];     // per N: B operand image (see upload)
+__device__ uint8_t g_wb_image[OZ2_MAX_MODULI + 1][1024];        // per N: B operand image (see upload)
 
-__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16])
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
 {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                 : "r"(taddr)
-                 : "memory");
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+
+// fold the byte slices S[0 .. 4 NW) of one element into C' and finish (C'' -> C -> alpha / beta -> store)
+template <int NW, bool WANT_CPP>
+__device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T, int64_t i, int64_t j, int64_t m, int esum,
+                                          double alpha, double beta, double *__restrict__ C, int64_t ldc,
+                                          uint64_t *__restrict__ Cpp)
+{
+    uint32_t c[NW + 1];
+    unsigned long long carry = 0;
+#pragma unroll
+    for (int k = 0; k < NW; k++) {       // V_k = sum_{b<4} S[4k+b] 256^b (< 2^46), then carries
+        unsigned long long v = (unsigned long long)S[4 * k] + ((unsigned long long)S[4 * k + 1] << 8) +
+                               ((unsigned long long)S[4 * k + 2] << 16) + ((unsigned long long)S[4 * k + 3] << 24) + carry;
+        c[k] = (uint32_t)v;
+        carry = v >> 32;
+    }
+    c[NW] = (uint32_t)carry;
+    uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr;
+    const double cij = crt_from_words<NW>(c, T, esum, cpp);
+    const double tt = alpha * cij;
+    double *dst = C + i + j * ldc;
+    *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
 }
 
 template <int NW, bool WANT_CPP>
-__global__ void __launch_bounds__(K5_THREADS, 4)
+__global__ void __launch_bounds__(K5_THREADS, 3)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n, const int32_t *__restrict__ e,
           const int32_t *__restrict__ f, double alpha, double beta, double *__restrict__ C, int64_t ldc,
           uint64_t *__restrict__ Cpp)
 {
     constexpr int NS = NW <= 4 ? 16 : 32;                    // byte slices = MMA N
+    constexpr int BUF_COLS = 2 * NS;                         // two 128-element MMAs per accumulator buffer
     // kind::i8 instruction descriptor: D = S32, A = B = unsigned 8 bit, A MN-major, B K-major, N = NS, M = 128
     constexpr uint32_t IDESC = (2u << 4) | (1u << 15) | ((uint32_t)(NS >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint8_t *wb = smem + K5_STAGES * K5_STAGE_BYTES;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(wb + 1024);
-    uint64_t *full = bars, *empty = bars + K5_STAGES, *tfull = bars + 2 * K5_STAGES, *tempty = tfull + K5_NBUF;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + K5_NBUF);
+    const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;           // shared-space addresses from here on
+    const uint32_t wb = smem0 + K5_STAGES * K5_STAGE_BYTES;
+    const uint32_t full = wb + 1024, empty = full + 8 * K5_STAGES, tfull = empty + 8 * K5_STAGES, tempty = tfull + 8 * K5_NBUF;
+    const uint32_t tmem_slot = tempty + 8 * K5_NBUF;
+    uint8_t *gen0 = smem_raw + (smem0 - smem_u32(smem_raw));                // generic pointer to the aligned base
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
     const int64_t total = tiles_i * n;
-    // tile t = j * tiles_i + ib, walked with stride gridDim.x without a division per tile
-    const int64_t step_j = (int64_t)gridDim.x / tiles_i, step_i = (int64_t)gridDim.x - step_j * tiles_i;
-    int64_t j = (int64_t)blockIdx.x / tiles_i, ib = (int64_t)blockIdx.x - j * tiles_i;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < K5_STAGES; s++) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int b = 0; b < K5_NBUF; b++) { mbar_init(tfull + b, 1); mbar_init(tempty + b, 4); }
+        for (int s = 0; s < K5_STAGES; s++) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(full + 8 * s));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(empty + 8 * s));
+        }
+        for (int b = 0; b < K5_NBUF; b++) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(tfull + 8 * b));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 4;" ::"r"(tempty + 8 * b));
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapU) : "memory");
     }
     // B operand image: generic-proxy writes, then made visible to the async (tensor core) proxy
     for (int t = threadIdx.x; t < 1024 / 16; t += K5_THREADS)
-        reinterpret_cast<uint4 *>(wb)[t] = reinterpret_cast<const uint4 *>(g_wb_image[N])[t];
+        reinterpret_cast<uint4 *>(gen0 + K5_STAGES * K5_STAGE_BYTES)[t] = reinterpret_cast<const uint4 *>(g_wb_image[N])[t];
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(K5_NBUF * NS) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "n"(K5_NBUF * BUF_COLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
     if (warp == 0) {
         if (lane == 0) {
+            // tile t = j * tiles_i + ib, walked with stride gridDim.x without a division per tile
+            const int64_t step_j = (int64_t)gridDim.x / tiles_i, step_i = (int64_t)gridDim.x - step_j * tiles_i;
+            int64_t j = (int64_t)blockIdx.x / tiles_i, ib = (int64_t)blockIdx.x - j * tiles_i;
             int s = 0; uint32_t ph = 0;
             for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-                mbar_wait(empty + s, ph ^ 1u);
-                mbar_expect_tx(full + s, K5_STAGE_BYTES);
-                tma_load_3d(&mapU, full + s, smem + s * K5_STAGE_BYTES, (int)(ib * K5_TILE_I), (int)j, 0);
+                mbar_wait_a(empty + 8 * s, ph ^ 1u);
+                mbar_expect_tx_a(full + 8 * s, K5_STAGE_BYTES);
+                const uint32_t dst = smem0 + s * K5_STAGE_BYTES;
+                tma_load_3d_a(&mapU, full + 8 * s, dst, (int)(ib * K5_TILE_I), (int)j, 0);
+                tma_load_3d_a(&mapU, full + 8 * s, dst + K5_STAGE_BYTES / 2, (int)(ib * K5_TILE_I + 128), (int)j, 0);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
                 ib += step_i; j += step_j;
                 if (ib >= tiles_i) { ib -= tiles_i; j++; }
@@ -284,18 +321,20 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
         if (lane == 0) {
             int s = 0, b = 0; uint32_t ph = 0, bph = 0;
             // B: K-major, no swizzle: core matrices 8 rows x 16 B; K-direction stride (LBO) 128 B, 8-row groups (SBO) 256 B
-            const uint64_t bdesc = (uint64_t)((smem_u32(wb) & 0x3FFFFu) >> 4) | ((uint64_t)(128u >> 4) << 16) |
+            const uint64_t bdesc = (uint64_t)((wb & 0x3FFFFu) >> 4) | ((uint64_t)(128u >> 4) << 16) |
                                    ((uint64_t)(256u >> 4) << 32) | (1ull << 46);
+            // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
+            const uint64_t adesc0 = ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
             for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-                mbar_wait(tempty + b, bph ^ 1u);
-                mbar_wait(full + s, ph);
+                mbar_wait_a(tempty + 8 * b, bph ^ 1u);
+                mbar_wait_a(full + 8 * s, ph);
                 tc_fence_after();
-                // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
-                const uint64_t adesc = (uint64_t)((smem_u32(smem + s * K5_STAGE_BYTES) & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) |
-                                       ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
-                tc_mma_i8(tmem_base + (uint32_t)(b * NS), adesc, bdesc, IDESC, 0u);
-                tc_commit(empty + s);
-                tc_commit(tfull + b);
+                const uint32_t sa = smem0 + s * K5_STAGE_BYTES;
+                tc_mma_i8(tmem_base + (uint32_t)(b * BUF_COLS), adesc0 | (uint64_t)((sa & 0x3FFFFu) >> 4), bdesc, IDESC, 0u);
+                tc_mma_i8(tmem_base + (uint32_t)(b * BUF_COLS + NS), adesc0 | (uint64_t)(((sa + K5_STAGE_BYTES / 2) & 0x3FFFFu) >> 4),
+                          bdesc, IDESC, 0u);
+                tc_commit_a(empty + 8 * s);
+                tc_commit_a(tfull + 8 * b);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
                 if (++b == K5_NBUF) { b = 0; bph ^= 1u; }
             }
@@ -305,68 +344,39 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
         const int set = (warp - 2) >> 2;                     // epilogue set 0 / 1 takes every second tile of the CTA
         const Oz2CrtTab &T = c_crt[N];
         int b = set; uint32_t bph = 0;
-        {   // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
-            const int64_t t0 = (int64_t)blockIdx.x + (int64_t)set * gridDim.x;
-            j = t0 / tiles_i; ib = t0 - j * tiles_i;
-        }
-        const int64_t step2_j = 2 * (int64_t)gridDim.x / tiles_i, step2_i = 2 * (int64_t)gridDim.x - step2_j * tiles_i;
-        for (int64_t t = (int64_t)blockIdx.x + (int64_t)set * gridDim.x; t < total; t += 2 * (int64_t)gridDim.x) {
+        // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
+        const int64_t t0 = (int64_t)blockIdx.x + (int64_t)set * gridDim.x;
+        int64_t j = t0 / tiles_i, ib = t0 - j * tiles_i;
+        const int64_t step_j = 2 * (int64_t)gridDim.x / tiles_i, step_i = 2 * (int64_t)gridDim.x - step_j * tiles_i;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
+        for (int64_t t = t0; t < total; t += 2 * (int64_t)gridDim.x) {
             const int64_t i = ib * K5_TILE_I + q * 32 + lane;
             const int64_t jcur = j;
-            ib += step2_i; j += step2_j;
+            ib += step_i; j += step_j;
             if (ib >= tiles_i) { ib -= tiles_i; j++; }
-            mbar_wait(tfull + b, bph);
+            const int fj = __ldg(f + jcur);
+            const int e0 = i < m ? __ldg(e + i) : 0, e1 = i + 128 < m ? __ldg(e + i + 128) : 0;
+            mbar_wait_a(tfull + 8 * b, bph);
             tc_fence_after();
-            uint32_t S[NS];
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * NS);
+            uint32_t S[BUF_COLS];
             if constexpr (NS == 16) {
-                tc_ld16(taddr, S);
+                tc_ld32(lane_base + (uint32_t)(b * BUF_COLS), *reinterpret_cast<uint32_t(*)[32]>(S));
             } else {
-                uint32_t lo[16], hi[16];
-                tc_ld16(taddr, lo);
-                tc_ld16(taddr + 16u, hi);
-#pragma unroll
-                for (int u = 0; u < 16; u++) { S[u] = lo[u]; S[16 + u] = hi[u]; }
+                tc_ld32(lane_base + (uint32_t)(b * BUF_COLS), *reinterpret_cast<uint32_t(*)[32]>(S));
+                tc_ld32(lane_base + (uint32_t)(b * BUF_COLS + 32), *reinterpret_cast<uint32_t(*)[32]>(S + 32));
             }
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tempty + b);
+            if (lane == 0) mbar_arrive_a(tempty + 8 * b);
             b += 2;
             if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
-            if (i < m) {
-                // C' words: V_k = sum_{b<4} S[4k+b] 256^b (< 2^46), then carries
-                uint32_t c[NW + 1];
-                unsigned long long carry = 0;
-#pragma unroll
-                for (int k = 0; k < NW; k++) {
-                    unsigned long long v = (unsigned long long)S[4 * k] + ((unsigned long long)S[4 * k + 1] << 8) +
-                                           ((unsigned long long)S[4 * k + 2] << 16) + ((unsigned long long)S[4 * k + 3] << 24) + carry;
-                    c[k] = (uint32_t)v;
-                    carry = v >> 32;
-                }
-                c[NW] = (uint32_t)carry;
-                uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)jcur * m + i) * 4 : nullptr;
-                const double cij = crt_from_words<NW>(c, T, __ldg(e + i) + __ldg(f + jcur), cpp);
-                const double tt = alpha * cij;
-                double *dst = C + i + jcur * ldc;
-                *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
-            }
+            if (i < m) k5_finish<NW, WANT_CPP>(S, T, i, jcur, m, e0 + fj, alpha, beta, C, ldc, Cpp);
+            if (i + 128 < m) k5_finish<NW, WANT_CPP>(S + NS, T, i + 128, jcur, m, e1 + fj, alpha, beta, C, ldc, Cpp);
         }
     }
     __syncthreads();
-    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(K5_NBUF * NS) : "memory");
-}
-
-template <int N>
-int launch_n(int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f, double alpha,
-             double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
-{
-    dim3 grid((unsigned)n, (unsigned)((m + 511) / 512));
-    if (Cpp) k4_crt<N, true><<<grid, 128, 0, st>>>(m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp);
-    else k4_crt<N, false><<<grid, 128, 0, st>>>(m, n, U, mp, e, f, alpha, beta, C, ldc, nullptr);
-    oz2_count_launches(1);
-    return (int)cudaGetLastError();
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(K5_NBUF * BUF_COLS) : "memory");
 }
 
 template <int NW>
@@ -379,7 +389,7 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
     CUtensorMap map;
     cuuint64_t dims[3] = { (cuuint64_t)mp, (cuuint64_t)n, (cuuint64_t)N };
     cuuint64_t strides[2] = { (cuuint64_t)mp, (cuuint64_t)(n * mp) };
-    cuuint32_t box[3] = { (cuuint32_t)K5_TILE_I, 1u, (cuuint32_t)K5_KPAD };
+    cuuint32_t box[3] = { 128u, 1u, (cuuint32_t)K5_KPAD };
     cuuint32_t estr[3] = { 1u, 1u, 1u };
     CUresult r = enc(&map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(U), dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -392,7 +402,7 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
     const int64_t tiles = ((m + K5_TILE_I - 1) / K5_TILE_I) * n;
-    const int per_sm = NW <= 4 ? 4 : 2;                   // TMEM: 128 / 256 columns per CTA
+    const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads
     int64_t grid = (int64_t)sms * per_sm;
     if (grid > tiles) grid = tiles;
     if (Cpp) k5_crt_tc<NW, true><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, Cpp);
