@@ -5,12 +5,12 @@
 //   C   = RN_64(C'') 2^-(e_i+f_j)                              (Step 4; reading R8)
 //   out = alpha C (+ beta C_in)                                (reading R9)
 //
-// Everything up to the single rounding RN_64 is EXACT integer arithmetic on 32-bit words held in registers
-// (the weights have up to 156 bits, C' up to 169): sum_l w_{l,t} U_l per word with 64-bit accumulators,
-// carry propagation, a quotient estimate Q ~ C'/P in FP64 (|error| < 2^-30; the rare near-half cases take an
-// exact compare against P/2), C'' = C' - Q P, then a 64-bit normalised mantissa with a sticky bit is rounded
-// once.  HBM traffic: N bytes in + 8 bytes out per element; the kernel is templated on N so that all weight
-// words are constant-bank operands of fully unrolled multiply-adds.
+// Everything up to the single rounding RN_64 is EXACT integer arithmetic (the weights have up to 156 bits, C' up
+// to 169).  The sum over the moduli is a dense contraction and runs on the tensor cores (k5_crt_tc below: one
+// tcgen05.mma kind::i8 per 128 elements over byte-sliced weights); the epilogue threads fold the byte slices into
+// 32-bit words, estimate Q ~ C'/P in FP64 (|error| < 2^-30; the rare near-half cases take an exact compare
+// against P/2), form C'' = C' - Q P in two's complement, and round a 64-bit normalised mantissa with a sticky
+// bit once.  HBM traffic: N bytes in + 8 bytes out per element.
 #include "oz2_common.cuh"
 #include "oz2_tc.cuh"
 #include <string.h>
@@ -136,67 +136,6 @@ __device__ __forceinline__ double crt_from_words(const uint32_t (&c)[NW + 1], co
         v = round_scaled_slow(mant, sticky, sc);
     }
     return __longlong_as_double(__double_as_longlong(v) | (long long)(m64 << 63));
-}
-
-template <int N>
-__device__ __forceinline__ double crt_one(const uint32_t (&u)[N], int esum, uint64_t *cpp_out)
-{
-    constexpr int NW = words_of_P(N);
-    const Oz2CrtTab &T = c_crt[N];
-    // ---- C' = sum_l w_l U_l, word by word
-    unsigned long long acc[NW];
-#pragma unroll
-    for (int t = 0; t < NW; t++) acc[t] = 0;
-#pragma unroll
-    for (int l = 0; l < N; l++)
-#pragma unroll
-        for (int t = 0; t < NW; t++) acc[t] += (unsigned long long)T.w[l][t] * u[l];
-    uint32_t c[NW + 1];
-    unsigned long long carry = 0;
-#pragma unroll
-    for (int t = 0; t < NW; t++) {
-        unsigned long long s = acc[t] + carry;
-        c[t] = (uint32_t)s;
-        carry = s >> 32;
-    }
-    c[NW] = (uint32_t)carry;                                          // < 2^13
-    return crt_from_words<NW>(c, T, esum, cpp_out);
-}
-
-template <int N, bool WANT_CPP>
-__global__ void __launch_bounds__(128)
-k4_crt(int64_t m, int64_t n, const uint8_t *__restrict__ U, int64_t mp, const int32_t *__restrict__ e,
-       const int32_t *__restrict__ f, double alpha, double beta, double *__restrict__ C, int64_t ldc,
-       uint64_t *__restrict__ Cpp)
-{
-    const int64_t i0 = 4 * ((int64_t)blockIdx.y * 128 + threadIdx.x);
-    const int64_t j = blockIdx.x;
-    if (i0 >= m) return;
-    const int64_t plane = n * mp;
-    uint32_t packed[N];
-#pragma unroll
-    for (int l = 0; l < N; l++) packed[l] = __ldg(reinterpret_cast<const uint32_t *>(U + l * plane + j * mp + i0));
-    const int fj = f[j];
-    double out[4];
-#pragma unroll 1
-    for (int s = 0; s < 4; s++) {
-        if (i0 + s >= m) { out[s] = 0.0; continue; }
-        uint32_t u[N];
-#pragma unroll
-        for (int l = 0; l < N; l++) u[l] = __byte_perm(packed[l], 0u, 0x4440 + s);
-        uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i0 + s) * 4 : nullptr;
-        double cij = crt_one<N>(u, e[i0 + s] + fj, cpp);
-        double t = alpha * cij;
-        double *dst = C + (i0 + s) + j * ldc;
-        out[s] = (beta == 0.0) ? t : fma(beta, *dst, t);
-    }
-    double *dst = C + i0 + j * ldc;
-    if (i0 + 3 < m && ((((uintptr_t)dst) & 15) == 0)) {
-        reinterpret_cast<double2 *>(dst)[0] = make_double2(out[0], out[1]);
-        reinterpret_cast<double2 *>(dst)[1] = make_double2(out[2], out[3]);
-    } else {
-        for (int s = 0; s < 4 && i0 + s < m; s++) dst[s] = out[s];
-    }
 }
 
 // =============================================================================================
