@@ -72,7 +72,11 @@ int ozaki2_set_workspace(void *device_ptr, size_t bytes);
 
 /*
  * The same call with HOST buffers: copies A and B to the device, runs ozaki2_dgemm, copies C
- * back (and C in first if beta != 0), all on `stream`, then synchronises the stream.
+ * back (and C in first if beta != 0), then synchronises `stream`.  For the two fast modes and
+ * n >= 512 the work is cut into column panels of B / C: the kernels stay on `stream`, the copies
+ * run on two library-owned streams ordered after `stream` by events, so that the H2D copy of the
+ * next panel and the D2H copy of the previous one overlap the kernels (same results bit for bit:
+ * e_i depends on row i of A only, f_j on column j of B only).
  * `device_scratch` is a caller-owned device buffer of at least
  * ozaki2_host_scratch_bytes(m, n, k) bytes that receives the device copies of A, B, C.
  * Host buffers should be page-locked for the copies to run at link speed.

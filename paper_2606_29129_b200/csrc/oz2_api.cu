@@ -150,12 +150,17 @@ HostConsts &host_consts()
 // per-device state
 // ---------------------------------------------------------------------------------------------
 constexpr int kMaxDevices = 64;
+constexpr int kMaxPanels = 16;
 struct DeviceState {
     bool tables_ready = false;
     bool checked = false;
     bool is_sm100 = false;
     void *ws = nullptr;
     size_t ws_bytes = 0;
+    // ozaki2_dgemm_host: copy streams and ordering events (created on first use)
+    bool host_ready = false;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev0 = nullptr, evA = nullptr, evEnd = nullptr, evB[kMaxPanels] = {}, evC[kMaxPanels] = {};
 };
 DeviceState g_dev[kMaxDevices];
 std::mutex g_mu;
@@ -311,7 +316,8 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
         if ((rc = oz2_launch_gemm_tc(1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
         if ((rc = oz2_launch_scale_accu_finish(N, m, n, EA, EB, rowmax, colmax, e, f, st))) return rc;
     } else {
-        if ((rc = oz2_launch_scale_fastprop(mode, N, m, n, k, A, lda, B, ldb, amax, ssq, e, f, st))) return rc;
+        if ((rc = oz2_launch_scale_rows(mode, N, m, k, A, lda, amax, ssq, e, st))) return rc;
+        if ((rc = oz2_launch_scale_cols(mode, N, n, k, B, ldb, f, st))) return rc;
     }
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[1], st));
@@ -351,6 +357,85 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
             for (int t = 0; t < 5; t++) cudaEventDestroy(ev[t]);
         }
     }
+    return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// ozaki2_dgemm_host, modes 1 and 2: column panels of B / C so that the H2D copy of panel p+1 and the D2H copy of
+// panel p-1 overlap the kernels of panel p.  (e_i depends on row i of A only and f_j on column j of B only, so a
+// panel is the same computation as the monolithic call; accurate mode needs all of B before any e_i and takes the
+// plain route.)  Kernels run on the caller's stream in order, so all panels share one workspace.
+// ---------------------------------------------------------------------------------------------
+static int ensure_host_streams(DeviceState *d)
+{
+    if (d->host_ready) return 0;
+    OZ2_CUDA_TRY(cudaStreamCreateWithFlags(&d->s_h2d, cudaStreamNonBlocking));
+    OZ2_CUDA_TRY(cudaStreamCreateWithFlags(&d->s_d2h, cudaStreamNonBlocking));
+    OZ2_CUDA_TRY(cudaEventCreateWithFlags(&d->ev0, cudaEventDisableTiming));
+    OZ2_CUDA_TRY(cudaEventCreateWithFlags(&d->evA, cudaEventDisableTiming));
+    OZ2_CUDA_TRY(cudaEventCreateWithFlags(&d->evEnd, cudaEventDisableTiming));
+    for (int p = 0; p < kMaxPanels; p++) {
+        OZ2_CUDA_TRY(cudaEventCreateWithFlags(&d->evB[p], cudaEventDisableTiming));
+        OZ2_CUDA_TRY(cudaEventCreateWithFlags(&d->evC[p], cudaEventDisableTiming));
+    }
+    d->host_ready = true;
+    return 0;
+}
+
+static int host_pipelined(int64_t m, int64_t n, int64_t k, double alpha, const double *A_host, int64_t lda,
+                          const double *B_host, int64_t ldb, double beta, double *C_host, int64_t ldc, int N, int mode,
+                          double *dA, double *dB, double *dC, cudaStream_t st, DeviceState *dev)
+{
+    int rc;
+    if ((rc = ensure_host_streams(dev))) return rc;
+    const Layout L = make_layout(m, n, k, N, mode);
+    if (!dev->ws || dev->ws_bytes < L.total) return OZAKI2_ERR_WORKSPACE;
+    uint8_t *ws = static_cast<uint8_t *>(dev->ws);
+    int32_t *e = reinterpret_cast<int32_t *>(ws + L.off_e), *f = reinterpret_cast<int32_t *>(ws + L.off_f);
+    unsigned long long *amax = reinterpret_cast<unsigned long long *>(ws + L.off_amax);
+    unsigned long long *ssq = reinterpret_cast<unsigned long long *>(ws + L.off_ssq);
+    int8_t *RA = reinterpret_cast<int8_t *>(ws + L.off_RA), *RB = reinterpret_cast<int8_t *>(ws + L.off_RB);
+    uint8_t *U = ws + L.off_U;
+    const int wide = needs_wide_words(N, mode) ? 1 : 0;
+    // panels: multiples of 256 columns (the GEMM tile), at most kMaxPanels / 2
+    int64_t np = oz2_round_up((n + kMaxPanels / 2 - 1) / (kMaxPanels / 2), 256);
+    const int panels = (int)((n + np - 1) / np);
+    cudaStream_t sh = dev->s_h2d, sd = dev->s_d2h;
+    OZ2_CUDA_TRY(cudaEventRecord(dev->ev0, st));
+    OZ2_CUDA_TRY(cudaStreamWaitEvent(sh, dev->ev0, 0));
+    OZ2_CUDA_TRY(cudaStreamWaitEvent(sd, dev->ev0, 0));
+    // ---- copies in: A, then the panels of B (and of C if it is read)
+    OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, 8 * (size_t)m, A_host, 8 * (size_t)lda, 8 * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, sh));
+    OZ2_CUDA_TRY(cudaEventRecord(dev->evA, sh));
+    for (int p = 0; p < panels; p++) {
+        const int64_t j0 = p * np, nc = (j0 + np < n ? np : n - j0);
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB + j0 * k, 8 * (size_t)k, B_host + j0 * ldb, 8 * (size_t)ldb, 8 * (size_t)k, (size_t)nc,
+                                       cudaMemcpyHostToDevice, sh));
+        if (beta != 0.0)
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC + j0 * m, 8 * (size_t)m, C_host + j0 * ldc, 8 * (size_t)ldc, 8 * (size_t)m, (size_t)nc,
+                                           cudaMemcpyHostToDevice, sh));
+        OZ2_CUDA_TRY(cudaEventRecord(dev->evB[p], sh));
+    }
+    // ---- rows of A: S1, S2
+    OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evA, 0));
+    if ((rc = oz2_launch_scale_rows(mode, N, m, k, dA, m, amax, ssq, e, st))) return rc;
+    if ((rc = oz2_launch_convert(0, N, wide, m, k, dA, m, e, RA, L.kp, st))) return rc;
+    // ---- panels: S1, S2 of the columns, S3, S4 + S5, copy out
+    for (int p = 0; p < panels; p++) {
+        const int64_t j0 = p * np, nc = (j0 + np < n ? np : n - j0);
+        OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evB[p], 0));
+        if ((rc = oz2_launch_scale_cols(mode, N, nc, k, dB + j0 * k, k, f, st))) return rc;
+        if ((rc = oz2_launch_convert(1, N, wide, nc, k, dB + j0 * k, k, f, RB, L.kp, st))) return rc;
+        if ((rc = oz2_launch_gemm_tc(N, 0, m, nc, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
+        if ((rc = oz2_launch_crt(N, m, nc, U, L.mp, e, f, alpha, beta, dC + j0 * m, m, nullptr, st))) return rc;
+        OZ2_CUDA_TRY(cudaEventRecord(dev->evC[p], st));
+        OZ2_CUDA_TRY(cudaStreamWaitEvent(sd, dev->evC[p], 0));
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host + j0 * ldc, 8 * (size_t)ldc, dC + j0 * m, 8 * (size_t)m, 8 * (size_t)m, (size_t)nc,
+                                       cudaMemcpyDeviceToHost, sd));
+    }
+    OZ2_CUDA_TRY(cudaEventRecord(dev->evEnd, sd));
+    OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evEnd, 0));
+    OZ2_CUDA_TRY(cudaStreamSynchronize(st));
     return 0;
 }
 
@@ -411,6 +496,12 @@ int ozaki2_dgemm_host(int64_t m, int64_t n, int64_t k, double alpha, const doubl
     double *dA = reinterpret_cast<double *>(base);
     double *dB = reinterpret_cast<double *>(base + align_up(8 * (size_t)m * k));
     double *dC = reinterpret_cast<double *>(base + align_up(8 * (size_t)m * k) + align_up(8 * (size_t)k * n));
+    if (k > 0 && alpha != 0.0 && scaling_mode != OZAKI2_MODE_ACCURATE && n >= 512) {
+        DeviceState *dev = nullptr;
+        if ((rc = ensure_device(&dev))) return rc;
+        return host_pipelined(m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ldc, num_moduli, scaling_mode, dA, dB, dC,
+                              st, dev);
+    }
     if (k > 0) {
         OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, 8 * (size_t)m, A_host, 8 * (size_t)lda, 8 * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, st));
         OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB, 8 * (size_t)k, B_host, 8 * (size_t)ldb, 8 * (size_t)k, (size_t)n, cudaMemcpyHostToDevice, st));

@@ -51,9 +51,9 @@ int oz2_gemm_upload_tables(const Oz2HostTables &t);
 int oz2_crt_upload_tables(const Oz2HostTables &t);
 
 // S1: exponents for modes 1 and 2, and the mode-0 pieces.  stat buffers: amax[rows] (u64), ssq[rows] (u64)
-int oz2_launch_scale_fastprop(int mode, int N, int64_t m, int64_t n, int64_t k, const double *A, int64_t lda,
-                              const double *B, int64_t ldb, unsigned long long *amaxA, unsigned long long *ssqA,
-                              int32_t *e, int32_t *f, cudaStream_t st);
+int oz2_launch_scale_rows(int mode, int N, int64_t m, int64_t k, const double *A, int64_t lda,
+                          unsigned long long *amaxA, unsigned long long *ssqA, int32_t *e, cudaStream_t st);
+int oz2_launch_scale_cols(int mode, int N, int64_t n, int64_t k, const double *B, int64_t ldb, int32_t *f, cudaStream_t st);
 int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B,
                                   int64_t ldb, unsigned long long *amaxA, int32_t *EA, int32_t *EB, int8_t *Abar,
                                   int8_t *Bbar, int64_t kp, int32_t *rowmax, int32_t *colmax, cudaStream_t st);

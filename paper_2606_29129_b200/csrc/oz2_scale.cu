@@ -274,10 +274,10 @@ int oz2_scale_upload_tables(const Oz2HostTables &t)
     return 0;
 }
 
-int oz2_launch_scale_fastprop(int mode, int N, int64_t m, int64_t n, int64_t k, const double *A, int64_t lda,
-                              const double *B, int64_t ldb, unsigned long long *amaxA, unsigned long long *ssqA,
-                              int32_t *e, int32_t *f, cudaStream_t st)
+int oz2_launch_scale_rows(int mode, int N, int64_t m, int64_t k, const double *A, int64_t lda,
+                          unsigned long long *amaxA, unsigned long long *ssqA, int32_t *e, cudaStream_t st)
 {
+    if (m <= 0) return 0;
     OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
     OZ2_CUDA_TRY(cudaMemsetAsync(ssqA, 0, sizeof(unsigned long long) * (size_t)m, st));
     int64_t kchunk;
@@ -286,8 +286,16 @@ int oz2_launch_scale_fastprop(int mode, int N, int64_t m, int64_t n, int64_t k, 
     k1_rows<0><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
     k1_rows<1><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
     k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e);
+    oz2_count_launches(3);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
+int oz2_launch_scale_cols(int mode, int N, int64_t n, int64_t k, const double *B, int64_t ldb, int32_t *f, cudaStream_t st)
+{
+    if (n <= 0) return 0;
     k1_cols<false><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, B, ldb, f, nullptr);
-    oz2_count_launches(4);
+    oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }

@@ -161,6 +161,29 @@ def test_host_buffer_entry_point(B):
     assert np.array_equal(Ch, O.dgemm(A, Bm, N, 2))
 
 
+@pytest.mark.parametrize("mode,alpha,beta", [(2, 1.0, 0.0), (1, -0.5, 2.0), (0, 1.0, 0.0)])
+def test_host_buffer_entry_point_column_panels(B, mode, alpha, beta):
+    # n >= 512: modes 1, 2 run as column panels with the copies overlapped (5 panels here, the last one ragged);
+    # padded leading dimensions on all three host matrices
+    import torch
+    m, n, k, N = 300, 1100, 200, 14
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 6)
+    lda, ldb, ldc = m + 4, k + 2, m + 6
+    Ah = np.zeros((lda, k), order="F"); Ah[:m] = A
+    Bh = np.zeros((ldb, n), order="F"); Bh[:k] = Bm
+    rng = np.random.Generator(np.random.PCG64(4))
+    Cin = np.asfortranarray(rng.standard_normal((ldc, n)))
+    Ch = Cin.copy(order="F")
+    B.ensure_workspace(m, n, k, N, mode)
+    nbytes = B.ozaki2_host_scratch_bytes(m, n, k)
+    scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    rc = B.ozaki2_dgemm_host(m, n, k, alpha, Ah, lda, Bh, ldb, beta, Ch, ldc, N, mode, scratch, nbytes)
+    assert rc == 0
+    want = O.dgemm(A, Bm, N, mode, alpha=alpha, beta=beta, C_in=Cin[:m].copy())
+    assert np.array_equal(Ch[:m], want)
+    assert np.array_equal(Ch[m:], Cin[m:])
+
+
 # --------------------------------------------------------------------------------------------- primitives
 def test_log2f_exhaustive_equals_oracle(B):
     import torch
