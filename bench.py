@@ -111,6 +111,17 @@ class ClockSampler:
                     reasons=sorted(reasons))
 
 
+def profiled_traffic(m, N, mode):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), only for
+    the workload that capture was taken on; None otherwise."""
+    path = os.path.join(ROOT, "profiles", "r01b_dram_traffic.json")
+    if not (os.path.exists(path) and m == 8192 and N == 16 and mode == 2):
+        return None
+    with open(path) as fh:
+        d = json.load(fh)
+    return d["bytes_per_launch"].get("k3_residue_gemm<0>")
+
+
 def cpu_slab_shape(m, n, k):
     """Bounded sample of the workload for the oracle: 512 rows of A against 4096 columns of B at the full k
     (about 15 s on the GPU box's 16 host threads at k = 8192, N = 16)."""
@@ -253,7 +264,9 @@ def main():
                     achieved=achieved, peak=int8_peak, unit="TFLOP/s", frac=achieved / int8_peak,
                     peak_source=f"2 x bf16_tflops_sustained ({peaks['source']}); INT8 has no measured entry",
                     frac_of_burst=achieved / (INT8_OVER_BF16 * peaks["bf16"]),
-                    frac_of_nominal_4500=achieved / NOMINAL_INT8_TOPS, ms_per_launch=s3_ms, traffic=None)
+                    frac_of_nominal_4500=achieved / NOMINAL_INT8_TOPS, ms_per_launch=s3_ms,
+                    traffic=profiled_traffic(m, N, mode), traffic_unit="bytes per launch (ncu dram read + write, profiles/r01b)",
+                    algorithmic_bytes=N * X + N * Y)
     stage_bytes = [8 * X if mode != 0 else 8 * X + 2 * X, (8 + N) * X, N * X + N * Y, (N + 8) * Y]
     stages = {}
     for nm, ms_, by in zip(("S1_scaling", "S2_conversion", "S3_residue_gemm", "S4S5_crt_unscale"), stage_ms, stage_bytes):
