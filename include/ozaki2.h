@@ -134,8 +134,9 @@ int ozaki2_debug_log2f(const float *x, float *y, int64_t count, void *stream);
 int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64_t count, void *stream);
 
 /* One INT8 product resA_l resB_l^T mod p_l for canonical planes (same layouts as above) on the
- * tensor-core kernel (use_tensor_cores != 0) or on a plain CUDA-core check kernel (== 0) that
- * ozaki2_dgemm never uses.  Both need no workspace. */
+ * tensor-core kernel (use_tensor_cores = 1: one CTA per 128 x 256 tile, what ozaki2_dgemm runs;
+ * 2: the cta_group::2 variant, CTA pairs on 256 x 256 tiles, a measured alternative) or on a
+ * plain CUDA-core check kernel (0) that ozaki2_dgemm never uses.  None needs a workspace. */
 int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA,
                               const int8_t *resB, uint8_t *U, int use_tensor_cores, void *stream);
 

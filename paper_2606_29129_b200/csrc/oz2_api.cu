@@ -586,7 +586,12 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
     if (k <= 0 || k % 128 != 0 || k > OZAKI2_MAX_K) return -4;      // canonical planes are used in place: pitch = k
     if (m % 16 != 0) return -2;                                     // U pitch = m
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (use_tensor_cores) return oz2_launch_gemm_tc(num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
+    if (use_tensor_cores) {
+        oz2_gemm_set_pair_mode(use_tensor_cores == 2 ? 1 : 0);      // 1: one CTA per tile (the ozaki2_dgemm path), 2: CTA pairs
+        const int rc2 = oz2_launch_gemm_tc(num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
+        oz2_gemm_set_pair_mode(0);
+        return rc2;
+    }
     return oz2_launch_gemm_check(num_moduli, m, n, k, resA, resB, k, U, m, st);
 }
 

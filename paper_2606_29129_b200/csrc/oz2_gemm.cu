@@ -230,6 +230,212 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     }
 }
 
+// =============================================================================================
+// CTA-pair variant (cta_group::2): a cluster of two CTAs on one TPC computes a 256 x 256 tile.  Each CTA loads its
+// own 128 rows of A and HALF of the B tile (128 of the 256 rows); the MMA (M = 256, issued by the leader CTA only)
+// reads both halves of B from the two shared memories, so every SM fills 32 KB instead of 48 KB per K step of its
+// 128 x 256 accumulator -- a third less L2 -> SM and shared-memory traffic.
+// Barriers: the leader's full[] collects the TMA bytes of BOTH CTAs; empty[] / tfull[] are signalled in both CTAs by
+// multicast commits; the leader's tempty[] counts the epilogue warps of both CTAs (the peer arrives remotely).
+// =============================================================================================
+constexpr int P2_TILE_M = 256;                          // per cluster
+constexpr int P2_STAGES = 6;
+constexpr int P2_A_BYTES = 128 * TILE_K, P2_B_BYTES = 128 * TILE_K;
+constexpr int P2_STAGE_BYTES = P2_A_BYTES + P2_B_BYTES; // 32 KB per CTA and stage
+constexpr int P2_SMEM = P2_STAGES * P2_STAGE_BYTES + 1024 + 256;
+constexpr uint32_t P2_IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TILE_N >> 3) << 17) |
+                              ((uint32_t)(P2_TILE_M >> 4) << 24);
+constexpr uint32_t PEER_MASK = 0xFEFFFFFFu;             // shared::cluster address of the same offset in the even CTA
+
+__device__ __forceinline__ void tma_load_3d_pair(const CUtensorMap *map, uint32_t leader_bar, uint32_t dst, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(dst), "l"(map), "r"(leader_bar), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void tc_mma_i8_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "setp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+__device__ __forceinline__ TileCoord decode_tile_pair(int64_t t, int tiles_m, int tiles_n)
+{
+    constexpr int G = GROUP_M / 2;                      // groups of 16 pair tiles = 4096 rows, as in the 1-CTA order
+    const int64_t per_plane = (int64_t)tiles_m * tiles_n;
+    TileCoord c;
+    c.plane = (int)(t / per_plane);
+    int rem = (int)(t - (int64_t)c.plane * per_plane);
+    const int group_sz = G * tiles_n;
+    int g = rem / group_sz;
+    int in_g = rem - g * group_sz;
+    int gm = tiles_m - g * G;
+    if (gm > G) gm = G;
+    int nt = in_g / gm;
+    int mt = g * G + (in_g - nt * gm);
+    c.m0 = mt * P2_TILE_M;
+    c.n0 = nt * TILE_N;
+    return c;
+}
+
+template <bool MAXEPI>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, int nplanes,
+                     int mod_base, int m, int n, int num_kb, uint8_t *__restrict__ U, int64_t mp,
+                     int32_t *__restrict__ rowmax, int32_t *__restrict__ colmax)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t full = smem0 + P2_STAGES * P2_STAGE_BYTES, empty = full + 8 * P2_STAGES, tfull = empty + 8 * P2_STAGES,
+                   tempty = tfull + 16, tmem_slot = tempty + 16;
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tiles_m = (m + P2_TILE_M - 1) / P2_TILE_M, tiles_n = (n + TILE_N - 1) / TILE_N;
+    const int64_t total = (int64_t)nplanes * tiles_m * tiles_n;
+    const int64_t cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < P2_STAGES; s++) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(full + 8 * s));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(empty + 8 * s));
+        }
+        for (int b = 0; b < 2; b++) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(tfull + 8 * b));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 8;" ::"r"(tempty + 8 * b));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapB) : "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(tmem_slot) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    if (warp == 0) {
+        // ===================== TMA producer (both CTAs): own 128 rows of A, own half of the B tile =====================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int64_t t = cluster_id; t < total; t += num_clusters) {
+                const TileCoord c = decode_tile_pair(t, tiles_m, tiles_n);
+                for (int kb = 0; kb < num_kb; kb++) {
+                    mbar_wait_a(empty + 8 * stage, phase ^ 1u);
+                    const uint32_t sa = smem0 + stage * P2_STAGE_BYTES, sb = sa + P2_A_BYTES;
+                    const uint32_t lbar = (full + 8 * stage) & PEER_MASK;
+                    if (rank == 0) mbar_expect_tx_a(full + 8 * stage, 2 * P2_STAGE_BYTES);
+                    tma_load_3d_pair(&mapA, lbar, sa, kb * TILE_K, c.m0 + (int)rank * 128, c.plane);
+                    tma_load_3d_pair(&mapB, lbar, sb, kb * TILE_K, c.n0 + (int)rank * 128, c.plane);
+                    if (++stage == P2_STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer: leader CTA only =====================
+        if (lane == 0 && rank == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int as = 0;
+            uint32_t aphase = 0;
+            for (int64_t t = cluster_id; t < total; t += num_clusters) {
+                mbar_wait_a(tempty + 8 * as, aphase ^ 1u);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(as * TILE_N);
+                for (int kb = 0; kb < num_kb; kb++) {
+                    mbar_wait_a(full + 8 * stage, phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem0 + stage * P2_STAGE_BYTES, sb = sa + P2_A_BYTES;
+                    const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
+#pragma unroll
+                    for (int ks = 0; ks < TILE_K / UMMA_K; ks++)
+                        tc_mma_i8_pair(d_tmem, adesc + (uint64_t)(ks * UMMA_K / 16), bdesc + (uint64_t)(ks * UMMA_K / 16), P2_IDESC,
+                                       (uint32_t)((kb | ks) != 0));
+                    tc_commit_pair(empty + 8 * stage);         // frees this stage in BOTH CTAs
+                    if (++stage == P2_STAGES) { stage = 0; phase ^= 1u; }
+                }
+                tc_commit_pair(tfull + 8 * as);                // accumulator complete, both CTAs
+                if (++as == 2) { as = 0; aphase ^= 1u; }
+            }
+        }
+    } else {
+        // ===================== epilogue: warps 2..5 of both CTAs, rows m0 + 128 rank + 32 q + lane =====================
+        const int q = warp & 3;
+        int as = 0;
+        uint32_t aphase = 0;
+        const uint32_t leader_tempty = tempty & PEER_MASK;
+        for (int64_t t = cluster_id; t < total; t += num_clusters) {
+            const TileCoord c = decode_tile_pair(t, tiles_m, tiles_n);
+            mbar_wait_a(tfull + 8 * as, aphase);
+            tc_fence_after();
+            const int i = c.m0 + (int)rank * 128 + q * 32 + lane;
+            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TILE_N);
+            if (!MAXEPI) {
+                const int l = mod_base + c.plane;
+                const Oz2ModTab tb = c_mod[l];
+                uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
+#pragma unroll 1
+                for (int cc = 0; cc < TILE_N / 32; cc++) {
+                    uint32_t v[32];
+                    tc_ld32(taddr + (uint32_t)(cc * 32), v);
+                    if (i < m) {
+#pragma unroll
+                        for (int u = 0; u < 32; u++) {
+                            const int j = c.n0 + cc * 32 + u;
+                            uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
+                            if (j < n) out[(int64_t)(cc * 32 + u) * mp] = (uint8_t)r;
+                        }
+                    }
+                }
+            } else {
+                int rmax = 0;
+#pragma unroll 1
+                for (int cc = 0; cc < TILE_N / 32; cc++) {
+                    uint32_t v[32];
+                    tc_ld32(taddr + (uint32_t)(cc * 32), v);
+#pragma unroll
+                    for (int u = 0; u < 32; u++) {
+                        const int j = c.n0 + cc * 32 + u;
+                        int val = (i < m && j < n) ? (int)v[u] : 0;
+                        rmax = max(rmax, val);
+                        int cm = __reduce_max_sync(0xffffffffu, val);
+                        if (lane == 0 && j < n && cm > 0) atomicMax(colmax + j, cm);
+                    }
+                }
+                if (i < m && rmax > 0) atomicMax(rowmax + i, rmax);
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(leader_tempty + 8 * as);
+            if (++as == 2) { as = 0; aphase ^= 1u; }
+        }
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
 // plain CUDA-core check kernel (never on the ozaki2_dgemm path): one thread per (i, j), dp4a over k
 // ---------------------------------------------------------------------------------------------
@@ -290,8 +496,17 @@ int oz2_gemm_upload_tables(const Oz2HostTables &t)
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_mod, t.mod, sizeof(t.mod)));
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
     return 0;
 }
+
+// 0: one CTA per 128 x 256 tile (default); 1: CTA pairs on 256 x 256 tiles.  Measured at 8192^3, N = 16 on random
+// residues, 20 calls back to back: 5.98 / 6.06 ms single vs 6.29 / 6.15 ms pairs -- the kernel is bound by the
+// power cap and the operand toggling, not by shared-memory or L2 traffic, so the pair variant stays a tested
+// alternative (ozaki2_debug_residue_gemm, use_tensor_cores = 2) and is not on the ozaki2_dgemm path.
+static int g_gemm_pair = 0;
+void oz2_gemm_set_pair_mode(int on) { g_gemm_pair = on; }
 
 int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA, const int8_t *RB,
                        int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
@@ -299,6 +514,26 @@ int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t 
     (void)k;
     if (m <= 0 || n <= 0 || nplanes <= 0) return 0;
     CUtensorMap mapA, mapB;
+    const int num_kb = (int)(kp / TILE_K);
+    if (g_gemm_pair && m > TILE_M) {
+        int rc = make_plane_map(&mapA, RA, kp, m, nplanes, 128);
+        if (rc) return rc;
+        rc = make_plane_map(&mapB, RB, kp, n, nplanes, 128);
+        if (rc) return rc;
+        const int64_t tiles = (int64_t)nplanes * ((m + P2_TILE_M - 1) / P2_TILE_M) * ((n + TILE_N - 1) / TILE_N);
+        int64_t clusters = num_sms() / 2;
+        if (tiles < clusters) clusters = tiles;
+        const unsigned grid = (unsigned)(2 * clusters);
+        if (rowmax)
+            k3_residue_gemm_pair<true><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
+                                                                         nullptr, mp, rowmax, colmax);
+        else
+            k3_residue_gemm_pair<false><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
+                                                                          U, mp, nullptr, nullptr);
+        oz2_count_launches(1);
+        OZ2_CUDA_TRY(cudaGetLastError());
+        return 0;
+    }
     int rc = make_plane_map(&mapA, RA, kp, m, nplanes, TILE_M);
     if (rc) return rc;
     rc = make_plane_map(&mapB, RB, kp, n, nplanes, TILE_N);
@@ -306,7 +541,6 @@ int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t 
     const int64_t tiles = (int64_t)nplanes * ((m + TILE_M - 1) / TILE_M) * ((n + TILE_N - 1) / TILE_N);
     int grid = num_sms();
     if (tiles < grid) grid = (int)tiles;
-    const int num_kb = (int)(kp / TILE_K);
     if (rowmax)
         k3_residue_gemm<true><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
                                                                    nullptr, mp, rowmax, colmax);

@@ -211,7 +211,8 @@ def test_epilogue_mod_p_all_moduli(B):
         assert np.array_equal(od.cpu().numpy(), (v.astype(np.int64) % p[l]).astype(np.uint8)), l
 
 
-@pytest.mark.parametrize("m,n,k,N", [(128, 256, 128, 1), (256, 512, 1024, 3), (384, 272, 2048, 20), (16, 8, 128, 2)])
+@pytest.mark.parametrize("m,n,k,N", [(128, 256, 128, 1), (256, 512, 1024, 3), (384, 272, 2048, 20), (16, 8, 128, 2),
+                                     (1040, 784, 512, 5)])
 def test_residue_gemm_tensor_core_vs_oracle_and_check_kernel(B, m, n, k, N):
     import torch
     rng = np.random.Generator(np.random.PCG64(k + N))
@@ -221,7 +222,7 @@ def test_residue_gemm_tensor_core_vs_oracle_and_check_kernel(B, m, n, k, N):
     want, _ = O.products(max(N, 2), RA if N > 1 else np.concatenate([RA, RA]), RB if N > 1 else np.concatenate([RB, RB]))
     want = want[:N]
     RAd, RBd = torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda()
-    for tc in (1, 0):
+    for tc in (2, 1, 0):            # CTA pairs / one CTA per tile / CUDA-core check kernel
         Ud = torch.zeros((N, n, m), dtype=torch.uint8, device="cuda")
         assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, tc) == 0
         torch.cuda.synchronize()
@@ -232,7 +233,7 @@ def test_int32_accumulator_wraps_at_k_2pow17(B):
     # reading R6: p = 256 residues of -128 over k = 2^17 give 2^31, which must WRAP (256 | 2^32), not saturate;
     # the odd moduli stay below 2^31.
     import torch
-    m, n, k, N = 128, 256, 1 << 17, 2
+    m, n, k, N = 256, 256, 1 << 17, 2
     RA = np.zeros((N, m, k), np.int8)
     RB = np.zeros((N, n, k), np.int8)
     RA[0] = -128; RB[0] = -128
@@ -242,8 +243,10 @@ def test_int32_accumulator_wraps_at_k_2pow17(B):
     assert maxR == 2 ** 31
     RAd, RBd = torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda()
     Ud = torch.zeros((N, n, m), dtype=torch.uint8, device="cuda")
-    assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, 1) == 0
-    torch.cuda.synchronize()
-    got = Ud.cpu().numpy()
-    assert np.array_equal(got[:, :8, :8], want)
-    assert np.all(got[1] == (127 * 127 * k) % 255)
+    for tc in (1, 2):
+        Ud.zero_()
+        assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, tc) == 0
+        torch.cuda.synchronize()
+        got = Ud.cpu().numpy()
+        assert np.array_equal(got[:, :8, :8], want)
+        assert np.all(got[1] == (127 * 127 * k) % 255)
