@@ -193,7 +193,7 @@ __device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T,
 }
 
 template <int NW, bool WANT_CPP>
-__global__ void __launch_bounds__(K5_THREADS, 3)
+__global__ void __launch_bounds__(K5_THREADS, NW <= 4 ? 3 : 2)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n, const int32_t *__restrict__ e,
           const int32_t *__restrict__ f, double alpha, double beta, double *__restrict__ C, int64_t ldc,
           uint64_t *__restrict__ Cpp)
