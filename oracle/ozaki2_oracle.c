@@ -787,6 +787,100 @@ done:
 }
 
 /* ------------------------------------------------------------------------------------ */
+/* SGEMM variant (Fig. 6): FP32 in, FP32 out.  Every float is a double, */
+/* so Steps 1-3 are the FP64 path on the promoted inputs (the scaling formulas do not       */
+/* depend on the input precision); only Step 4 changes:               */
+/*   c = RN_32(C'' 2^-(e_i+f_j))  -- one rounding of the exact integer to FP32 --           */
+/*   out = alpha c (+ beta C_in) in FP32  (readings R8, R9 with FP32 in place of FP64).     */
+/* ------------------------------------------------------------------------------------ */
+static float w_to_float_scaled(wint v, long sh)
+{
+    if (w_iszero(v)) return 0.0f;
+    int neg = w_isneg(v);
+    wint a = w_abs(v);
+    int t = w_bitlen(a) - 1;               /* a in [2^t, 2^(t+1)) */
+    long E = (long)t + sh;                 /* value in [2^E, 2^(E+1)) */
+    long qe = E - 23;                      /* exponent of the last kept bit (24-bit significand) */
+    if (qe < -149) qe = -149;              /* FP32 subnormal quantum */
+    long r = qe - sh;                      /* bits of a dropped below the quantum */
+    uint64_t q;
+    if (r <= 0) {
+        q = a.w[0] << (-r);                /* nothing dropped: a has at most 24 bits here */
+    } else if (r > 256) {
+        q = 0;
+    } else {
+        q = 0;
+        for (int b = 0; b < 25; b++) q |= (uint64_t)w_bit(a, (int)r + b) << b;
+        int half = w_bit(a, (int)r - 1);
+        int sticky = 0;
+        for (int b = 0; b < (int)r - 1 && !sticky; b++) sticky = w_bit(a, b);
+        if (half && (sticky || (q & 1))) q += 1;
+    }
+    float d = ldexpf((float)q, (int)qe);   /* q <= 2^24: exact; overflows to inf */
+    return neg ? -d : d;
+}
+
+float oz2o_words_to_float(const uint64_t *words, long sh)
+{
+    wint v;
+    memcpy(v.w, words, 32);
+    return w_to_float_scaled(v, sh);
+}
+
+int oz2o_unscale_f32(long m, long n, const uint64_t *Cpp, const int32_t *e, const int32_t *f,
+                     float alpha, float beta, float *C, long ldc)
+{
+#pragma omp parallel for schedule(static)
+    for (long j = 0; j < n; j++)
+        for (long i = 0; i < m; i++) {
+            wint v;
+            memcpy(v.w, Cpp + ((size_t)j * m + i) * 4, 32);
+            float cij = w_to_float_scaled(v, -((long)e[i] + (long)f[j]));
+            volatile float t = alpha * cij;
+            float *dst = &C[(size_t)j * ldc + i];
+            *dst = (beta == 0.0f) ? t : fmaf(beta, *dst, t);
+        }
+    return 0;
+}
+
+int oz2o_sgemm(long m, long n, long k, float alpha, const float *A, long lda,
+               const float *B, long ldb, float beta, float *C, long ldc,
+               int N, int mode, int32_t *e_out, int32_t *f_out)
+{
+    if (m < 0 || n < 0 || k < 0) return -1;
+    if (m == 0 || n == 0) return 0;
+    int rc = 0;
+    size_t ka = (size_t)(k > 0 ? k : 1);
+    double *Ad = malloc(sizeof(double) * (size_t)m * ka), *Bd = malloc(sizeof(double) * ka * (size_t)n);
+    int32_t *e = malloc(sizeof(int32_t) * (size_t)m), *f = malloc(sizeof(int32_t) * (size_t)n);
+    int8_t *RA = malloc((size_t)N * m * ka), *RB = malloc((size_t)N * n * ka);
+    uint8_t *U = malloc((size_t)N * m * n);
+    uint64_t *Cpp = malloc((size_t)m * n * 32);
+    if (!Ad || !Bd || !e || !f || !RA || !RB || !U || !Cpp) { rc = -9; goto done; }
+    for (long h = 0; h < k; h++)
+        for (long i = 0; i < m; i++) Ad[(size_t)h * m + i] = (double)A[(size_t)h * lda + i];       /* exact */
+    for (long j = 0; j < n; j++)
+        for (long h = 0; h < k; h++) Bd[(size_t)j * k + h] = (double)B[(size_t)j * ldb + h];
+    long ldad = m > 1 ? m : 1, ldbd = k > 1 ? k : 1;
+    rc = oz2o_exponents(mode, N, m, n, k, Ad, ldad, Bd, ldbd, e, f, 0, 0, 0, 0, 0, 0);
+    if (rc) goto done;
+    rc = oz2o_residues(0, N, m, k, Ad, ldad, e, RA);
+    if (rc) goto done;
+    rc = oz2o_residues(1, N, n, k, Bd, ldbd, f, RB);
+    if (rc) goto done;
+    rc = oz2o_products(N, m, n, k, RA, RB, U, 0);
+    if (rc) goto done;
+    rc = oz2o_crt(N, m, n, U, Cpp);
+    if (rc) goto done;
+    rc = oz2o_unscale_f32(m, n, Cpp, e, f, alpha, beta, C, ldc);
+    if (e_out) memcpy(e_out, e, sizeof(int32_t) * (size_t)m);
+    if (f_out) memcpy(f_out, f, sizeof(int32_t) * (size_t)n);
+done:
+    free(Ad); free(Bd); free(e); free(f); free(RA); free(RB); free(U); free(Cpp);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------ */
 /* O10: reference AB in double-double: two-product by fma, two-sum accumulation.  */
 /* hi, lo: [n][m] column-major contiguous (ld = m).                                       */
 /* ------------------------------------------------------------------------------------ */

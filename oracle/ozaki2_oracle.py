@@ -37,6 +37,8 @@ def lib():
         L.oz2o_words_to_double.restype = C.c_double
         L.oz2o_words_to_double.argtypes = [C.c_void_p, C.c_long]
         L.oz2o_num_threads.restype = C.c_int
+        L.oz2o_words_to_float.restype = C.c_float
+        L.oz2o_words_to_float.argtypes = [C.c_void_p, C.c_long]
     return _LIB
 
 
@@ -231,6 +233,30 @@ def dgemm(A, B, N: int, mode: int, alpha: float = 1.0, beta: float = 0.0, C_in=N
                           C.c_int(N), C.c_int(mode), _p(e), _p(f))
     if rc:
         raise ValueError(f"oz2o_dgemm -> {rc}")
+    if return_exponents:
+        return out, e[:m], f[:n]
+    return out
+
+
+def words_to_float(words, sh: int) -> np.float32:
+    words = np.ascontiguousarray(words, np.uint64)
+    return np.float32(lib().oz2o_words_to_float(_p(words), C.c_long(sh)))
+
+
+def sgemm(A, B, N: int, mode: int, alpha: float = 1.0, beta: float = 0.0, C_in=None, return_exponents=False):
+    """SGEMM variant (Fig. 6): FP32 in / FP32 out, Steps 1-3 on the promoted inputs, one rounding to FP32."""
+    A = np.asfortranarray(np.asarray(A, dtype=np.float32))
+    B = np.asfortranarray(np.asarray(B, dtype=np.float32))
+    m, k = A.shape
+    _, n = B.shape
+    out = np.zeros((m, n), np.float32, order="F") if C_in is None else np.array(C_in, np.float32, order="F")
+    e = np.zeros(max(1, m), np.int32)
+    f = np.zeros(max(1, n), np.int32)
+    rc = lib().oz2o_sgemm(C.c_long(m), C.c_long(n), C.c_long(k), C.c_float(alpha), _p(A), C.c_long(max(1, m)),
+                          _p(B), C.c_long(max(1, k)), C.c_float(beta), _p(out), C.c_long(max(1, m)),
+                          C.c_int(N), C.c_int(mode), _p(e), _p(f))
+    if rc:
+        raise ValueError(f"oz2o_sgemm -> {rc}")
     if return_exponents:
         return out, e[:m], f[:n]
     return out
