@@ -60,7 +60,18 @@ int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A,
                  const double *B, int64_t ldb, double beta, double *C, int64_t ldc,
                  int num_moduli, int scaling_mode, void *stream);
 
-/* Bytes of device workspace ozaki2_dgemm needs for this problem (0 for an invalid one). */
+/*
+ * SGEMM variant (Fig. 6): A, B, C are FP32 (4-byte aligned device pointers, same
+ * column-major conventions).  Every FP32 input is an FP64 number, so S1-S4 are the steps above on
+ * the promoted inputs; S5 rounds the exact integer once to FP32, C = RN_32(C'' 2^-(e_i+f_j)), and
+ * alpha / beta are applied in FP32 (t = alpha C; out = beta == 0 ? t : fmaf(beta, C_in, t)).  Same
+ * workspace, quick returns and error codes as ozaki2_dgemm; the paper uses 3..12 moduli here.
+ */
+int ozaki2_sgemm(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
+                 const float *B, int64_t ldb, float beta, float *C, int64_t ldc,
+                 int num_moduli, int scaling_mode, void *stream);
+
+/* Bytes of device workspace ozaki2_dgemm / ozaki2_sgemm needs for this problem (0 for an invalid one). */
 size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 
 /*
@@ -115,6 +126,11 @@ typedef struct ozaki2_stage_outputs {
 int ozaki2_dgemm_stages(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
                         const double *B, int64_t ldb, double beta, double *C, int64_t ldc,
                         int num_moduli, int scaling_mode, void *stream, const ozaki2_stage_outputs *out);
+
+/* ozaki2_dgemm_stages for the SGEMM variant (same outputs; C'' is the same integer as in the FP64 path). */
+int ozaki2_sgemm_stages(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda, const float *B,
+                        int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode,
+                        void *stream, const ozaki2_stage_outputs *out);
 
 /*
  * Constants of Step 1 for `num_moduli` moduli, written to HOST arrays (any may be NULL):

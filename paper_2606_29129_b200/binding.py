@@ -47,6 +47,11 @@ def lib() -> C.CDLL:
         L.ozaki2_dgemm.restype = ci
         L.ozaki2_dgemm_stages.argtypes = gemm_args + [C.POINTER(ozaki2_stage_outputs)]
         L.ozaki2_dgemm_stages.restype = ci
+        sgemm_args = [i64, i64, i64, C.c_float, vp, i64, vp, i64, C.c_float, vp, i64, ci, ci, vp]
+        L.ozaki2_sgemm.argtypes = sgemm_args
+        L.ozaki2_sgemm.restype = ci
+        L.ozaki2_sgemm_stages.argtypes = sgemm_args + [C.POINTER(ozaki2_stage_outputs)]
+        L.ozaki2_sgemm_stages.restype = ci
         L.ozaki2_dgemm_host.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, ci, ci, vp, C.c_size_t, vp]
         L.ozaki2_dgemm_host.restype = ci
         L.ozaki2_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
@@ -129,6 +134,18 @@ def ozaki2_dgemm_stages(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_modul
                                          scaling_mode, _stream(stream), C.byref(out) if out is not None else None))
 
 
+def ozaki2_sgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None) -> int:
+    """SGEMM variant: A, B, Cm are FP32 device tensors or addresses."""
+    return int(lib().ozaki2_sgemm(m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc, num_moduli,
+                                  scaling_mode, _stream(stream)))
+
+
+def ozaki2_sgemm_stages(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None,
+                        out: ozaki2_stage_outputs | None = None) -> int:
+    return int(lib().ozaki2_sgemm_stages(m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc, num_moduli,
+                                         scaling_mode, _stream(stream), C.byref(out) if out is not None else None))
+
+
 def ozaki2_dgemm_host(m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ldc, num_moduli, scaling_mode,
                       device_scratch, scratch_bytes, stream=None) -> int:
     return int(lib().ozaki2_dgemm_host(m, n, k, alpha, _ptr(A_host), lda, _ptr(B_host), ldb, beta, _ptr(C_host), ldc,
@@ -190,10 +207,10 @@ def ensure_workspace(m, n, k, num_moduli, scaling_mode):
     return cur
 
 
-def colmajor_to_device(a: np.ndarray):
+def colmajor_to_device(a: np.ndarray, dtype=np.float64):
     """numpy (rows, cols) matrix -> device tensor of shape (cols, rows) whose memory is the column-major matrix."""
     import torch
-    return torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=np.float64).T)).cuda()
+    return torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=dtype).T)).cuda()
 
 
 def device_to_colmajor(t) -> np.ndarray:
@@ -235,8 +252,9 @@ def dgemm_stages(A_dev, B_dev, num_moduli, scaling_mode, alpha=1.0, beta=0.0, C_
     n, _ = B_dev.shape
     N = num_moduli
     dev = A_dev.device
+    f32 = A_dev.dtype == torch.float32
     if C_dev is None:
-        C_dev = torch.empty((n, m), dtype=torch.float64, device=dev)
+        C_dev = torch.empty((n, m), dtype=A_dev.dtype, device=dev)
     ensure_workspace(m, n, k, N, scaling_mode)
     bufs = {}
     shapes = dict(e=((m,), torch.int32), f=((n,), torch.int32), rowmax=((m,), torch.int32), colmax=((n,), torch.int32),
@@ -250,10 +268,10 @@ def dgemm_stages(A_dev, B_dev, num_moduli, scaling_mode, alpha=1.0, beta=0.0, C_
     ms = (C.c_float * 5)()
     if timing:
         out.stage_ms = C.cast(ms, C.POINTER(C.c_float))
-    rc = ozaki2_dgemm_stages(m, n, k, alpha, A_dev, max(1, m), B_dev, max(1, k), beta, C_dev, max(1, m), N,
-                             scaling_mode, stream, out)
+    call = ozaki2_sgemm_stages if f32 else ozaki2_dgemm_stages
+    rc = call(m, n, k, alpha, A_dev, max(1, m), B_dev, max(1, k), beta, C_dev, max(1, m), N, scaling_mode, stream, out)
     if rc:
-        raise Ozaki2Error(rc, "ozaki2_dgemm_stages")
+        raise Ozaki2Error(rc, "ozaki2_sgemm_stages" if f32 else "ozaki2_dgemm_stages")
     bufs["C"] = C_dev
     if timing:
         bufs["stage_ms"] = [float(x) for x in ms]

@@ -239,8 +239,8 @@ bool needs_wide_words(int N, int mode)
     return width > 64;
 }
 
-int check_args(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B, int64_t ldb,
-               const double *C, int64_t ldc, int N, int mode)
+int check_args(int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B, int64_t ldb,
+               const void *C, int64_t ldc, int N, int mode)
 {
     if (m < 0) return -1;
     if (n < 0) return -2;
@@ -257,13 +257,14 @@ int check_args(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, co
     return 0;
 }
 
-__global__ void k_scale_c(int64_t m, int64_t n, double beta, double *C, int64_t ldc)
+template <typename T>
+__global__ void k_scale_c(int64_t m, int64_t n, T beta, T *C, int64_t ldc)
 {
     int64_t i = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
     int64_t j = blockIdx.x;
     if (i < m) {
-        double *p = C + i + j * ldc;
-        *p = beta == 0.0 ? 0.0 : beta * *p;
+        T *p = C + i + j * ldc;
+        *p = beta == (T)0 ? (T)0 : beta * *p;
     }
 }
 
@@ -272,8 +273,9 @@ __global__ void k_scale_c(int64_t m, int64_t n, double beta, double *C, int64_t 
 // =============================================================================================
 // the path
 // =============================================================================================
-static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
-                    int64_t ldb, double beta, double *C, int64_t ldc, int N, int mode, cudaStream_t st,
+// f32 = 0: ozaki2_dgemm (A, B, C FP64); f32 = 1: ozaki2_sgemm (A, B, C FP32; alpha, beta hold floats)
+static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda, const void *B,
+                    int64_t ldb, double beta, void *C, int64_t ldc, int N, int mode, cudaStream_t st,
                     const ozaki2_stage_outputs *out)
 {
     int rc = check_args(m, n, k, A, lda, B, ldb, C, ldc, N, mode);
@@ -284,7 +286,9 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
     if (k == 0 || alpha == 0.0) {
         // C := beta C (zeros if beta == 0, BLAS rule)
         if (!(beta == 1.0)) {
-            k_scale_c<<<dim3((unsigned)n, (unsigned)((m + 255) / 256)), 256, 0, st>>>(m, n, beta, C, ldc);
+            const dim3 grid((unsigned)n, (unsigned)((m + 255) / 256));
+            if (f32) k_scale_c<float><<<grid, 256, 0, st>>>(m, n, (float)beta, static_cast<float *>(C), ldc);
+            else k_scale_c<double><<<grid, 256, 0, st>>>(m, n, beta, static_cast<double *>(C), ldc);
             oz2_count_launches(1);
             OZ2_CUDA_TRY(cudaGetLastError());
         }
@@ -312,19 +316,19 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
     // ---- S1 scaling
     if (mode == OZAKI2_MODE_ACCURATE) {
         int8_t *Abar = reinterpret_cast<int8_t *>(ws + L.off_Abar), *Bbar = reinterpret_cast<int8_t *>(ws + L.off_Bbar);
-        if ((rc = oz2_launch_scale_accu_prepare(m, n, k, A, lda, B, ldb, amax, EA, EB, Abar, Bbar, L.kp, rowmax, colmax, st))) return rc;
+        if ((rc = oz2_launch_scale_accu_prepare(f32, m, n, k, A, lda, B, ldb, amax, EA, EB, Abar, Bbar, L.kp, rowmax, colmax, st))) return rc;
         if ((rc = oz2_launch_gemm_tc(1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
         if ((rc = oz2_launch_scale_accu_finish(N, m, n, EA, EB, rowmax, colmax, e, f, st))) return rc;
     } else {
-        if ((rc = oz2_launch_scale_rows(mode, N, m, k, A, lda, amax, ssq, e, st))) return rc;
-        if ((rc = oz2_launch_scale_cols(mode, N, n, k, B, ldb, f, st))) return rc;
+        if ((rc = oz2_launch_scale_rows(mode, N, f32, m, k, A, lda, amax, ssq, e, st))) return rc;
+        if ((rc = oz2_launch_scale_cols(mode, N, f32, n, k, B, ldb, f, st))) return rc;
     }
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[1], st));
     // ---- S2 conversion
     const int wide = needs_wide_words(N, mode) ? 1 : 0;
-    if ((rc = oz2_launch_convert(0, N, wide, m, k, A, lda, e, RA, L.kp, st))) return rc;
-    if ((rc = oz2_launch_convert(1, N, wide, n, k, B, ldb, f, RB, L.kp, st))) return rc;
+    if ((rc = oz2_launch_convert(0, N, wide, f32, m, k, A, lda, e, RA, L.kp, st))) return rc;
+    if ((rc = oz2_launch_convert(1, N, wide, f32, n, k, B, ldb, f, RB, L.kp, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[2], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[2], st));
     // ---- S3 residue GEMMs
@@ -332,7 +336,7 @@ static int run_path(int64_t m, int64_t n, int64_t k, double alpha, const double 
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[3], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[3], st));
     // ---- S4 + S5
-    if ((rc = oz2_launch_crt(N, m, n, U, L.mp, e, f, alpha, beta, C, ldc, out ? out->Cpp : nullptr, st))) return rc;
+    if ((rc = oz2_launch_crt(N, f32, m, n, U, L.mp, e, f, alpha, beta, C, ldc, out ? out->Cpp : nullptr, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[4], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[4], st));
 
@@ -418,16 +422,16 @@ static int host_pipelined(int64_t m, int64_t n, int64_t k, double alpha, const d
     }
     // ---- rows of A: S1, S2
     OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evA, 0));
-    if ((rc = oz2_launch_scale_rows(mode, N, m, k, dA, m, amax, ssq, e, st))) return rc;
-    if ((rc = oz2_launch_convert(0, N, wide, m, k, dA, m, e, RA, L.kp, st))) return rc;
+    if ((rc = oz2_launch_scale_rows(mode, N, 0, m, k, dA, m, amax, ssq, e, st))) return rc;
+    if ((rc = oz2_launch_convert(0, N, wide, 0, m, k, dA, m, e, RA, L.kp, st))) return rc;
     // ---- panels: S1, S2 of the columns, S3, S4 + S5, copy out
     for (int p = 0; p < panels; p++) {
         const int64_t j0 = p * np, nc = (j0 + np < n ? np : n - j0);
         OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evB[p], 0));
-        if ((rc = oz2_launch_scale_cols(mode, N, nc, k, dB + j0 * k, k, f, st))) return rc;
-        if ((rc = oz2_launch_convert(1, N, wide, nc, k, dB + j0 * k, k, f, RB, L.kp, st))) return rc;
+        if ((rc = oz2_launch_scale_cols(mode, N, 0, nc, k, dB + j0 * k, k, f, st))) return rc;
+        if ((rc = oz2_launch_convert(1, N, wide, 0, nc, k, dB + j0 * k, k, f, RB, L.kp, st))) return rc;
         if ((rc = oz2_launch_gemm_tc(N, 0, m, nc, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
-        if ((rc = oz2_launch_crt(N, m, nc, U, L.mp, e, f, alpha, beta, dC + j0 * m, m, nullptr, st))) return rc;
+        if ((rc = oz2_launch_crt(N, 0, m, nc, U, L.mp, e, f, alpha, beta, dC + j0 * m, m, nullptr, st))) return rc;
         OZ2_CUDA_TRY(cudaEventRecord(dev->evC[p], st));
         OZ2_CUDA_TRY(cudaStreamWaitEvent(sd, dev->evC[p], 0));
         OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host + j0 * ldc, 8 * (size_t)ldc, dC + j0 * m, 8 * (size_t)m, 8 * (size_t)m, (size_t)nc,
@@ -444,7 +448,7 @@ extern "C" {
 int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
                  int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream)
 {
-    return run_path(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+    return run_path(0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
                     static_cast<cudaStream_t>(stream), nullptr);
 }
 
@@ -452,7 +456,22 @@ int ozaki2_dgemm_stages(int64_t m, int64_t n, int64_t k, double alpha, const dou
                         int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream,
                         const ozaki2_stage_outputs *out)
 {
-    return run_path(m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+    return run_path(0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+                    static_cast<cudaStream_t>(stream), out);
+}
+
+int ozaki2_sgemm(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda, const float *B, int64_t ldb,
+                 float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream)
+{
+    return run_path(1, m, n, k, (double)alpha, A, lda, B, ldb, (double)beta, C, ldc, num_moduli, scaling_mode,
+                    static_cast<cudaStream_t>(stream), nullptr);
+}
+
+int ozaki2_sgemm_stages(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda, const float *B,
+                        int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream,
+                        const ozaki2_stage_outputs *out)
+{
+    return run_path(1, m, n, k, (double)alpha, A, lda, B, ldb, (double)beta, C, ldc, num_moduli, scaling_mode,
                     static_cast<cudaStream_t>(stream), out);
 }
 
@@ -508,7 +527,7 @@ int ozaki2_dgemm_host(int64_t m, int64_t n, int64_t k, double alpha, const doubl
     }
     if (beta != 0.0)
         OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC, 8 * (size_t)m, C_host, 8 * (size_t)ldc, 8 * (size_t)m, (size_t)n, cudaMemcpyHostToDevice, st));
-    rc = run_path(m, n, k, alpha, dA, m > 1 ? m : 1, dB, k > 1 ? k : 1, beta, dC, m > 1 ? m : 1, num_moduli, scaling_mode, st, nullptr);
+    rc = run_path(0, m, n, k, alpha, dA, m > 1 ? m : 1, dB, k > 1 ? k : 1, beta, dC, m > 1 ? m : 1, num_moduli, scaling_mode, st, nullptr);
     if (rc) return rc;
     OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host, 8 * (size_t)ldc, dC, 8 * (size_t)m, 8 * (size_t)m, (size_t)n, cudaMemcpyDeviceToHost, st));
     OZ2_CUDA_TRY(cudaStreamSynchronize(st));

@@ -51,10 +51,11 @@ int oz2_gemm_upload_tables(const Oz2HostTables &t);
 int oz2_crt_upload_tables(const Oz2HostTables &t);
 
 // S1: exponents for modes 1 and 2, and the mode-0 pieces.  stat buffers: amax[rows] (u64), ssq[rows] (u64)
-int oz2_launch_scale_rows(int mode, int N, int64_t m, int64_t k, const double *A, int64_t lda,
+// f32 != 0: the input matrices are FP32 (SGEMM variant); every element is promoted to FP64 exactly on load
+int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const void *A, int64_t lda,
                           unsigned long long *amaxA, unsigned long long *ssqA, int32_t *e, cudaStream_t st);
-int oz2_launch_scale_cols(int mode, int N, int64_t n, int64_t k, const double *B, int64_t ldb, int32_t *f, cudaStream_t st);
-int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B,
+int oz2_launch_scale_cols(int mode, int N, int f32, int64_t n, int64_t k, const void *B, int64_t ldb, int32_t *f, cudaStream_t st);
+int oz2_launch_scale_accu_prepare(int f32, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B,
                                   int64_t ldb, unsigned long long *amaxA, int32_t *EA, int32_t *EB, int8_t *Abar,
                                   int8_t *Bbar, int64_t kp, int32_t *rowmax, int32_t *colmax, cudaStream_t st);
 int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA, const int32_t *EB,
@@ -62,7 +63,7 @@ int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA,
 int oz2_launch_log2f(const float *x, float *y, int64_t count, cudaStream_t st);
 
 // S2: residues of op(X) for all N moduli in one pass.  planes: [N][rows][kp]
-int oz2_launch_convert(int op, int N, int wide, int64_t rows, int64_t k, const double *X, int64_t ldx,
+int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k, const void *X, int64_t ldx,
                        const int32_t *ex, int8_t *planes, int64_t kp, cudaStream_t st);
 
 // S3: batched INT8 GEMM with mod-p epilogue (tcgen05).  nplanes GEMMs; modulus index of plane b is mod_base + b.
@@ -75,8 +76,9 @@ int oz2_launch_gemm_check(int nplanes, int64_t m, int64_t n, int64_t k, const in
 int oz2_launch_mod_p(int l, const int32_t *in, uint8_t *out, int64_t count, cudaStream_t st);
 
 // S4 + S5: CRT, rmod P, RN to FP64, unscale, alpha / beta.  Cpp (optional): [n][m][4] u64 words.
-int oz2_launch_crt(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f,
-                   double alpha, double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st);
+// f32 != 0: C is FP32, the one rounding is RN_32, alpha / beta are applied in FP32
+int oz2_launch_crt(int N, int f32, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f,
+                   double alpha, double beta, void *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st);
 
 // kernel-launch accounting behind ozaki2_kernel_launches()
 void oz2_count_launches(int n);

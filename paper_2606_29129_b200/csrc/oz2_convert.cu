@@ -146,9 +146,9 @@ __device__ __forceinline__ void quad_bar(const double (&a)[4], int E, int8_t *ds
 // ---------------------------------------------------------------------------------------------
 // A path.  MODE 0: residues (NB words)   MODE 1: Abar
 // ---------------------------------------------------------------------------------------------
-template <int NB, int MODE>
+template <int NB, int MODE, typename T>
 __global__ void __launch_bounds__(CONV_THREADS)
-k2_rows(int N, int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, const int32_t *__restrict__ e,
+k2_rows(int N, int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, const int32_t *__restrict__ e,
         int8_t *__restrict__ planes, int64_t kp)
 {
     __shared__ __align__(16) double tile[TI * SROW];
@@ -158,12 +158,12 @@ k2_rows(int N, int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, 
     {
         const int64_t i = i0 + lane;
         const bool iok = i < m;
-        const double *src = A + i + (h0 + warp) * lda;
+        const T *src = A + i + (h0 + warp) * lda;
         double v[16];
 #pragma unroll
         for (int s = 0; s < 16; s++) {
             const int64_t h = h0 + warp + 8 * s;
-            v[s] = (iok && h < k) ? __ldg(src + (int64_t)(8 * s) * lda) : 0.0;
+            v[s] = (iok && h < k) ? (double)__ldg(src + (int64_t)(8 * s) * lda) : 0.0;
         }
 #pragma unroll
         for (int s = 0; s < 16; s++) tile[lane * SROW + warp + 8 * s] = v[s];
@@ -197,9 +197,21 @@ k2_rows(int N, int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, 
 // ---------------------------------------------------------------------------------------------
 // B path: warp = 256 consecutive h of column j; lane holds the quads at 4 lane and 128 + 4 lane
 // ---------------------------------------------------------------------------------------------
-template <int NB, int MODE>
+// four consecutive elements of a column as doubles: two 16-byte loads (FP64) or one (FP32)
+__device__ __forceinline__ void ld4(const double *p, double (&a)[4])
+{
+    const double2 v0 = __ldg(reinterpret_cast<const double2 *>(p)), v1 = __ldg(reinterpret_cast<const double2 *>(p + 2));
+    a[0] = v0.x; a[1] = v0.y; a[2] = v1.x; a[3] = v1.y;
+}
+__device__ __forceinline__ void ld4(const float *p, double (&a)[4])
+{
+    const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
+    a[0] = (double)v.x; a[1] = (double)v.y; a[2] = (double)v.z; a[3] = (double)v.w;
+}
+
+template <int NB, int MODE, typename T>
 __global__ void __launch_bounds__(CONV_THREADS)
-k2_cols(int N, int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, const int32_t *__restrict__ f,
+k2_cols(int N, int64_t n, int64_t k, const T *__restrict__ B, int64_t ldb, const int32_t *__restrict__ f,
         int8_t *__restrict__ planes, int64_t kp)
 {
     const int lane = threadIdx.x & 31;
@@ -207,7 +219,7 @@ k2_cols(int N, int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, 
     const int64_t item = (int64_t)blockIdx.x * (CONV_THREADS / 32) + (threadIdx.x >> 5);
     if (item >= n * chunks) return;
     const int64_t j = item / chunks, c = item - j * chunks;
-    const double *col = B + j * ldb;
+    const T *col = B + j * ldb;
     const int ex = __ldg(f + j);
     const bool vec = ((((uintptr_t)col) & 15) == 0);
     const int64_t plane_stride = n * kp;
@@ -216,12 +228,10 @@ k2_cols(int N, int64_t n, int64_t k, const double *__restrict__ B, int64_t ldb, 
     for (int t = 0; t < 2; t++) {
         const int64_t h = c * 256 + 128 * t + 4 * lane;
         if (vec && h + 3 < k) {
-            const double2 v0 = __ldg(reinterpret_cast<const double2 *>(col + h));
-            const double2 v1 = __ldg(reinterpret_cast<const double2 *>(col + h + 2));
-            a[t][0] = v0.x; a[t][1] = v0.y; a[t][2] = v1.x; a[t][3] = v1.y;
+            ld4(col + h, a[t]);
         } else {
 #pragma unroll
-            for (int u = 0; u < 4; u++) a[t][u] = (h + u < k) ? __ldg(col + h + u) : 0.0;
+            for (int u = 0; u < 4; u++) a[t][u] = (h + u < k) ? (double)__ldg(col + h + u) : 0.0;
         }
     }
     const int64_t h = c * 256 + 4 * lane;           // first quad; kp is a multiple of 128, so it is inside
@@ -249,25 +259,34 @@ int oz2_convert_upload_tables(const Oz2HostTables &t)
     return 0;
 }
 
-// op 0: rows of A, op 1: columns of B.  N >= 1: residue planes [N][rows][kp] with exponents `ex`.  N == 0: the
-// single plane ceil(mu' |.|) of accurate mode (P:131-133); `ex` then holds E = floor(log2 max |.|) per row.
-int oz2_launch_convert(int op, int N, int wide, int64_t rows, int64_t k, const double *X, int64_t ldx,
-                       const int32_t *ex, int8_t *planes, int64_t kp, cudaStream_t st)
+template <typename T>
+static int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *X, int64_t ldx, const int32_t *ex,
+                            int8_t *planes, int64_t kp, cudaStream_t st)
 {
-    if (rows <= 0) return 0;
     if (op == 0) {
         dim3 grid((unsigned)((rows + TI - 1) / TI), (unsigned)(kp / TH));
-        if (N == 0) k2_rows<2, 1><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else if (wide) k2_rows<3, 0><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else k2_rows<2, 0><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        if (N == 0) k2_rows<2, 1, T><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else if (wide) k2_rows<3, 0, T><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else k2_rows<2, 0, T><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
     } else {
         const int64_t items = rows * ((kp + 255) / 256);
         const unsigned gx = (unsigned)((items + CONV_THREADS / 32 - 1) / (CONV_THREADS / 32));
-        if (N == 0) k2_cols<2, 1><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else if (wide) k2_cols<3, 0><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else k2_cols<2, 0><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        if (N == 0) k2_cols<2, 1, T><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else if (wide) k2_cols<3, 0, T><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        else k2_cols<2, 0, T><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
     }
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
+}
+
+// op 0: rows of A, op 1: columns of B.  N >= 1: residue planes [N][rows][kp] with exponents `ex`.  N == 0: the
+// single plane ceil(mu' |.|) of accurate mode (P:131-133); `ex` then holds E = floor(log2 max |.|) per row.
+// f32 != 0: X is FP32 (SGEMM variant), promoted exactly on load.
+int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k, const void *X, int64_t ldx,
+                       const int32_t *ex, int8_t *planes, int64_t kp, cudaStream_t st)
+{
+    if (rows <= 0) return 0;
+    if (f32) return launch_convert_t<float>(op, N, wide, rows, k, static_cast<const float *>(X), ldx, ex, planes, kp, st);
+    return launch_convert_t<double>(op, N, wide, rows, k, static_cast<const double *>(X), ldx, ex, planes, kp, st);
 }

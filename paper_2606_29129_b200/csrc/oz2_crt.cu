@@ -25,14 +25,17 @@ __host__ __device__ constexpr int words_of_P(int N)
     return N <= 4 ? 1 : N <= 8 ? 2 : N <= 12 ? 3 : N <= 16 ? 4 : 5;
 }
 
-// RN of (mant64 | sticky) * 2^sc with a single rounding, subnormals and overflow included
+// RN of (mant64 | sticky) * 2^sc to a format with PB significand bits, subnormal quantum 2^QMIN and largest exponent
+// EMAX (FP64: 53, -1074, 1023; FP32: 24, -149, 127), with a single rounding, subnormals and overflow included.
+// The result is returned as a double (exact for both formats).
+template <int PB, int QMIN, int EMAX>
 __device__ __noinline__ double round_scaled_slow(unsigned long long mant, uint32_t sticky, int sc)
 {
     // value in [2^(63+sc), 2^(64+sc))
     int Ex = 63 + sc;
-    if (Ex > 1023) return __longlong_as_double(0x7FF0000000000000ll);
-    int rs = -1074 - sc;                          // bits dropped below the subnormal quantum 2^-1074
-    if (rs < 11) rs = 11;                         // never keep more than 53 bits
+    if (Ex > EMAX) return __longlong_as_double(0x7FF0000000000000ll);
+    int rs = QMIN - sc;                           // bits dropped below the subnormal quantum
+    if (rs < 64 - PB) rs = 64 - PB;               // never keep more than PB bits
     unsigned long long q, half, low;
     if (rs >= 65) return 0.0;
     if (rs == 64) { q = 0; half = mant >> 63; low = (mant << 1) | sticky; }
@@ -40,7 +43,7 @@ __device__ __noinline__ double round_scaled_slow(unsigned long long mant, uint32
     if (half && (low || (q & 1ull))) q += 1;
     // q * 2^(sc + rs)
     int qe = sc + rs;
-    if (qe == -1074) return __longlong_as_double((long long)q);       // subnormal (or the smallest normal)
+    if (PB == 53 && qe == -1074) return __longlong_as_double((long long)q);   // FP64 subnormal (or the smallest normal)
     double d = (double)(long long)q;                                   // q <= 2^53: exact
     // qe > -1074 here means the result is normal; scale in two exact steps to stay in range
     int h1 = qe / 2, h2 = qe - h1;
@@ -50,9 +53,10 @@ __device__ __noinline__ double round_scaled_slow(unsigned long long mant, uint32
 }
 
 // C'' = rmod(C', P), RN_64(C'') 2^-esum from the words c[0..NW] of C' = sum_l w_l U_l (c[NW] < 2^13)
-template <int NW>
-__device__ __forceinline__ double crt_from_words(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum,
-                                                 uint64_t *cpp_out)
+// TO = double: RN_64; TO = float: RN_32 of the same exact integer (SGEMM variant)
+template <int NW, typename TO>
+__device__ __forceinline__ TO crt_from_words(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum,
+                                             uint64_t *cpp_out)
 {
     // ---- Q = round(C' / P), estimated from the top three words
     double top = (double)(long long)(((unsigned long long)c[NW] << 32) | c[NW - 1]);
@@ -121,21 +125,32 @@ __device__ __forceinline__ double crt_from_words(const uint32_t (&c)[NW + 1], co
     if (NW >= 5 && X2 != 0ull) { ptop = X2; pmid = X1; plow = X0; base = 128; }
     else if (NW >= 3 && X1 != 0ull) { ptop = X1; pmid = X0; plow = 0ull; base = 64; }
     else { ptop = X0; pmid = 0ull; plow = 0ull; base = 0; }
-    if (ptop == 0ull) return 0.0;
+    if (ptop == 0ull) return (TO)0;
     const int lz = __clzll((long long)ptop);
     const unsigned long long mant = (ptop << lz) | ((pmid >> 1) >> (63 - lz));
     const uint32_t sticky = (((pmid << lz) | plow) != 0ull) ? 1u : 0u;
     const int pos = base + 63 - lz;                                   // |C''| in [2^pos, 2^(pos+1))
     const int sc = pos - 63 - esum;                                   // result = mant 2^sc
-    double v;
     const int Ex = pos - esum;
-    if (Ex >= -1020 && Ex <= 1021) {
-        const double d = __ull2double_rn(mant | sticky);              // the one rounding, ties to even
-        v = __longlong_as_double(__double_as_longlong(d) + ((long long)sc << 52));
+    if constexpr (sizeof(TO) == 8) {
+        double v;
+        if (Ex >= -1020 && Ex <= 1021) {
+            const double d = __ull2double_rn(mant | sticky);          // the one rounding, ties to even
+            v = __longlong_as_double(__double_as_longlong(d) + ((long long)sc << 52));
+        } else {
+            v = round_scaled_slow<53, -1074, 1023>(mant, sticky, sc);
+        }
+        return __longlong_as_double(__double_as_longlong(v) | (long long)(m64 << 63));
     } else {
-        v = round_scaled_slow(mant, sticky, sc);
+        float v;
+        if (Ex >= -124 && Ex <= 125) {
+            const float d = __ull2float_rn(mant | sticky);            // the one rounding, ties to even
+            v = __int_as_float(__float_as_int(d) + sc * 8388608);
+        } else {
+            v = (float)round_scaled_slow<24, -149, 127>(mant, sticky, sc);      // exact conversion
+        }
+        return __int_as_float(__float_as_int(v) | (int)((uint32_t)negm & 0x80000000u));
     }
-    return __longlong_as_double(__double_as_longlong(v) | (long long)(m64 << 63));
 }
 
 // =============================================================================================
@@ -170,9 +185,9 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
 }
 
 // fold the byte slices S[0 .. 4 NW) of one element into C' and finish (C'' -> C -> alpha / beta -> store)
-template <int NW, bool WANT_CPP>
+template <int NW, bool WANT_CPP, typename TO>
 __device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T, int64_t i, int64_t j, int64_t m, int esum,
-                                          double alpha, double beta, double *__restrict__ C, int64_t ldc,
+                                          TO alpha, TO beta, TO *__restrict__ C, int64_t ldc,
                                           uint64_t *__restrict__ Cpp)
 {
     uint32_t c[NW + 1];
@@ -186,16 +201,21 @@ __device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T,
     }
     c[NW] = (uint32_t)carry;
     uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr;
-    const double cij = crt_from_words<NW>(c, T, esum, cpp);
-    const double tt = alpha * cij;
-    double *dst = C + i + j * ldc;
-    *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
+    const TO cij = crt_from_words<NW, TO>(c, T, esum, cpp);
+    TO *dst = C + i + j * ldc;
+    if constexpr (sizeof(TO) == 8) {
+        const double tt = alpha * cij;
+        *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
+    } else {
+        const float tt = __fmul_rn(alpha, cij);
+        *dst = (beta == 0.0f) ? tt : __fmaf_rn(beta, *dst, tt);
+    }
 }
 
-template <int NW, bool WANT_CPP>
+template <int NW, bool WANT_CPP, typename TO>
 __global__ void __launch_bounds__(K5_THREADS, NW <= 4 ? 3 : 2)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n, const int32_t *__restrict__ e,
-          const int32_t *__restrict__ f, double alpha, double beta, double *__restrict__ C, int64_t ldc,
+          const int32_t *__restrict__ f, TO alpha, TO beta, TO *__restrict__ C, int64_t ldc,
           uint64_t *__restrict__ Cpp)
 {
     constexpr int NS = NW <= 4 ? 16 : 32;                    // byte slices = MMA N
@@ -310,17 +330,17 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
             if (lane == 0) mbar_arrive_a(tempty + 8 * b);
             b += 2;
             if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
-            if (i < m) k5_finish<NW, WANT_CPP>(S, T, i, jcur, m, e0 + fj, alpha, beta, C, ldc, Cpp);
-            if (i + 128 < m) k5_finish<NW, WANT_CPP>(S + NS, T, i + 128, jcur, m, e1 + fj, alpha, beta, C, ldc, Cpp);
+            if (i < m) k5_finish<NW, WANT_CPP, TO>(S, T, i, jcur, m, e0 + fj, alpha, beta, C, ldc, Cpp);
+            if (i + 128 < m) k5_finish<NW, WANT_CPP, TO>(S + NS, T, i + 128, jcur, m, e1 + fj, alpha, beta, C, ldc, Cpp);
         }
     }
     __syncthreads();
     if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(K5_NBUF * BUF_COLS) : "memory");
 }
 
-template <int NW>
-int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f, double alpha,
-              double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
+template <int NW, typename TO>
+int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f, TO alpha,
+              TO beta, TO *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
 {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return (int)cudaErrorNotSupported;
@@ -344,8 +364,8 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
     const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads
     int64_t grid = (int64_t)sms * per_sm;
     if (grid > tiles) grid = tiles;
-    if (Cpp) k5_crt_tc<NW, true><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, Cpp);
-    else k5_crt_tc<NW, false><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, nullptr);
+    if (Cpp) k5_crt_tc<NW, true, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, Cpp);
+    else k5_crt_tc<NW, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, nullptr);
     oz2_count_launches(1);
     return (int)cudaGetLastError();
 }
@@ -368,16 +388,24 @@ int oz2_crt_upload_tables(const Oz2HostTables &t)
     return 0;
 }
 
-int oz2_launch_crt(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f,
-                   double alpha, double beta, double *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
+template <typename TO>
+static int launch_crt_t(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f,
+                        TO alpha, TO beta, TO *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
+{
+    switch (words_of_P(N)) {
+        case 1: return launch_tc<1, TO>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        case 2: return launch_tc<2, TO>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        case 3: return launch_tc<3, TO>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        case 4: return launch_tc<4, TO>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+        default: return launch_tc<5, TO>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
+    }
+}
+
+int oz2_launch_crt(int N, int f32, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f,
+                   double alpha, double beta, void *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
 {
     if (m <= 0 || n <= 0) return 0;
     if (N < 2 || N > OZ2_MAX_MODULI) return -1;
-    switch (words_of_P(N)) {
-        case 1: return launch_tc<1>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
-        case 2: return launch_tc<2>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
-        case 3: return launch_tc<3>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
-        case 4: return launch_tc<4>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
-        default: return launch_tc<5>(N, m, n, U, mp, e, f, alpha, beta, C, ldc, Cpp, st);
-    }
+    if (f32) return launch_crt_t<float>(N, m, n, U, mp, e, f, (float)alpha, (float)beta, static_cast<float *>(C), ldc, Cpp, st);
+    return launch_crt_t<double>(N, m, n, U, mp, e, f, alpha, beta, static_cast<double *>(C), ldc, Cpp, st);
 }

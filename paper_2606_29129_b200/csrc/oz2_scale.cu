@@ -123,16 +123,16 @@ __device__ int exponent_accurate(const Oz2CrtTab &c, int E, int M)
 // ---------------------------------------------------------------------------------------------
 // rows of A
 // ---------------------------------------------------------------------------------------------
-template <int PASS> // 0: max |a|   1: sum of squared, normalised terms
+template <int PASS, typename T> // PASS 0: max |a|   1: sum of squared, normalised terms;  T: double or float (SGEMM)
 __global__ void __launch_bounds__(ROWS_PER_BLOCK *KSLICES)
-k1_rows(int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, int64_t kchunk,
+k1_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, int64_t kchunk,
         unsigned long long *__restrict__ amax, unsigned long long *__restrict__ ssq)
 {
     int64_t i = (int64_t)blockIdx.x * ROWS_PER_BLOCK + threadIdx.x;
     int64_t h0 = (int64_t)blockIdx.y * kchunk;
     int64_t h1 = h0 + kchunk < k ? h0 + kchunk : k;
     if (i >= m) return;
-    const double *p = A + i;
+    const T *p = A + i;
     unsigned long long acc = 0;
     int E = 0;
     if (PASS == 1) {
@@ -144,7 +144,7 @@ k1_rows(int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, int64_t
     for (; h + 7 * KSLICES < h1; h += 8 * KSLICES) {
         double v[8];
 #pragma unroll
-        for (int u = 0; u < 8; u++) v[u] = __ldg(p + (h + u * KSLICES) * lda);
+        for (int u = 0; u < 8; u++) v[u] = (double)__ldg(p + (h + u * KSLICES) * lda);
 #pragma unroll
         for (int u = 0; u < 8; u++) {
             unsigned long long b = abs_bits(v[u]);
@@ -153,7 +153,7 @@ k1_rows(int64_t m, int64_t k, const double *__restrict__ A, int64_t lda, int64_t
         }
     }
     for (; h < h1; h += KSLICES) {
-        unsigned long long b = abs_bits(__ldg(p + h * lda));
+        unsigned long long b = abs_bits((double)__ldg(p + h * lda));
         if (PASS == 0) acc = b > acc ? b : acc;
         else acc += sq_term(b, E);
     }
@@ -188,24 +188,32 @@ __device__ __forceinline__ unsigned long long block_reduce(unsigned long long v,
 }
 
 // MODE 1/2: f[j]; MODE 0 (accurate prepare): EB[j] only
-template <bool ACCU>
+// two consecutive elements of a column as doubles (16-byte load for FP64, 8-byte for FP32)
+__device__ __forceinline__ double2 ld2(const double *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+__device__ __forceinline__ double2 ld2(const float *p)
+{
+    const float2 v = __ldg(reinterpret_cast<const float2 *>(p));
+    return make_double2((double)v.x, (double)v.y);
+}
+
+template <bool ACCU, typename T>
 __global__ void __launch_bounds__(COL_THREADS)
-k1_cols(int mode, int N, int64_t k, const double *__restrict__ B, int64_t ldb, int32_t *__restrict__ f,
+k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_t *__restrict__ f,
         int32_t *__restrict__ EB)
 {
     __shared__ unsigned long long sm[COL_THREADS / 32];
-    const double *col = B + (int64_t)blockIdx.x * ldb;
-    bool vec = ((((uintptr_t)col) & 15) == 0);
+    const T *col = B + (int64_t)blockIdx.x * ldb;
+    bool vec = ((((uintptr_t)col) & (2 * sizeof(T) - 1)) == 0);
     unsigned long long mx = 0;
     int64_t kv = vec ? (k & ~(int64_t)1) : 0;
     for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {
-        double2 v = __ldg(reinterpret_cast<const double2 *>(col + h));
+        double2 v = ld2(col + h);
         unsigned long long b0 = abs_bits(v.x), b1 = abs_bits(v.y);
         mx = b0 > mx ? b0 : mx;
         mx = b1 > mx ? b1 : mx;
     }
     for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) {
-        unsigned long long b = abs_bits(__ldg(col + h));
+        unsigned long long b = abs_bits((double)__ldg(col + h));
         mx = b > mx ? b : mx;
     }
     mx = block_reduce(mx, true, sm);
@@ -220,10 +228,10 @@ k1_cols(int mode, int N, int64_t k, const double *__restrict__ B, int64_t ldb, i
     int E = floor_log2_bits(mx);
     unsigned long long acc = 0;
     for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {      // second read: L2 hits
-        double2 v = __ldg(reinterpret_cast<const double2 *>(col + h));
+        double2 v = ld2(col + h);
         acc += sq_term(abs_bits(v.x), E) + sq_term(abs_bits(v.y), E);
     }
-    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits(__ldg(col + h)), E);
+    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits((double)__ldg(col + h)), E);
     acc = block_reduce(acc, false, sm);
     if (threadIdx.x == 0) f[blockIdx.x] = exponent_fastprop(mode, c_crt[N], mx, acc);
 }
@@ -274,33 +282,41 @@ int oz2_scale_upload_tables(const Oz2HostTables &t)
     return 0;
 }
 
-int oz2_launch_scale_rows(int mode, int N, int64_t m, int64_t k, const double *A, int64_t lda,
+int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const void *Av, int64_t lda,
                           unsigned long long *amaxA, unsigned long long *ssqA, int32_t *e, cudaStream_t st)
 {
+    const double *A = static_cast<const double *>(Av);
+    const float *Af = static_cast<const float *>(Av);
     if (m <= 0) return 0;
     OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
     OZ2_CUDA_TRY(cudaMemsetAsync(ssqA, 0, sizeof(unsigned long long) * (size_t)m, st));
     int64_t kchunk;
     int gy = rows_grid_y(m, k, &kchunk);
     dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
-    k1_rows<0><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
-    k1_rows<1><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
+    if (f32) {
+        k1_rows<0, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA);
+        k1_rows<1, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA);
+    } else {
+        k1_rows<0, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
+        k1_rows<1, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
+    }
     k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e);
     oz2_count_launches(3);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
 
-int oz2_launch_scale_cols(int mode, int N, int64_t n, int64_t k, const double *B, int64_t ldb, int32_t *f, cudaStream_t st)
+int oz2_launch_scale_cols(int mode, int N, int f32, int64_t n, int64_t k, const void *B, int64_t ldb, int32_t *f, cudaStream_t st)
 {
     if (n <= 0) return 0;
-    k1_cols<false><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, B, ldb, f, nullptr);
+    if (f32) k1_cols<false, float><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const float *>(B), ldb, f, nullptr);
+    else k1_cols<false, double><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const double *>(B), ldb, f, nullptr);
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
 
-int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double *A, int64_t lda, const double *B,
+int oz2_launch_scale_accu_prepare(int f32, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B,
                                   int64_t ldb, unsigned long long *amaxA, int32_t *EA, int32_t *EB, int8_t *Abar,
                                   int8_t *Bbar, int64_t kp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
 {
@@ -310,14 +326,16 @@ int oz2_launch_scale_accu_prepare(int64_t m, int64_t n, int64_t k, const double 
     int64_t kchunk;
     int gy = rows_grid_y(m, k, &kchunk);
     dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
-    k1_rows<0><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, nullptr);
+    if (f32) k1_rows<0, float><<<grid, block, 0, st>>>(m, k, static_cast<const float *>(A), lda, kchunk, amaxA, nullptr);
+    else k1_rows<0, double><<<grid, block, 0, st>>>(m, k, static_cast<const double *>(A), lda, kchunk, amaxA, nullptr);
     k1_rows_E<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(m, amaxA, EA);
-    k1_cols<true><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, B, ldb, nullptr, EB);
+    if (f32) k1_cols<true, float><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const float *>(B), ldb, nullptr, EB);
+    else k1_cols<true, double><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const double *>(B), ldb, nullptr, EB);
     oz2_count_launches(3);
     OZ2_CUDA_TRY(cudaGetLastError());
     int rc;
-    if ((rc = oz2_launch_convert(0, 0, 0, m, k, A, lda, EA, Abar, kp, st))) return rc;
-    if ((rc = oz2_launch_convert(1, 0, 0, n, k, B, ldb, EB, Bbar, kp, st))) return rc;
+    if ((rc = oz2_launch_convert(0, 0, 0, f32, m, k, A, lda, EA, Abar, kp, st))) return rc;
+    if ((rc = oz2_launch_convert(1, 0, 0, f32, n, k, B, ldb, EB, Bbar, kp, st))) return rc;
     return 0;
 }
 
