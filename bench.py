@@ -26,6 +26,8 @@ import sys
 import threading
 import time
 
+import numpy as np
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
@@ -44,6 +46,8 @@ def parse_args():
     ap.add_argument("--moduli", type=int, default=16, help="number of moduli N (BASELINE configs[2]: 14..18)")
     ap.add_argument("--mode", type=int, default=2, help="0 accurate, 1 original fast, 2 revised fast (headline)")
     ap.add_argument("--size", type=int, default=8192, help="m = n = k (8192 is the BASELINE workload)")
+    ap.add_argument("--sgemm", action="store_true", help="SURVEY 8(f) #1: the FP32 in / FP32 out variant (paper: N = 3..12); "
+                    "no host-buffer entry point exists for it, so e2e is null")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: leave out the oracle leg")
     return ap.parse_args()
@@ -133,7 +137,7 @@ def time_oracle_slab(A, B, N, mode, shape):
     ms, ns, k = shape
     As, Bs = A[:ms, :], B[:, :ns]
     t0 = time.perf_counter()
-    Cs = O.dgemm(As, Bs, N, mode)
+    Cs = (O.sgemm if As.dtype == np.float32 else O.dgemm)(As, Bs, N, mode)
     dt = time.perf_counter() - t0
     return Cs, dt, O.num_threads()
 
@@ -204,8 +208,12 @@ def main():
 
     # ---- inputs: eq. (15), seeded, one variant per rank (replicas)
     A, B = W.config_matrices(2, rank, shape=(m, n, k))
-    Ad, Bd = pkg.colmajor_to_device(A), pkg.colmajor_to_device(B)
-    Cd = torch.empty((n, m), dtype=torch.float64, device="cuda")
+    f32 = bool(args.sgemm)
+    npdt, tdt, esz = (np.float32, torch.float32, 4) if f32 else (np.float64, torch.float64, 8)
+    if f32:
+        A, B = np.asfortranarray(A.astype(np.float32)), np.asfortranarray(B.astype(np.float32))
+    Ad, Bd = pkg.colmajor_to_device(A, npdt), pkg.colmajor_to_device(B, npdt)
+    Cd = torch.empty((n, m), dtype=tdt, device="cuda")
     pkg.ensure_workspace(m, n, k, N, mode)
     stream = torch.cuda.current_stream()
 
@@ -216,9 +224,9 @@ def main():
 
     def step(events=None):
         if events is None:
-            rc = pkg.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, stream)
+            rc = (pkg.ozaki2_sgemm if f32 else pkg.ozaki2_dgemm)(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, stream)
         else:
-            rc = pkg.dgemm_with_stage_events(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, events, stream)
+            rc = pkg.dgemm_with_stage_events(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, events, stream, f32=f32)
         if rc:
             raise pkg.Ozaki2Error(rc, "ozaki2_dgemm")
 
@@ -267,13 +275,13 @@ def main():
                     frac_of_nominal_4500=achieved / NOMINAL_INT8_TOPS, ms_per_launch=s3_ms,
                     traffic=profiled_traffic(m, N, mode), traffic_unit="bytes per launch (ncu dram read + write, profiles/r01b)",
                     algorithmic_bytes=N * X + N * Y)
-    stage_bytes = [8 * X if mode != 0 else 8 * X + 2 * X, (8 + N) * X, N * X + N * Y, (N + 8) * Y]
+    stage_bytes = [esz * X if mode != 0 else esz * X + 2 * X, (esz + N) * X, N * X + N * Y, (N + esz) * Y]
     stages = {}
     for nm, ms_, by in zip(("S1_scaling", "S2_conversion", "S3_residue_gemm", "S4S5_crt_unscale"), stage_ms, stage_bytes):
         stages[nm] = dict(ms=ms_, algorithmic_gb=by / 1e9, gbs=by / (ms_ * 1e-3) / 1e9,
                           hbm_frac=by / (ms_ * 1e-3) / 1e9 / peaks["hbm_gbs"])
     stages["S3_residue_gemm"]["int8_tops"] = achieved
-    total_bytes = (16 + 2 * N) * X + (2 * N + 8) * Y
+    total_bytes = (2 * esz + 2 * N) * X + (2 * N + esz) * Y
     t_roof_ms = max(s3_ops / (int8_peak * 1e12), total_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
     t_roof_nominal_ms = max(s3_ops / (NOMINAL_INT8_TOPS * 1e12), total_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
     path = dict(roofline_ms=t_roof_ms, frac=t_roof_ms / ms_per_step, roofline_ms_nominal_4500=t_roof_nominal_ms,
@@ -282,7 +290,7 @@ def main():
 
     # ---- e2e: host buffers through ozaki2_dgemm_host (pinned), copies inside the timed region
     e2e = None
-    if not args.skip_e2e:
+    if not args.skip_e2e and not f32:
         Ah = torch.empty((k, m), dtype=torch.float64, pin_memory=True)
         Bh = torch.empty((n, k), dtype=torch.float64, pin_memory=True)
         Ch = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
@@ -332,13 +340,15 @@ def main():
             cpu["gpu_slab_bit_exact_vs_oracle"] = bool(np.array_equal(Cg, Cs))
 
     if rank == 0:
-        line = dict(metric="emulated_fp64_tflops", value=value, unit="TFLOPS", n_gpus=world, steps=K, warmup=Wm,
+        line = dict(metric="emulated_fp32_tflops" if f32 else "emulated_fp64_tflops", value=value, unit="TFLOPS",
+                    n_gpus=world, steps=K, warmup=Wm,
                     ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
-                    dtype="int8xint8->int32 (tcgen05 kind::i8), fp64 in/out", data="synthetic",
-                    config=dict(workload=f"BASELINE configs[2]: m=n=k={m}, eq.(15) phi=0.5, N={N} moduli, "
-                                         f"mode={MODE_NAMES[mode]}", moduli=N, scaling_mode=MODE_NAMES[mode],
+                    dtype="int8xint8->int32 (tcgen05 kind::i8), %s in/out" % ("fp32" if f32 else "fp64"), data="synthetic",
+                    config=dict(workload=f"BASELINE configs[2]%s: m=n=k={m}, eq.(15) phi=0.5, N={N} moduli, "
+                                         f"mode={MODE_NAMES[mode]}" % (" as SGEMM (SURVEY 8(f) #1)" if f32 else ""),
+                                moduli=N, scaling_mode=MODE_NAMES[mode],
                                 l2="inputs larger than L2 (A + B = %.2f GB per step, residue planes %.2f GB)" %
-                                   (8 * X / 1e9, N * X / 1e9), parallelism="replicas" if world > 1 else "single GPU"),
+                                   (esz * X / 1e9, N * X / 1e9), parallelism="replicas" if world > 1 else "single GPU"),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, stages=stages, path=path,
                     cpu_baseline=cpu, peaks=dict(hbm_gbs=peaks["hbm_gbs"], bf16_tflops=peaks["bf16"],
                                                  bf16_tflops_sustained=peaks["bf16_sustained"], source=peaks["source"]),

@@ -234,14 +234,16 @@ def dgemm(A_dev, B_dev, num_moduli, scaling_mode=OZAKI2_MODE_PROP, alpha=1.0, be
     return C_dev
 
 
-def dgemm_with_stage_events(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, events, stream=None) -> int:
+def dgemm_with_stage_events(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, events, stream=None,
+                            f32=False) -> int:
     """ozaki2_dgemm_stages with nothing but `stage_events`: the same kernels as ozaki2_dgemm, plus five
     cudaEventRecord calls.  `events`: five torch.cuda.Event(enable_timing=True) that have been recorded once
     (torch creates the CUDA event lazily).  No synchronisation."""
     out = ozaki2_stage_outputs()
     arr = (C.c_void_p * 5)(*[ev.cuda_event for ev in events])
     out.stage_events = C.cast(arr, C.POINTER(C.c_void_p))
-    return ozaki2_dgemm_stages(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream, out)
+    call = ozaki2_sgemm_stages if f32 else ozaki2_dgemm_stages
+    return call(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream, out)
 
 
 def dgemm_stages(A_dev, B_dev, num_moduli, scaling_mode, alpha=1.0, beta=0.0, C_dev=None, want=("e", "f", "resA", "resB", "U", "Cpp"),
