@@ -61,6 +61,17 @@ int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A,
                  int num_moduli, int scaling_mode, void *stream);
 
 /*
+ * Transposed operands (the paper states C = A B only): C := alpha op(A) op(B) + beta C with
+ * op(X) = X (trans = 0) or X^T (trans = 1).  A is stored m x k (transa = 0) or k x m (transa = 1), B is stored
+ * k x n or n x k, column-major, lda / ldb >= the stored row count.  Same results as ozaki2_dgemm on the
+ * materialised op(A), op(B), bit for bit.  Errors: -1 / -2 for a bad flag, then -(i + 2) for argument i of
+ * ozaki2_dgemm.
+ */
+int ozaki2_dgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha, const double *A,
+                   int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc,
+                   int num_moduli, int scaling_mode, void *stream);
+
+/*
  * SGEMM variant (Fig. 6): A, B, C are FP32 (4-byte aligned device pointers, same
  * column-major conventions).  Every FP32 input is an FP64 number, so S1-S4 are the steps above on
  * the promoted inputs; S5 rounds the exact integer once to FP32, C = RN_32(C'' 2^-(e_i+f_j)), and

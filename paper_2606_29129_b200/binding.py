@@ -47,6 +47,8 @@ def lib() -> C.CDLL:
         L.ozaki2_dgemm.restype = ci
         L.ozaki2_dgemm_stages.argtypes = gemm_args + [C.POINTER(ozaki2_stage_outputs)]
         L.ozaki2_dgemm_stages.restype = ci
+        L.ozaki2_dgemm_t.argtypes = [ci, ci] + gemm_args
+        L.ozaki2_dgemm_t.restype = ci
         sgemm_args = [i64, i64, i64, C.c_float, vp, i64, vp, i64, C.c_float, vp, i64, ci, ci, vp]
         L.ozaki2_sgemm.argtypes = sgemm_args
         L.ozaki2_sgemm.restype = ci
@@ -132,6 +134,11 @@ def ozaki2_dgemm_stages(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_modul
                         out: ozaki2_stage_outputs | None = None) -> int:
     return int(lib().ozaki2_dgemm_stages(m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc, num_moduli,
                                          scaling_mode, _stream(stream), C.byref(out) if out is not None else None))
+
+
+def ozaki2_dgemm_t(transa, transb, m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None) -> int:
+    return int(lib().ozaki2_dgemm_t(transa, transb, m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc,
+                                    num_moduli, scaling_mode, _stream(stream)))
 
 
 def ozaki2_sgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None) -> int:

@@ -211,8 +211,8 @@ Layout make_layout(int64_t m, int64_t n, int64_t k, int N, int mode)
     size_t o = 0;
     L.off_e = o;      o = align_up(o + 4 * (size_t)m);
     L.off_f = o;      o = align_up(o + 4 * (size_t)n);
-    L.off_amax = o;   o = align_up(o + 8 * (size_t)m);
-    L.off_ssq = o;    o = align_up(o + 8 * (size_t)m);
+    L.off_amax = o;   o = align_up(o + 8 * (size_t)(m > n ? m : n));      // strided side: rows of A, or of B^T
+    L.off_ssq = o;    o = align_up(o + 8 * (size_t)(m > n ? m : n));
     L.off_EA = o;     o = align_up(o + 4 * (size_t)m);
     L.off_EB = o;     o = align_up(o + 4 * (size_t)n);
     L.off_rowmax = o; o = align_up(o + 4 * (size_t)m);
@@ -240,15 +240,16 @@ bool needs_wide_words(int N, int mode)
 }
 
 int check_args(int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B, int64_t ldb,
-               const void *C, int64_t ldc, int N, int mode)
+               const void *C, int64_t ldc, int N, int mode, int transa = 0, int transb = 0)
 {
+    const int64_t rows_a = transa ? k : m, rows_b = transb ? n : k;
     if (m < 0) return -1;
     if (n < 0) return -2;
     if (k < 0 || k > OZAKI2_MAX_K) return -3;
     if (m > 0 && k > 0 && !A) return -5;
-    if (lda < (m > 1 ? m : 1)) return -6;
+    if (lda < (rows_a > 1 ? rows_a : 1)) return -6;
     if (n > 0 && k > 0 && !B) return -7;
-    if (ldb < (k > 1 ? k : 1)) return -8;
+    if (ldb < (rows_b > 1 ? rows_b : 1)) return -8;
     if (m > 0 && n > 0 && !C) return -10;
     if (ldc < (m > 1 ? m : 1)) return -11;
     if (N < OZAKI2_MIN_MODULI || N > OZAKI2_MAX_MODULI) return -12;
@@ -274,11 +275,15 @@ __global__ void k_scale_c(int64_t m, int64_t n, T beta, T *C, int64_t ldc)
 // the path
 // =============================================================================================
 // f32 = 0: ozaki2_dgemm (A, B, C FP64); f32 = 1: ozaki2_sgemm (A, B, C FP32; alpha, beta hold floats)
+// transa / transb != 0: the stored matrix is op(X)^T (k x m for A, n x k for B, column-major).  The vectors whose
+// statistics and residues are needed -- rows of op(A), columns of op(B) -- are then contiguous for A and strided for
+// B, i.e. the two movers / reductions simply swap sides.
 static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda, const void *B,
                     int64_t ldb, double beta, void *C, int64_t ldc, int N, int mode, cudaStream_t st,
-                    const ozaki2_stage_outputs *out)
+                    const ozaki2_stage_outputs *out, int transa = 0, int transb = 0)
 {
-    int rc = check_args(m, n, k, A, lda, B, ldb, C, ldc, N, mode);
+    int rc = check_args(m, n, k, A, lda, B, ldb, C, ldc, N, mode, transa, transb);
+    const int strided_a = transa ? 0 : 1, strided_b = transb ? 1 : 0;
     if (rc) return rc;
     if (m == 0 || n == 0) return 0;
     DeviceState *dev = nullptr;
@@ -316,19 +321,26 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
     // ---- S1 scaling
     if (mode == OZAKI2_MODE_ACCURATE) {
         int8_t *Abar = reinterpret_cast<int8_t *>(ws + L.off_Abar), *Bbar = reinterpret_cast<int8_t *>(ws + L.off_Bbar);
-        if ((rc = oz2_launch_scale_accu_prepare(f32, m, n, k, A, lda, B, ldb, amax, EA, EB, Abar, Bbar, L.kp, rowmax, colmax, st))) return rc;
+        OZ2_CUDA_TRY(cudaMemsetAsync(rowmax, 0, sizeof(int32_t) * (size_t)m, st));
+        OZ2_CUDA_TRY(cudaMemsetAsync(colmax, 0, sizeof(int32_t) * (size_t)n, st));
+        if ((rc = oz2_launch_scale_accu_side(f32, strided_a, m, k, A, lda, amax, EA, Abar, L.kp, st))) return rc;
+        if ((rc = oz2_launch_scale_accu_side(f32, strided_b, n, k, B, ldb, amax, EB, Bbar, L.kp, st))) return rc;
         if ((rc = oz2_launch_gemm_tc(1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
         if ((rc = oz2_launch_scale_accu_finish(N, m, n, EA, EB, rowmax, colmax, e, f, st))) return rc;
     } else {
-        if ((rc = oz2_launch_scale_rows(mode, N, f32, m, k, A, lda, amax, ssq, e, st))) return rc;
-        if ((rc = oz2_launch_scale_cols(mode, N, f32, n, k, B, ldb, f, st))) return rc;
+        if (strided_a) rc = oz2_launch_scale_rows(mode, N, f32, m, k, A, lda, amax, ssq, e, st);
+        else rc = oz2_launch_scale_cols(mode, N, f32, m, k, A, lda, e, st);
+        if (rc) return rc;
+        if (strided_b) rc = oz2_launch_scale_rows(mode, N, f32, n, k, B, ldb, amax, ssq, f, st);
+        else rc = oz2_launch_scale_cols(mode, N, f32, n, k, B, ldb, f, st);
+        if (rc) return rc;
     }
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[1], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[1], st));
     // ---- S2 conversion
     const int wide = needs_wide_words(N, mode) ? 1 : 0;
-    if ((rc = oz2_launch_convert(0, N, wide, f32, m, k, A, lda, e, RA, L.kp, st))) return rc;
-    if ((rc = oz2_launch_convert(1, N, wide, f32, n, k, B, ldb, f, RB, L.kp, st))) return rc;
+    if ((rc = oz2_launch_convert(strided_a ? 0 : 1, N, wide, f32, m, k, A, lda, e, RA, L.kp, st))) return rc;
+    if ((rc = oz2_launch_convert(strided_b ? 0 : 1, N, wide, f32, n, k, B, ldb, f, RB, L.kp, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[2], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[2], st));
     // ---- S3 residue GEMMs
@@ -473,6 +485,17 @@ int ozaki2_sgemm_stages(int64_t m, int64_t n, int64_t k, float alpha, const floa
 {
     return run_path(1, m, n, k, (double)alpha, A, lda, B, ldb, (double)beta, C, ldc, num_moduli, scaling_mode,
                     static_cast<cudaStream_t>(stream), out);
+}
+
+int ozaki2_dgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
+                   const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode,
+                   void *stream)
+{
+    if (transa != 0 && transa != 1) return -1;
+    if (transb != 0 && transb != 1) return -2;
+    const int rc = run_path(0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+                            static_cast<cudaStream_t>(stream), nullptr, transa, transb);
+    return rc < 0 && rc > -100 ? rc - 2 : rc;              // argument numbers shift by the two leading flags
 }
 
 size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode)

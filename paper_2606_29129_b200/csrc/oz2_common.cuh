@@ -55,9 +55,8 @@ int oz2_crt_upload_tables(const Oz2HostTables &t);
 int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const void *A, int64_t lda,
                           unsigned long long *amaxA, unsigned long long *ssqA, int32_t *e, cudaStream_t st);
 int oz2_launch_scale_cols(int mode, int N, int f32, int64_t n, int64_t k, const void *B, int64_t ldb, int32_t *f, cudaStream_t st);
-int oz2_launch_scale_accu_prepare(int f32, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B,
-                                  int64_t ldb, unsigned long long *amaxA, int32_t *EA, int32_t *EB, int8_t *Abar,
-                                  int8_t *Bbar, int64_t kp, int32_t *rowmax, int32_t *colmax, cudaStream_t st);
+int oz2_launch_scale_accu_side(int f32, int strided, int64_t cnt, int64_t k, const void *X, int64_t ldx,
+                               unsigned long long *amax, int32_t *E, int8_t *bar, int64_t kp, cudaStream_t st);
 int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA, const int32_t *EB,
                                  const int32_t *rowmax, const int32_t *colmax, int32_t *e, int32_t *f, cudaStream_t st);
 int oz2_launch_log2f(const float *x, float *y, int64_t count, cudaStream_t st);

@@ -316,27 +316,29 @@ int oz2_launch_scale_cols(int mode, int N, int f32, int64_t n, int64_t k, const 
     return 0;
 }
 
-int oz2_launch_scale_accu_prepare(int f32, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B,
-                                  int64_t ldb, unsigned long long *amaxA, int32_t *EA, int32_t *EB, int8_t *Abar,
-                                  int8_t *Bbar, int64_t kp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
+// accurate mode, one side: E[i] = floor(log2 max_h |x_ih|) for the `cnt` vectors of length k of X, and the INT8 plane
+// ceil(|x| 2^(5-E)).  strided != 0: vector i is X[i + h ldx] (rows of a column-major matrix), else
+// X[h + i ldx] (its columns).  amax: u64 scratch of `cnt` entries (strided side only).
+int oz2_launch_scale_accu_side(int f32, int strided, int64_t cnt, int64_t k, const void *X, int64_t ldx,
+                               unsigned long long *amax, int32_t *E, int8_t *bar, int64_t kp, cudaStream_t st)
 {
-    OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
-    OZ2_CUDA_TRY(cudaMemsetAsync(rowmax, 0, sizeof(int32_t) * (size_t)m, st));
-    OZ2_CUDA_TRY(cudaMemsetAsync(colmax, 0, sizeof(int32_t) * (size_t)n, st));
-    int64_t kchunk;
-    int gy = rows_grid_y(m, k, &kchunk);
-    dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
-    if (f32) k1_rows<0, float><<<grid, block, 0, st>>>(m, k, static_cast<const float *>(A), lda, kchunk, amaxA, nullptr);
-    else k1_rows<0, double><<<grid, block, 0, st>>>(m, k, static_cast<const double *>(A), lda, kchunk, amaxA, nullptr);
-    k1_rows_E<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(m, amaxA, EA);
-    if (f32) k1_cols<true, float><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const float *>(B), ldb, nullptr, EB);
-    else k1_cols<true, double><<<(unsigned)n, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const double *>(B), ldb, nullptr, EB);
-    oz2_count_launches(3);
+    if (cnt <= 0) return 0;
+    if (strided) {
+        OZ2_CUDA_TRY(cudaMemsetAsync(amax, 0, sizeof(unsigned long long) * (size_t)cnt, st));
+        int64_t kchunk;
+        int gy = rows_grid_y(cnt, k, &kchunk);
+        dim3 grid((unsigned)((cnt + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
+        if (f32) k1_rows<0, float><<<grid, block, 0, st>>>(cnt, k, static_cast<const float *>(X), ldx, kchunk, amax, nullptr);
+        else k1_rows<0, double><<<grid, block, 0, st>>>(cnt, k, static_cast<const double *>(X), ldx, kchunk, amax, nullptr);
+        k1_rows_E<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(cnt, amax, E);
+        oz2_count_launches(2);
+    } else {
+        if (f32) k1_cols<true, float><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const float *>(X), ldx, nullptr, E);
+        else k1_cols<true, double><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const double *>(X), ldx, nullptr, E);
+        oz2_count_launches(1);
+    }
     OZ2_CUDA_TRY(cudaGetLastError());
-    int rc;
-    if ((rc = oz2_launch_convert(0, 0, 0, f32, m, k, A, lda, EA, Abar, kp, st))) return rc;
-    if ((rc = oz2_launch_convert(1, 0, 0, f32, n, k, B, ldb, EB, Bbar, kp, st))) return rc;
-    return 0;
+    return oz2_launch_convert(strided ? 0 : 1, 0, 0, f32, cnt, k, X, ldx, E, bar, kp, st);
 }
 
 int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA, const int32_t *EB,

@@ -184,6 +184,28 @@ def test_host_buffer_entry_point_column_panels(B, mode, alpha, beta):
     assert np.array_equal(Ch[m:], Cin[m:])
 
 
+@pytest.mark.parametrize("transa,transb", [(0, 0), (1, 0), (0, 1), (1, 1)])
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_transposed_operands(B, transa, transb, mode):
+    # the stored matrices are op(X)^T with padded leading dimensions; the result must be the oracle's on the logical A, B
+    import torch
+    m, n, k, N = 150, 90, 260, 15
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 321)
+    SA = A.T if transa else A                                # stored A: k x m or m x k
+    SB = Bm.T if transb else Bm                              # stored B: n x k or k x n
+    lda, ldb = SA.shape[0] + 3, SB.shape[0] + 5
+    PA = np.zeros((lda, SA.shape[1]), order="F"); PA[:SA.shape[0]] = SA
+    PB = np.zeros((ldb, SB.shape[1]), order="F"); PB[:SB.shape[0]] = SB
+    Ad, Bd = B.colmajor_to_device(PA), B.colmajor_to_device(PB)
+    Cd = torch.full((n, m), float("nan"), dtype=torch.float64, device="cuda")
+    B.ensure_workspace(m, n, k, N, mode)
+    assert B.ozaki2_dgemm_t(transa, transb, m, n, k, 1.0, Ad, lda, Bd, ldb, 0.0, Cd, m, N, mode) == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(B.device_to_colmajor(Cd), O.dgemm(A, Bm, N, mode))
+    assert B.ozaki2_dgemm_t(2, 0, m, n, k, 1.0, Ad, lda, Bd, ldb, 0.0, Cd, m, N, mode) == -1
+    assert B.ozaki2_dgemm_t(transa, transb, m, n, k, 1.0, Ad, SA.shape[0] - 1, Bd, ldb, 0.0, Cd, m, N, mode) == -8
+
+
 # --------------------------------------------------------------------------------------------- primitives
 def test_log2f_exhaustive_equals_oracle(B):
     import torch
