@@ -378,12 +378,24 @@ static int floor_log2_abs(double v)
 /* ------------------------------------------------------------------------------------ */
 /* O2 statistics of one vector v[0..k) with stride `st`                                  */
 /*   E    = floor(log2 max|v_h|)                                                         */
-/*   Sfix = sum_h ceil(2^44 (v_h / 2^E)^2)   (exact integers; reading R2: an order-       */
+/*   Sfix = sum_h ceil(2^SQ (v_h / 2^E)^2)   (exact integers; reading R2: an order-       */
 /*          independent "rounding-up" evaluation of the sum of squares)     */
+/*   SQ = 44 for k <= 2^17 (the range of P:113).  For longer k (blocked products)  */
+/*   the fixed-point position drops by 2 for every factor 4 of k so that Sfix < 2^64:      */
+/*   SQ = 44 - 2 ceil((ceil(log2 k) - 17) / 2)   (reading R2b of DESIGN.md)                */
 /* returns 0 if the vector is all zero                                                   */
 /* ------------------------------------------------------------------------------------ */
+static int sq_shift(long k)
+{
+    int lg = 0;
+    while (((long)1 << lg) < k) lg++;       /* ceil(log2 k) */
+    int extra = lg > 17 ? lg - 17 : 0;
+    return 44 - 2 * ((extra + 1) / 2);
+}
+
 static int vec_stats(const double *v, size_t st, long k, int *E_out, uint64_t *Sfix_out)
 {
+    const int SQ = sq_shift(k);
     double vmax = 0.0;
     for (long h = 0; h < k; h++) {
         double a = fabs(v[(size_t)h * st]);
@@ -397,9 +409,9 @@ static int vec_stats(const double *v, size_t st, long k, int *E_out, uint64_t *S
         if (a == 0.0) continue;
         uint64_t M; int q;
         decompose(a, &M, &q);
-        /* 2^44 (a/2^E)^2 = M^2 * 2^(2(q-E)+44); M^2 < 2^106 */
+        /* 2^SQ (a/2^E)^2 = M^2 * 2^(2(q-E)+SQ); M^2 < 2^106 */
         u128 M2 = (u128)M * M;
-        long sh = 2L * (q - E) + 44;        /* <= -60 because |a| < 2^(E+1) */
+        long sh = 2L * (q - E) + SQ;        /* <= -60 because |a| < 2^(E+1) */
         uint64_t T;
         if (sh >= 0) return -1;             /* cannot happen */
         if (-sh >= 128) T = 1;              /* 0 < value < 1 */
@@ -408,7 +420,7 @@ static int vec_stats(const double *v, size_t st, long k, int *E_out, uint64_t *S
             u128 rem = M2 & ((((u128)1) << (-sh)) - 1);
             T = (uint64_t)fl + (rem != 0);
         }
-        S += T;                             /* <= k * 2^46 <= 2^63 for k <= 2^17 */
+        S += T;                             /* <= k * 2^(SQ+2) <= 2^63 */
     }
     *E_out = E;
     *Sfix_out = S;
@@ -416,13 +428,13 @@ static int vec_stats(const double *v, size_t st, long k, int *E_out, uint64_t *S
 }
 
 /* Alg.1 / Alg.2 on the statistics of one row or column (O3, modes 1 and 2).
- * F = RU_32(Sfix), shat = floor(log2 F) - 44, x = F / 2^floor(log2 F), L = LOG2F(x). */
-static int exponent_fast_or_prop(int mode, const oz_consts *c, int E, uint64_t Sfix)
+ * F = RU_32(Sfix), shat = floor(log2 F) - SQ, x = F / 2^floor(log2 F), L = LOG2F(x). */
+static int exponent_fast_or_prop(int mode, const oz_consts *c, int E, uint64_t Sfix, int SQ)
 {
     float F = f32_from_u64_up(Sfix);
     int fe;
     float fm = frexpf(F, &fe);              /* F = fm 2^fe, fm in [0.5,1) */
-    int shat = (fe - 1) - 44;
+    int shat = (fe - 1) - SQ;
     float x = 2.0f * fm;                    /* in [1,2), exact */
     float L = oz2o_log2f(x);
     if (mode == 2) {
@@ -511,8 +523,8 @@ int oz2o_exponents(int mode, int N, long m, long n, long k,
         Eb[j] = E; Sb[j] = S;
     }
     if (mode == 1 || mode == 2) {
-        for (long i = 0; i < m; i++) e[i] = nzA[i] ? exponent_fast_or_prop(mode, &c, Ea[i], Sa[i]) : 0;
-        for (long j = 0; j < n; j++) f[j] = nzB[j] ? exponent_fast_or_prop(mode, &c, Eb[j], Sb[j]) : 0;
+        for (long i = 0; i < m; i++) e[i] = nzA[i] ? exponent_fast_or_prop(mode, &c, Ea[i], Sa[i], sq_shift(k)) : 0;
+        for (long j = 0; j < n; j++) f[j] = nzB[j] ? exponent_fast_or_prop(mode, &c, Eb[j], Sb[j], sq_shift(k)) : 0;
     } else {
         /* accurate mode: Abar, Bbar, Cbar = Abar Bbar, row/col maxima */
         int8_t *Ab = malloc((size_t)m * (size_t)k + 1), *Bb = malloc((size_t)k * (size_t)n + 1);

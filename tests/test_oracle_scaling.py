@@ -272,3 +272,55 @@ def test_prop_mode_2u32_term_on_boundary_rows():
                 assert int(e[0]) == want
                 hits += 1
     assert hits >= 10
+
+
+# --------------------------------------------------------------------------------------------- k > 2^17
+def _sq_shift(k):
+    lg = max(0, (k - 1).bit_length())
+    extra = max(0, lg - 17)
+    return 44 - 2 * ((extra + 1) // 2)
+
+
+@pytest.mark.parametrize("k", [(1 << 17) + 5, (1 << 18), (1 << 19) + 1])
+def test_long_k_row_statistics_exact_integers(k):
+    # reading R2b: beyond k = 2^17 the fixed-point position of the rounded-up sum drops by 2 per factor 4 of k
+    import math
+    rng = np.random.Generator(np.random.PCG64(k))
+    A = np.asfortranarray(((rng.random((1, k)) - 0.5) * np.exp(rng.standard_normal((1, k)))))
+    Bm = np.asfortranarray(np.ones((k, 1)))
+    _, _, ext = O.exponents(PROP, 14, A, Bm, extras=True)
+    SQ = _sq_shift(k)
+    assert SQ == {131077: 42, 262144: 42, 524289: 40}[k]
+    row = A[0]
+    E = floor_log2(np.max(np.abs(row)))
+    S = 0
+    for x in row.tolist():                      # exact: |x| = M 2^q, term = ceil(M^2 2^(2(q-E)+SQ))
+        mant, ex = math.frexp(abs(x))
+        M, q = int(mant * (1 << 53)), ex - 53
+        r = -(2 * (q - E) + SQ)
+        assert r > 0
+        S += (M * M + (1 << r) - 1) >> r
+    assert int(ext["SA"][0]) == S and S < 2 ** 63
+    assert Fraction(S, 1 << SQ) * pow2(2 * E) >= sum(Fraction(x) ** 2 for x in row[:2000].tolist())
+
+
+@pytest.mark.parametrize("N,t", [(14, 18), (16, 19), (20, 20)])
+def test_long_k_all_ones_closed_form(N, t):
+    # all-ones, k = 2^t: the normalised sum is exactly k, LOG2F(1) = 0, so Algorithm 2 gives
+    # e = floor(single_down(P'_prop - t/2) - 2^-23) whatever the fixed-point position is;
+    # P'_prop - t/2 is exact in FP32 here (same binade or coarser) and its fraction is far from 0 and 2^-23
+    k = 1 << t
+    A, Bm = W.all_ones_scaled(2, 2, k, 1.0)
+    e, f = O.exponents(PROP, N, A, Bm)
+    c = O.constants(N)
+    want = int(np.floor(float(c["Pprop"]) - 0.5 * t - 2.0 ** -23))
+    assert e[0] == want == f[0]
+    assert 2 * k * (1 << (2 * want)) < c["P"]                    # condition (1): k 2^(2e) < P / 2
+
+
+def test_long_k_condition_1_and_recovery_random():
+    k = (1 << 18) + 37
+    A, Bm = W.eq15_matrices(3, 2, k, 1.0, 77)
+    st = O.stages(A, Bm, 16, PROP, want_exact=True)
+    assert st["counts"]["violations"] == 0 and st["counts"]["wrong"] == 0
+    assert np.array_equal(st["Cpp"], st["Z"])
