@@ -37,7 +37,9 @@ extern "C" {
 
 #define OZAKI2_MIN_MODULI 2
 #define OZAKI2_MAX_MODULI 20           /* prefix of eq. (14)                           */
-#define OZAKI2_MAX_K (1 << 17)         /* INT32 accumulator bound                          */
+#define OZAKI2_K_BLOCK (1 << 17)       /* INT32 accumulator bound: longer k is blocked      */
+#define OZAKI2_MAX_K (1 << 22)         /* blocked products up to here (sum of squares in 64 bits)  */
+#define OZAKI2_MAX_K_ACCURATE (1 << 18) /* accurate mode: the auxiliary product 2^12 k fits INT32  */
 
 #define OZAKI2_ERR_WORKSPACE (-100)
 #define OZAKI2_ERR_DEVICE (-101)
@@ -52,7 +54,9 @@ extern "C" {
  *   S5  C = diag(mu)^-1 C'' diag(nu)^-1, then alpha / beta
  * A, B, C: device pointers, 8-byte aligned; C must not overlap A or B.  C is read only if
  * beta != 0.  alpha, beta by value.  Quick returns: m == 0 or n == 0 does nothing; k == 0 or
- * alpha == 0 gives C := beta * C (zeros if beta == 0).  k <= OZAKI2_MAX_K.
+ * alpha == 0 gives C := beta * C (zeros if beta == 0).  k <= OZAKI2_MAX_K (OZAKI2_MAX_K_ACCURATE in
+ * accurate mode); beyond OZAKI2_K_BLOCK the residue products are computed in blocks of 2^17 and summed mod p_l
+ * (P:113).
  * Needs a workspace of ozaki2_workspace_bytes(m, n, k, num_moduli, scaling_mode) bytes
  * registered with ozaki2_set_workspace for the current device.  Asynchronous on `stream`.
  */

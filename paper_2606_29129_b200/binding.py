@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libozaki2.so")
 
 OZAKI2_MODE_ACCURATE, OZAKI2_MODE_FAST, OZAKI2_MODE_PROP = 0, 1, 2
 OZAKI2_ERR_WORKSPACE, OZAKI2_ERR_DEVICE = -100, -101
-OZAKI2_MAX_K = 1 << 17
+OZAKI2_K_BLOCK, OZAKI2_MAX_K, OZAKI2_MAX_K_ACCURATE = 1 << 17, 1 << 22, 1 << 18
 
 _lib = None
 

@@ -246,6 +246,7 @@ int check_args(int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, cons
     if (m < 0) return -1;
     if (n < 0) return -2;
     if (k < 0 || k > OZAKI2_MAX_K) return -3;
+    if (mode == OZAKI2_MODE_ACCURATE && k > OZAKI2_MAX_K_ACCURATE) return -3;
     if (m > 0 && k > 0 && !A) return -5;
     if (lda < (rows_a > 1 ? rows_a : 1)) return -6;
     if (n > 0 && k > 0 && !B) return -7;

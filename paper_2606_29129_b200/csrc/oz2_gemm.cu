@@ -100,7 +100,7 @@ __device__ __forceinline__ TileCoord decode_tile(int64_t t, int tiles_m, int til
 template <bool MAXEPI>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, int nplanes,
-                int mod_base, int m, int n, int num_kb, uint8_t *__restrict__ U, int64_t mp,
+                int mod_base, int m, int n, int kb0, int num_kb, int accum, uint8_t *__restrict__ U, int64_t mp,
                 int32_t *__restrict__ rowmax, int32_t *__restrict__ colmax)
 {
     extern __shared__ uint8_t smem_raw[];
@@ -140,8 +140,8 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                     mbar_wait(empty + stage, phase ^ 1u);
                     uint8_t *sa = smem + stage * STAGE_BYTES, *sb = sa + A_STAGE_BYTES;
                     mbar_expect_tx(full + stage, STAGE_BYTES);
-                    tma_load_3d(&mapA, full + stage, sa, kb * TILE_K, c.m0, c.plane);
-                    tma_load_3d(&mapB, full + stage, sb, kb * TILE_K, c.n0, c.plane);
+                    tma_load_3d(&mapA, full + stage, sa, (kb0 + kb) * TILE_K, c.m0, c.plane);
+                    tma_load_3d(&mapB, full + stage, sb, (kb0 + kb) * TILE_K, c.n0, c.plane);
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
@@ -197,7 +197,14 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                         for (int u = 0; u < 32; u++) {
                             const int j = c.n0 + cc * 32 + u;
                             uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
-                            if (j < n) out[(int64_t)(cc * 32 + u) * mp] = (uint8_t)r;
+                            if (j < n) {
+                                uint8_t *o = out + (int64_t)(cc * 32 + u) * mp;
+                                if (accum) {                   // k blocked at 2^17: add the earlier blocks mod p
+                                    r += *o;
+                                    r = l == 0 ? (r & 0xFFu) : (r >= tb.p ? r - tb.p : r);
+                                }
+                                *o = (uint8_t)r;
+                            }
                         }
                     }
                 }
@@ -515,7 +522,7 @@ int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t 
     if (m <= 0 || n <= 0 || nplanes <= 0) return 0;
     CUtensorMap mapA, mapB;
     const int num_kb = (int)(kp / TILE_K);
-    if (g_gemm_pair && m > TILE_M) {
+    if (g_gemm_pair && m > TILE_M && kp <= (1 << 17)) {
         int rc = make_plane_map(&mapA, RA, kp, m, nplanes, 128);
         if (rc) return rc;
         rc = make_plane_map(&mapB, RB, kp, n, nplanes, 128);
@@ -541,13 +548,21 @@ int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t 
     const int64_t tiles = (int64_t)nplanes * ((m + TILE_M - 1) / TILE_M) * ((n + TILE_N - 1) / TILE_N);
     int grid = num_sms();
     if (tiles < grid) grid = (int)tiles;
-    if (rowmax)
-        k3_residue_gemm<true><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
-                                                                   nullptr, mp, rowmax, colmax);
-    else
-        k3_residue_gemm<false><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
-                                                                    U, mp, nullptr, nullptr);
-    oz2_count_launches(1);
+    if (rowmax) {
+        // accurate mode's auxiliary product: entries <= 64, the API keeps k <= 2^18 so that 2^12 k fits INT32
+        k3_residue_gemm<true><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, 0, num_kb,
+                                                                   0, nullptr, mp, rowmax, colmax);
+        oz2_count_launches(1);
+    } else {
+        // the INT32 accumulator holds k <= 2^17; longer products are blocked and summed mod p_l in the epilogue
+        constexpr int KB_MAX = (1 << 17) / TILE_K;
+        for (int kb0 = 0; kb0 < num_kb; kb0 += KB_MAX) {
+            const int nkb = num_kb - kb0 < KB_MAX ? num_kb - kb0 : KB_MAX;
+            k3_residue_gemm<false><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, kb0, nkb,
+                                                                        kb0 > 0 ? 1 : 0, U, mp, nullptr, nullptr);
+            oz2_count_launches(1);
+        }
+    }
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }

@@ -47,13 +47,13 @@ __device__ __forceinline__ void decompose(unsigned long long b, unsigned long lo
 
 // T = ceil(2^44 (v / 2^E)^2) for |v| < 2^(E+1): exact.  (reading R2)
 // Slow path, any input: exact 128-bit integer square.
-__device__ __noinline__ unsigned long long sq_term_int(unsigned long long b, int E)
+__device__ __noinline__ unsigned long long sq_term_int(unsigned long long b, int E, int SQ)
 {
     unsigned long long M;
     int q;
     decompose(b, M, q);
-    // 2^44 (v/2^E)^2 = M^2 2^-s with s = 2 (E - q) - 44.
-    int s = 2 * (E - q) - 44;
+    // 2^SQ (v/2^E)^2 = M^2 2^-s with s = 2 (E - q) - SQ.
+    int s = 2 * (E - q) - SQ;
     unsigned long long lo = M * M, hi = __umul64hi(M, M);
     if (s <= 0) return lo << (-s);                    // exact, the value is at most 2^46
     if (s < 64) return ((hi << (64 - s)) | (lo >> s)) + ((lo & ((1ull << s) - 1)) ? 1ull : 0ull);
@@ -68,13 +68,15 @@ __device__ __noinline__ unsigned long long sq_term_int(unsigned long long b, int
 // Fast path: x = |v| 2^(22-E) is an exact exponent shift while it stays a normal number (x < 2^23), x^2 < 2^46 has
 // a quantum <= 2^-7 in FP64, so RU(x x) <= ceil(x^2) (integers below 2^53 are representable) and
 // ceil(RU(x x)) = ceil(x^2) exactly: one DMUL.RU and one F2I.CEIL.
-__device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int E)
+// SQ (even; 44 for k <= 2^17, reading R2b beyond) is the fixed-point position of the sum.
+__device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int E, int SQ)
 {
     if (b == 0) return 0;
     const int be = (int)(b >> 52);
-    const int ne = be + 22 - E;                       // biased exponent of x
-    if (be == 0 || ne < 1) return sq_term_int(b, E);  // subnormal input or subnormal x: rare
-    const double x = __longlong_as_double((long long)(b + ((unsigned long long)(long long)(22 - E) << 52)));
+    const int hs = (SQ >> 1) - E;                     // x = |v| 2^hs
+    const int ne = be + hs;                           // biased exponent of x
+    if (be == 0 || ne < 1) return sq_term_int(b, E, SQ);  // subnormal input or subnormal x: rare
+    const double x = __longlong_as_double((long long)(b + ((unsigned long long)(long long)hs << 52)));
     return __double2ull_ru(__dmul_ru(x, x));
 }
 
@@ -82,13 +84,13 @@ __device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int 
 __device__ __forceinline__ float log2f_rn(float x) { return __double2float_rn(log2((double)x)); }
 
 // Algorithm 2 (mode 2) / Algorithm 1 (mode 1) on the statistics (E, S) of one row or column.
-__device__ int exponent_fastprop(int mode, const Oz2CrtTab &c, unsigned long long amax, unsigned long long S)
+__device__ int exponent_fastprop(int mode, const Oz2CrtTab &c, unsigned long long amax, unsigned long long S, int SQ)
 {
     if (amax == 0) return 0;                                            // reading R4
     int E = floor_log2_bits(amax);
     float F = __ull2float_ru(S);                                        // "rounding-up"
     int fb = __float_as_int(F);
-    int shat = ((fb >> 23) - 127) - 44;                                 // floor(log2 F) - 44
+    int shat = ((fb >> 23) - 127) - SQ;                                 // floor(log2 F) - SQ
     float x = __int_as_float((fb & 0x007FFFFF) | 0x3F800000);           // F / 2^floor(log2 F) in [1,2)
     float L = log2f_rn(x);
     if (mode == 2) {
@@ -126,7 +128,7 @@ __device__ int exponent_accurate(const Oz2CrtTab &c, int E, int M)
 template <int PASS, typename T> // PASS 0: max |a|   1: sum of squared, normalised terms;  T: double or float (SGEMM)
 __global__ void __launch_bounds__(ROWS_PER_BLOCK *KSLICES)
 k1_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, int64_t kchunk,
-        unsigned long long *__restrict__ amax, unsigned long long *__restrict__ ssq)
+        unsigned long long *__restrict__ amax, unsigned long long *__restrict__ ssq, int SQ)
 {
     int64_t i = (int64_t)blockIdx.x * ROWS_PER_BLOCK + threadIdx.x;
     int64_t h0 = (int64_t)blockIdx.y * kchunk;
@@ -149,23 +151,23 @@ k1_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, int64_t kchu
         for (int u = 0; u < 8; u++) {
             unsigned long long b = abs_bits(v[u]);
             if (PASS == 0) acc = b > acc ? b : acc;
-            else acc += sq_term(b, E);
+            else acc += sq_term(b, E, SQ);
         }
     }
     for (; h < h1; h += KSLICES) {
         unsigned long long b = abs_bits((double)__ldg(p + h * lda));
         if (PASS == 0) acc = b > acc ? b : acc;
-        else acc += sq_term(b, E);
+        else acc += sq_term(b, E, SQ);
     }
     if (PASS == 0) { if (acc) atomicMax(amax + i, acc); }
     else if (acc) atomicAdd(ssq + i, acc);
 }
 
 __global__ void k1_rows_finalize(int mode, int N, int64_t m, const unsigned long long *__restrict__ amax,
-                                 const unsigned long long *__restrict__ ssq, int32_t *__restrict__ e)
+                                 const unsigned long long *__restrict__ ssq, int32_t *__restrict__ e, int SQ)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < m) e[i] = exponent_fastprop(mode, c_crt[N], amax[i], ssq[i]);
+    if (i < m) e[i] = exponent_fastprop(mode, c_crt[N], amax[i], ssq[i], SQ);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -199,7 +201,7 @@ __device__ __forceinline__ double2 ld2(const float *p)
 template <bool ACCU, typename T>
 __global__ void __launch_bounds__(COL_THREADS)
 k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_t *__restrict__ f,
-        int32_t *__restrict__ EB)
+        int32_t *__restrict__ EB, int SQ)
 {
     __shared__ unsigned long long sm[COL_THREADS / 32];
     const T *col = B + (int64_t)blockIdx.x * ldb;
@@ -229,11 +231,11 @@ k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_
     unsigned long long acc = 0;
     for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {      // second read: L2 hits
         double2 v = ld2(col + h);
-        acc += sq_term(abs_bits(v.x), E) + sq_term(abs_bits(v.y), E);
+        acc += sq_term(abs_bits(v.x), E, SQ) + sq_term(abs_bits(v.y), E, SQ);
     }
-    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits((double)__ldg(col + h)), E);
+    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits((double)__ldg(col + h)), E, SQ);
     acc = block_reduce(acc, false, sm);
-    if (threadIdx.x == 0) f[blockIdx.x] = exponent_fastprop(mode, c_crt[N], mx, acc);
+    if (threadIdx.x == 0) f[blockIdx.x] = exponent_fastprop(mode, c_crt[N], mx, acc, SQ);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -258,6 +260,15 @@ __global__ void k_log2f(const float *__restrict__ x, float *__restrict__ y, int6
 {
     int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t < count) y[t] = log2f_rn(x[t]);
+}
+
+// fixed-point position of the rounded-up sum of squares (reading R2 / R2b)
+int sq_shift(int64_t k)
+{
+    int lg = 0;
+    while (((int64_t)1 << lg) < k) lg++;
+    const int extra = lg > 17 ? lg - 17 : 0;
+    return 44 - 2 * ((extra + 1) / 2);
 }
 
 int rows_grid_y(int64_t m, int64_t k, int64_t *kchunk)
@@ -294,13 +305,13 @@ int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const 
     int gy = rows_grid_y(m, k, &kchunk);
     dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
     if (f32) {
-        k1_rows<0, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA);
-        k1_rows<1, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA);
+        k1_rows<0, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA, sq_shift(k));
+        k1_rows<1, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA, sq_shift(k));
     } else {
-        k1_rows<0, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
-        k1_rows<1, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA);
+        k1_rows<0, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA, sq_shift(k));
+        k1_rows<1, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA, sq_shift(k));
     }
-    k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e);
+    k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e, sq_shift(k));
     oz2_count_launches(3);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
@@ -309,8 +320,8 @@ int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const 
 int oz2_launch_scale_cols(int mode, int N, int f32, int64_t n, int64_t k, const void *B, int64_t ldb, int32_t *f, cudaStream_t st)
 {
     if (n <= 0) return 0;
-    if (f32) k1_cols<false, float><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const float *>(B), ldb, f, nullptr);
-    else k1_cols<false, double><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const double *>(B), ldb, f, nullptr);
+    if (f32) k1_cols<false, float><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const float *>(B), ldb, f, nullptr, sq_shift(k));
+    else k1_cols<false, double><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const double *>(B), ldb, f, nullptr, sq_shift(k));
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
@@ -328,13 +339,13 @@ int oz2_launch_scale_accu_side(int f32, int strided, int64_t cnt, int64_t k, con
         int64_t kchunk;
         int gy = rows_grid_y(cnt, k, &kchunk);
         dim3 grid((unsigned)((cnt + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
-        if (f32) k1_rows<0, float><<<grid, block, 0, st>>>(cnt, k, static_cast<const float *>(X), ldx, kchunk, amax, nullptr);
-        else k1_rows<0, double><<<grid, block, 0, st>>>(cnt, k, static_cast<const double *>(X), ldx, kchunk, amax, nullptr);
+        if (f32) k1_rows<0, float><<<grid, block, 0, st>>>(cnt, k, static_cast<const float *>(X), ldx, kchunk, amax, nullptr, 44);
+        else k1_rows<0, double><<<grid, block, 0, st>>>(cnt, k, static_cast<const double *>(X), ldx, kchunk, amax, nullptr, 44);
         k1_rows_E<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(cnt, amax, E);
         oz2_count_launches(2);
     } else {
-        if (f32) k1_cols<true, float><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const float *>(X), ldx, nullptr, E);
-        else k1_cols<true, double><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const double *>(X), ldx, nullptr, E);
+        if (f32) k1_cols<true, float><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const float *>(X), ldx, nullptr, E, 44);
+        else k1_cols<true, double><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const double *>(X), ldx, nullptr, E, 44);
         oz2_count_launches(1);
     }
     OZ2_CUDA_TRY(cudaGetLastError());

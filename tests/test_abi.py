@@ -53,7 +53,8 @@ def test_argument_checks_xerbla_numbering(B):
     assert call(m=-1) == -1
     assert call(n=-1) == -2
     assert call(k=-1) == -3
-    assert call(k=(1 << 17) + 1) == -3            # INT32 accumulator bound
+    assert call(k=(1 << 22) + 1) == -3            # OZAKI2_MAX_K (blocked beyond 2^17)
+    assert call(k=(1 << 18) + 1, scaling_mode=0) == -3   # accurate mode: auxiliary product must fit INT32
     assert call(A=None) == -5
     assert call(lda=7) == -6
     assert call(B=None) == -7
@@ -75,7 +76,7 @@ def test_workspace_size_formula(B):
     assert 16 * (m * k + k * n) + 16 * m * n <= w <= 16 * (m * k + k * n) + 16 * m * n + (1 << 20)
     wa = B.ozaki2_workspace_bytes(m, n, k, 16, 0)
     assert wa - w >= m * k + k * n
-    assert B.ozaki2_workspace_bytes(m, n, (1 << 17) + 1, 16, 2) == 0
+    assert B.ozaki2_workspace_bytes(m, n, (1 << 22) + 1, 16, 2) == 0
     assert B.ozaki2_workspace_bytes(m, n, k, 21, 2) == 0
     assert B.ozaki2_host_scratch_bytes(4, 5, 6) >= 8 * (24 + 30 + 20)
 

@@ -73,7 +73,8 @@ def test_config0_128_all_stages(B, mode):
     (200, 77, 333, 14, 2), (1, 1, 1, 2, 2), (129, 257, 127, 9, 1), (37, 300, 1000, 16, 0), (130, 40, 129, 17, 2),
     (64, 513, 260, 20, 0), (255, 255, 4097, 20, 2), (16, 16, 16, 3, 1), (300, 5, 31, 15, 0), (5, 300, 2049, 8, 2),
     (260, 260, 100, 12, 2), (128, 256, 128, 4, 2), (131, 100, 777, 5, 0), (100, 131, 64, 18, 1), (77, 77, 77, 13, 2),
-    (33, 65, 640, 6, 2), (90, 70, 50, 7, 1), (48, 40, 131072, 14, 2), (40, 24, 131072, 20, 0), (70, 90, 150, 10, 0), (50, 60, 70, 11, 2), (61, 67, 71, 19, 0),
+    (33, 65, 640, 6, 2), (90, 70, 50, 7, 1), (48, 40, 131072, 14, 2), (40, 24, 131072, 20, 0),
+    (40, 24, (1 << 18) + 384, 14, 2), (24, 40, (1 << 18) + 129, 16, 1), (130, 20, 1 << 18, 15, 0), (70, 90, 150, 10, 0), (50, 60, 70, 11, 2), (61, 67, 71, 19, 0),
 ])
 def test_ragged_shapes_and_every_moduli_count(B, m, n, k, N, mode):
     A, Bm = W.eq15_matrices(m, n, k, 1.0, 1000 + m + n + k + N)
@@ -249,6 +250,26 @@ def test_residue_gemm_tensor_core_vs_oracle_and_check_kernel(B, m, n, k, N):
         assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, tc) == 0
         torch.cuda.synchronize()
         assert np.array_equal(Ud.cpu().numpy(), want), f"tensor_cores={tc}"
+
+
+def test_k_blocked_residue_gemm_beyond_2pow17(B):
+    # k > 2^17 is computed in blocks of 2^17 whose residues are added mod p_l in the epilogue; worst-case
+    # operands (-128 x -128 for p = 256, 127 x 127 for 255) over 2 1/2 blocks
+    import torch
+    m, n, k, N = 128, 256, (1 << 18) + (1 << 16), 3
+    rng = np.random.Generator(np.random.PCG64(11))
+    RA = np.zeros((N, m, k), np.int8); RB = np.zeros((N, n, k), np.int8)
+    RA[0] = -128; RB[0] = -128
+    RA[1] = 127; RB[1] = 127
+    RA[2, :8] = rng.integers(-126, 127, size=(8, k)); RB[2, :8] = rng.integers(-126, 127, size=(8, k))
+    want, _ = O.products(N, RA[:, :8], RB[:, :8])
+    RAd, RBd = torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda()
+    Ud = torch.zeros((N, n, m), dtype=torch.uint8, device="cuda")
+    assert B.ozaki2_debug_residue_gemm(N, m, n, k, RAd, RBd, Ud, 1) == 0
+    torch.cuda.synchronize()
+    got = Ud.cpu().numpy()
+    assert np.array_equal(got[:, :8, :8], want)
+    assert np.all(got[0] == (128 * 128 * k) % 256) and np.all(got[1] == (127 * 127 * k) % 255)
 
 
 def test_int32_accumulator_wraps_at_k_2pow17(B):
