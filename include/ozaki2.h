@@ -92,7 +92,9 @@ size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, i
 /*
  * Register a caller-owned device buffer (256-byte aligned) as the workspace of the current
  * device; it must stay valid until replaced.  (NULL, 0) unregisters.  Not stream ordered: do
- * not replace it while calls that use it are in flight.
+ * not replace it while calls that use it are in flight.  All calls on a device share this one
+ * workspace, so concurrent calls must be ordered with respect to each other (same stream, or
+ * events); calls on different devices are independent.
  */
 int ozaki2_set_workspace(void *device_ptr, size_t bytes);
 

@@ -207,6 +207,24 @@ def test_transposed_operands(B, transa, transb, mode):
     assert B.ozaki2_dgemm_t(transa, transb, m, n, k, 1.0, Ad, SA.shape[0] - 1, Bd, ldb, 0.0, Cd, m, N, mode) == -8
 
 
+@pytest.mark.parametrize("mode", [1, 2])
+def test_non_finite_inputs_stay_in_their_row_and_column(B, mode):
+    # include/ozaki2.h: Inf / NaN are not detected; they may spoil their own row of A / column of B only (in the
+    # fast modes e_i, f_j and the residues are row / column local) and never hang or fault
+    import torch
+    m, n, k, N = 96, 80, 300, 14
+    A, Bm = W.eq15_matrices(m, n, k, 0.5, 42)
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    clean = B.device_to_colmajor(B.dgemm(Ad, Bd, N, mode))
+    A2, B2 = A.copy(order="F"), Bm.copy(order="F")
+    A2[3, 7] = np.nan; A2[10, 0] = np.inf; B2[5, 9] = -np.inf; B2[100, 33] = np.nan
+    dirty = B.device_to_colmajor(B.dgemm(B.colmajor_to_device(A2), B.colmajor_to_device(B2), N, mode))
+    torch.cuda.synchronize()
+    rows = np.ones(m, bool); rows[[3, 10]] = False
+    cols = np.ones(n, bool); cols[[9, 33]] = False
+    assert np.array_equal(dirty[np.ix_(rows, cols)], clean[np.ix_(rows, cols)])
+
+
 # --------------------------------------------------------------------------------------------- primitives
 def test_log2f_exhaustive_equals_oracle(B):
     import torch
