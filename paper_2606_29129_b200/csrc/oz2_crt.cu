@@ -53,10 +53,11 @@ __device__ __noinline__ double round_scaled_slow(unsigned long long mant, uint32
 }
 
 // C'' = rmod(C', P), RN_64(C'') 2^-esum from the words c[0..NW] of C' = sum_l w_l U_l (c[NW] < 2^13)
-// TO = double: RN_64; TO = float: RN_32 of the same exact integer (SGEMM variant)
+// TO = double: RN_64; TO = float: RN_32 of the same exact integer (SGEMM variant).
+// crt_exact handles every case (near-half quotients, subnormal / overflowing results, the C'' words for the parity
+// surface); crt_fast below is its branch-free common case and says when it does not apply.
 template <int NW, typename TO>
-__device__ __forceinline__ TO crt_from_words(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum,
-                                             uint64_t *cpp_out)
+__device__ __noinline__ TO crt_exact(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum, uint64_t *cpp_out)
 {
     // ---- Q = round(C' / P), estimated from the top three words
     double top = (double)(long long)(((unsigned long long)c[NW] << 32) | c[NW - 1]);
@@ -153,6 +154,57 @@ __device__ __forceinline__ TO crt_from_words(const uint32_t (&c)[NW + 1], const 
     }
 }
 
+// The common case of crt_exact without a branch: the quotient estimate is away from a half-integer and the result
+// is a normal number.  `rare` is set when that does not hold (the caller then takes crt_exact).
+template <int NW, typename TO>
+__device__ __forceinline__ TO crt_fast(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum, bool &rare)
+{
+    double top = (double)(long long)(((unsigned long long)c[NW] << 32) | c[NW - 1]);
+    if constexpr (NW >= 2) top = fma((double)c[NW - 2], 2.3283064365386963e-10, top);
+    const double qd = top * T.invP;
+    const double qr = floor(qd + 0.5);
+    const uint32_t Q = (uint32_t)(int)qr;
+    rare = fabs(qd - qr) > 0.5 - 9.5367431640625e-07;
+    uint32_t r[NW + 1];
+    long long br = 0;
+#pragma unroll
+    for (int t = 0; t <= NW; t++) {
+        long long s = (long long)c[t] + br - (long long)((unsigned long long)Q * (t < NW ? T.P[t] : 0u));
+        r[t] = (uint32_t)s;
+        br = s >> 32;
+    }
+    const uint32_t negm = (uint32_t)((int32_t)r[NW] >> 31);
+    const unsigned long long m64 = (unsigned long long)(long long)(int32_t)negm;
+    auto W = [&](int t) -> uint32_t { return t <= NW ? r[t <= NW ? t : 0] : negm; };
+    const unsigned long long R0 = ((unsigned long long)W(1) << 32) | W(0);
+    const unsigned long long R1 = ((unsigned long long)W(3) << 32) | W(2);
+    const unsigned long long R2 = ((unsigned long long)W(5) << 32) | W(4);
+    const unsigned long long X0 = (R0 ^ m64) + (m64 & 1ull);
+    const unsigned long long c0 = (m64 & 1ull) & (unsigned long long)(X0 == 0ull);
+    const unsigned long long X1 = (R1 ^ m64) + c0;
+    const unsigned long long c1 = c0 & (unsigned long long)(X1 == 0ull);
+    const unsigned long long X2 = (R2 ^ m64) + c1;
+    const bool use2 = NW >= 5 && X2 != 0ull, use1 = !use2 && NW >= 3 && X1 != 0ull;
+    const unsigned long long ptop = use2 ? X2 : (use1 ? X1 : X0), pmid = use2 ? X1 : (use1 ? X0 : 0ull), plow = use2 ? X0 : 0ull;
+    const int base = use2 ? 128 : (use1 ? 64 : 0);
+    const bool zero = ptop == 0ull;
+    const int lz = __clzll((long long)(ptop | (unsigned long long)zero));
+    const unsigned long long mant = (ptop << lz) | ((pmid >> 1) >> (63 - lz));
+    const uint32_t sticky = (((pmid << lz) | plow) != 0ull) ? 1u : 0u;
+    const int pos = base + 63 - lz, sc = pos - 63 - esum, Ex = pos - esum;
+    if constexpr (sizeof(TO) == 8) {
+        rare |= !zero && (Ex < -1020 || Ex > 1021);
+        const double d = __ull2double_rn(mant | sticky);
+        const long long bits = (__double_as_longlong(d) + ((long long)sc << 52)) | (long long)(m64 << 63);
+        return __longlong_as_double(zero ? 0ll : bits);
+    } else {
+        rare |= !zero && (Ex < -124 || Ex > 125);
+        const float d = __ull2float_rn(mant | sticky);
+        const int bits = (__float_as_int(d) + sc * 8388608) | (int)(negm & 0x80000000u);
+        return __int_as_float(zero ? 0 : bits);
+    }
+}
+
 // =============================================================================================
 // Tensor-core CRT.  sum_l w_l U_l is itself a small dense contraction: with the weights cut into bytes,
 //     S[i][t] = sum_l U_l[i] * byte_t(w_l),   t = 0 .. 4 NW - 1,      C'[i] = sum_t S[i][t] 256^t,
@@ -184,13 +236,10 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
         : "memory");
 }
 
-// fold the byte slices S[0 .. 4 NW) of one element into C' and finish (C'' -> C -> alpha / beta -> store)
-template <int NW, bool WANT_CPP, typename TO>
-__device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T, int64_t i, int64_t j, int64_t m, int esum,
-                                          TO alpha, TO beta, TO *__restrict__ C, int64_t ldc,
-                                          uint64_t *__restrict__ Cpp)
+// fold the byte slices S[0 .. 4 NW) of one element into the words of C'
+template <int NW>
+__device__ __forceinline__ void k5_fold(const uint32_t *S, uint32_t (&c)[NW + 1])
 {
-    uint32_t c[NW + 1];
     unsigned long long carry = 0;
 #pragma unroll
     for (int k = 0; k < NW; k++) {       // V_k = sum_{b<4} S[4k+b] 256^b (< 2^46), then carries
@@ -200,9 +249,11 @@ __device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T,
         carry = v >> 32;
     }
     c[NW] = (uint32_t)carry;
-    uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr;
-    const TO cij = crt_from_words<NW, TO>(c, T, esum, cpp);
-    TO *dst = C + i + j * ldc;
+}
+
+template <typename TO>
+__device__ __forceinline__ void k5_store(TO cij, TO alpha, TO beta, TO *dst)
+{
     if constexpr (sizeof(TO) == 8) {
         const double tt = alpha * cij;
         *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
@@ -210,6 +261,27 @@ __device__ __forceinline__ void k5_finish(const uint32_t *S, const Oz2CrtTab &T,
         const float tt = __fmul_rn(alpha, cij);
         *dst = (beta == 0.0f) ? tt : __fmaf_rn(beta, *dst, tt);
     }
+}
+
+// the two elements (i, j) and (i + 128, j) of one thread: C'' -> C -> alpha / beta -> store.  Both go through the
+// branch-free crt_fast side by side (two independent dependency chains per thread); crt_exact is the rare path.
+template <int NW, bool WANT_CPP, typename TO>
+__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, const Oz2CrtTab &T, int64_t i, int64_t j,
+                                           int64_t m, int esum_a, int esum_b, TO alpha, TO beta, TO *__restrict__ C,
+                                           int64_t ldc, uint64_t *__restrict__ Cpp)
+{
+    const bool ok_a = i < m, ok_b = i + 128 < m;
+    uint32_t ca[NW + 1], cb[NW + 1];
+    k5_fold<NW>(Sa, ca);
+    k5_fold<NW>(Sb, cb);
+    bool rare_a, rare_b;
+    TO va = crt_fast<NW, TO>(ca, T, esum_a, rare_a);
+    TO vb = crt_fast<NW, TO>(cb, T, esum_b, rare_b);
+    if ((WANT_CPP || rare_a) && ok_a) va = crt_exact<NW, TO>(ca, T, esum_a, WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr);
+    if ((WANT_CPP || rare_b) && ok_b) vb = crt_exact<NW, TO>(cb, T, esum_b, WANT_CPP ? Cpp + ((size_t)j * m + i + 128) * 4 : nullptr);
+    TO *dst = C + i + j * ldc;
+    if (ok_a) k5_store<TO>(va, alpha, beta, dst);
+    if (ok_b) k5_store<TO>(vb, alpha, beta, dst + 128);
 }
 
 template <int NW, bool WANT_CPP, typename TO>
@@ -330,8 +402,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
             if (lane == 0) mbar_arrive_a(tempty + 8 * b);
             b += 2;
             if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
-            if (i < m) k5_finish<NW, WANT_CPP, TO>(S, T, i, jcur, m, e0 + fj, alpha, beta, C, ldc, Cpp);
-            if (i + 128 < m) k5_finish<NW, WANT_CPP, TO>(S + NS, T, i + 128, jcur, m, e1 + fj, alpha, beta, C, ldc, Cpp);
+            if (i < m) k5_finish2<NW, WANT_CPP, TO>(S, S + NS, T, i, jcur, m, e0 + fj, e1 + fj, alpha, beta, C, ldc, Cpp);
         }
     }
     __syncthreads();
