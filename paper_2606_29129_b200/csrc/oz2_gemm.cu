@@ -8,7 +8,7 @@
 //     SWIZZLE_128B shared-memory tiles (A 128 x 128 B, B 256 x 128 B per stage),
 //   * math: tcgen05.mma.cta_group::1.kind::i8, M = 128, N = 256, K = 32 per instruction, issued by one thread;
 //     INT32 accumulators live in tensor memory (2 x 256 columns, double buffered), they never touch HBM,
-//   * epilogue: 4 warps read the accumulator with tcgen05.ld, reduce mod p_l and write one byte per element,
+//   * epilogue: 8 warps (two per TMEM lane quarter) read the accumulator with tcgen05.ld, reduce mod p_l and write one byte per element,
 //     overlapping the MMAs of the next tile,
 //   * persistent grid (one CTA per SM), static tile order: modulus-major, then groups of 32 M-tiles so that the
 //     148 tiles in flight share A / B panels in L2.
@@ -29,7 +29,8 @@ constexpr int A_STAGE_BYTES = TILE_M * TILE_K;    // 16 KB
 constexpr int B_STAGE_BYTES = TILE_N * TILE_K;    // 32 KB
 constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
-constexpr int NUM_THREADS = 192;                  // warp 0: TMA, warp 1: MMA + TMEM alloc, warps 2..5: epilogue
+constexpr int EPI_SPLIT = 4;                       // epilogue warps per TMEM lane quarter (256 / EPI_SPLIT columns each)
+constexpr int NUM_THREADS = 64 + 128 * EPI_SPLIT;  // warp 0: TMA, warp 1: MMA + TMEM alloc, then the epilogue warps
 constexpr int GROUP_M = 32;
 
 // tcgen05 instruction descriptor (kind::i8): D = S32, A = B = signed 8 bit, both K-major, N = 256, M = 128
@@ -115,7 +116,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; s++) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int s = 0; s < 2; s++) { mbar_init(tfull + s, 1); mbar_init(tempty + s, 4); }
+        for (int s = 0; s < 2; s++) { mbar_init(tfull + s, 1); mbar_init(tempty + s, 4 * EPI_SPLIT); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapB) : "memory");
@@ -174,8 +175,9 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             }
         }
     } else {
-        // ===================== epilogue: warps 2..5, TMEM lane quarter = warp % 4 =====================
-        const int q = warp & 3;
+        // ===================== epilogue: warps 2..9, TMEM lane quarter = warp % 4, column half = (warp - 2) / 4 =====================
+        const int q = warp & 3;                                // TMEM lane quarter
+        const int half = (warp - 2) >> 2;                      // column slice of the tile
         int as = 0;
         uint32_t aphase = 0;
         for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
@@ -189,7 +191,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
                 const Oz2ModTab tb = c_mod[l];
                 uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
 #pragma unroll 1
-                for (int cc = 0; cc < TILE_N / 32; cc++) {
+                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
                     uint32_t v[32];
                     tc_ld32(taddr + (uint32_t)(cc * 32), v);
                     if (i < m) {
@@ -211,7 +213,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             } else {
                 int rmax = 0;
 #pragma unroll 1
-                for (int cc = 0; cc < TILE_N / 32; cc++) {
+                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
                     uint32_t v[32];
                     tc_ld32(taddr + (uint32_t)(cc * 32), v);
 #pragma unroll
@@ -325,7 +327,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
         }
         for (int b = 0; b < 2; b++) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(tfull + 8 * b));
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 8;" ::"r"(tempty + 8 * b));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tempty + 8 * b), "n"(8 * EPI_SPLIT));
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapA) : "memory");
@@ -387,8 +389,9 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
             }
         }
     } else {
-        // ===================== epilogue: warps 2..5 of both CTAs, rows m0 + 128 rank + 32 q + lane =====================
-        const int q = warp & 3;
+        // ===================== epilogue: warps 2..9 of both CTAs, rows m0 + 128 rank + 32 q + lane =====================
+        const int q = warp & 3;                                // TMEM lane quarter
+        const int half = (warp - 2) >> 2;                      // column slice of the tile
         int as = 0;
         uint32_t aphase = 0;
         const uint32_t leader_tempty = tempty & PEER_MASK;
@@ -403,7 +406,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
                 const Oz2ModTab tb = c_mod[l];
                 uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
 #pragma unroll 1
-                for (int cc = 0; cc < TILE_N / 32; cc++) {
+                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
                     uint32_t v[32];
                     tc_ld32(taddr + (uint32_t)(cc * 32), v);
                     if (i < m) {
@@ -418,7 +421,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
             } else {
                 int rmax = 0;
 #pragma unroll 1
-                for (int cc = 0; cc < TILE_N / 32; cc++) {
+                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
                     uint32_t v[32];
                     tc_ld32(taddr + (uint32_t)(cc * 32), v);
 #pragma unroll
