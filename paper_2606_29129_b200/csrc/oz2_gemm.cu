@@ -189,23 +189,64 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             if (!MAXEPI) {
                 const int l = mod_base + c.plane;
                 const Oz2ModTab tb = c_mod[l];
-                uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
+                if (!accum) {
+                    // Packed path.  A thread holds 32 columns of ITS row; the bytes are packed four columns to a word and
+                    // 4 x 4 byte blocks are transposed inside each lane quad (two shuffles + two byte permutes per word),
+                    // after which lane 4g + t holds rows 4g .. 4g+3 of the columns = t (mod 4): 4-byte stores, a quarter
+                    // of the store instructions and no per-element address arithmetic.
+                    const int t4 = lane & 3, row4 = c.m0 + q * 32 + (lane & ~3);
+                    const uint32_t selA = (t4 & 1) ? 0x3715u : 0x6240u, selB = (t4 & 2) ? 0x3276u : 0x5410u;
 #pragma unroll 1
-                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
-                    uint32_t v[32];
-                    tc_ld32(taddr + (uint32_t)(cc * 32), v);
-                    if (i < m) {
+                    for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
+                        uint32_t v[32];
+                        tc_ld32(taddr + (uint32_t)(cc * 32), v);
+                        uint32_t W[8];
+                        if (l == 0) {
 #pragma unroll
-                        for (int u = 0; u < 32; u++) {
-                            const int j = c.n0 + cc * 32 + u;
-                            uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
-                            if (j < n) {
-                                uint8_t *o = out + (int64_t)(cc * 32 + u) * mp;
-                                if (accum) {                   // k blocked at 2^17: add the earlier blocks mod p
+                            for (int w = 0; w < 8; w++)
+                                W[w] = __byte_perm(__byte_perm(v[4 * w], v[4 * w + 1], 0x0040), __byte_perm(v[4 * w + 2], v[4 * w + 3], 0x0040), 0x5410);
+                        } else {
+#pragma unroll
+                            for (int w = 0; w < 8; w++) {
+                                const uint32_t r0 = mod_p_i32((int32_t)v[4 * w], tb), r1 = mod_p_i32((int32_t)v[4 * w + 1], tb);
+                                const uint32_t r2 = mod_p_i32((int32_t)v[4 * w + 2], tb), r3 = mod_p_i32((int32_t)v[4 * w + 3], tb);
+                                W[w] = __byte_perm(__byte_perm(r0, r1, 0x0040), __byte_perm(r2, r3, 0x0040), 0x5410);
+                            }
+                        }
+#pragma unroll
+                        for (int w = 0; w < 8; w++) {
+                            uint32_t y = __shfl_xor_sync(0xffffffffu, W[w], 1);
+                            W[w] = __byte_perm(W[w], y, selA);
+                            y = __shfl_xor_sync(0xffffffffu, W[w], 2);
+                            W[w] = __byte_perm(W[w], y, selB);
+                        }
+                        const int col0 = c.n0 + cc * 32 + t4;
+                        if (row4 < mp) {                       // rows m .. mp-1 are pitch padding: written, never read back
+                            uint8_t *o = U + ((int64_t)c.plane * n + col0) * mp + row4;
+#pragma unroll
+                            for (int w = 0; w < 8; w++) {
+                                if (col0 + 4 * w < n) *reinterpret_cast<uint32_t *>(o) = W[w];
+                                o += 4 * mp;
+                            }
+                        }
+                    }
+                } else {
+                    // k blocked at 2^17: add the residues of the earlier blocks mod p, element by element
+                    uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
+#pragma unroll 1
+                    for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
+                        uint32_t v[32];
+                        tc_ld32(taddr + (uint32_t)(cc * 32), v);
+                        if (i < m) {
+#pragma unroll
+                            for (int u = 0; u < 32; u++) {
+                                const int j = c.n0 + cc * 32 + u;
+                                uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
+                                if (j < n) {
+                                    uint8_t *o = out + (int64_t)(cc * 32 + u) * mp;
                                     r += *o;
-                                    r = l == 0 ? (r & 0xFFu) : (r >= tb.p ? r - tb.p : r);
+                                    *o = (uint8_t)(l == 0 ? (r & 0xFFu) : (r >= tb.p ? r - tb.p : r));
                                 }
-                                *o = (uint8_t)r;
                             }
                         }
                     }
