@@ -118,7 +118,7 @@ class ClockSampler:
 def profiled_traffic(m, N, mode):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), only for
     the workload that capture was taken on; None otherwise."""
-    path = os.path.join(ROOT, "profiles", "r01b_dram_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r01c_dram_traffic.json")
     if not (os.path.exists(path) and m == 8192 and N == 16 and mode == 2):
         return None
     with open(path) as fh:
@@ -273,7 +273,7 @@ def main():
                     peak_source=f"2 x bf16_tflops_sustained ({peaks['source']}); INT8 has no measured entry",
                     frac_of_burst=achieved / (INT8_OVER_BF16 * peaks["bf16"]),
                     frac_of_nominal_4500=achieved / NOMINAL_INT8_TOPS, ms_per_launch=s3_ms,
-                    traffic=profiled_traffic(m, N, mode), traffic_unit="bytes per launch (ncu dram read + write, profiles/r01b)",
+                    traffic=profiled_traffic(m, N, mode), traffic_unit="bytes per launch (ncu dram read + write, profiles/r01c)",
                     algorithmic_bytes=N * X + N * Y)
     stage_bytes = [esz * X if mode != 0 else esz * X + 2 * X, (esz + N) * X, N * X + N * Y, (N + esz) * Y]
     stages = {}
