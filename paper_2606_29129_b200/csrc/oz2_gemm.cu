@@ -182,7 +182,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
         uint32_t aphase = 0;
         for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
             const TileCoord c = decode_tile(t, tiles_m, tiles_n);
-            mbar_wait(tfull + as, aphase);
+            mbar_wait_idle(smem_u32(tfull + as), aphase);
             tc_fence_after();
             const int i = c.m0 + q * 32 + lane;                // output row of this thread
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TILE_N);

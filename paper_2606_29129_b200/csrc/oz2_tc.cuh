@@ -75,6 +75,23 @@ __device__ __forceinline__ void mbar_wait_a(uint32_t addr, uint32_t parity)
         if (++spins > SPIN_LIMIT) __trap();
     }
 }
+// wait of a warp that is expected to idle for a long time (an epilogue warp waiting for the next accumulator):
+// sleep between polls so that the idle warps do not burn issue slots (and power) next to the MMA warp
+__device__ __forceinline__ void mbar_wait_idle(uint32_t addr, uint32_t parity)
+{
+    uint32_t done = 0, spins = 0;
+    while (true) {
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(addr), "r"(parity)
+                     : "memory");
+        if (done) break;
+        __nanosleep(200);
+        if (++spins > SPIN_LIMIT) __trap();
+    }
+}
 __device__ __forceinline__ void mbar_arrive_a(uint32_t addr)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
