@@ -118,12 +118,14 @@ class ClockSampler:
 def profiled_traffic(m, N, mode):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), only for
     the workload that capture was taken on; None otherwise."""
-    path = os.path.join(ROOT, "profiles", "r01c_dram_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r01c_dram_traffic.csv")
     if not (os.path.exists(path) and m == 8192 and N == 16 and mode == 2):
         return None
     with open(path) as fh:
-        d = json.load(fh)
-    return d["bytes_per_launch"].get("k3_residue_gemm<0>")
+        for line in fh:
+            if line.startswith('"k3_residue_gemm<0>"'):
+                return float(line.rsplit(",", 1)[1])
+    return None
 
 
 def cpu_slab_shape(m, n, k):
