@@ -58,7 +58,9 @@ extern "C" {
  * accurate mode); beyond OZAKI2_K_BLOCK the residue products are computed in blocks of 2^17 and summed mod p_l
  * (P:113).
  * Needs a workspace of ozaki2_workspace_bytes(m, n, k, num_moduli, scaling_mode) bytes
- * registered with ozaki2_set_workspace for the current device.  Asynchronous on `stream`.
+ * registered with ozaki2_set_workspace for the current device.  Asynchronous on `stream`.  After the first call
+ * on a device (which uploads the constant tables) the call only enqueues kernels and memsets on `stream` and can
+ * be captured into a CUDA graph.
  */
 int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
                  const double *B, int64_t ldb, double beta, double *C, int64_t ldc,

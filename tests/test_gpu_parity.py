@@ -225,6 +225,32 @@ def test_non_finite_inputs_stay_in_their_row_and_column(B, mode):
     assert np.array_equal(dirty[np.ix_(rows, cols)], clean[np.ix_(rows, cols)])
 
 
+def test_call_is_cuda_graph_capturable(B):
+    # "CUDA streams and graphs": after the first call on a device (which uploads the constant tables) the path only
+    # enqueues kernels and memsets on the caller's stream, so it can be captured and replayed
+    import torch
+    m, n, k, N = 256, 192, 320, 14
+    A, Bm = W.eq15_matrices(m, n, k, 0.5, 12)
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    Cd = torch.empty((n, m), dtype=torch.float64, device="cuda")
+    B.ensure_workspace(m, n, k, N, 2)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        assert B.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == 0
+    torch.cuda.synchronize()
+    want = O.dgemm(A, Bm, N, 2)
+    assert np.array_equal(B.device_to_colmajor(Cd), want)
+    g = torch.cuda.CUDAGraph()
+    Cd.zero_()
+    with torch.cuda.graph(g):
+        assert B.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == 0
+    for _ in range(3):
+        Cd.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(B.device_to_colmajor(Cd), want)
+
+
 # --------------------------------------------------------------------------------------------- primitives
 def test_log2f_exhaustive_equals_oracle(B):
     import torch
