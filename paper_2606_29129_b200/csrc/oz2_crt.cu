@@ -338,7 +338,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
             int64_t j = (int64_t)blockIdx.x / tiles_i, ib = (int64_t)blockIdx.x - j * tiles_i;
             int s = 0; uint32_t ph = 0;
             for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-                mbar_wait_a(empty + 8 * s, ph ^ 1u);
+                mbar_wait_idle(empty + 8 * s, ph ^ 1u);          // the epilogue paces this kernel: poll lazily
                 mbar_expect_tx_a(full + 8 * s, K5_STAGE_BYTES);
                 const uint32_t dst = smem0 + s * K5_STAGE_BYTES;
                 tma_load_3d_a(&mapU, full + 8 * s, dst, (int)(ib * K5_TILE_I), (int)j, 0);
@@ -357,8 +357,8 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
             // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
             const uint64_t adesc0 = ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
             for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-                mbar_wait_a(tempty + 8 * b, bph ^ 1u);
-                mbar_wait_a(full + 8 * s, ph);
+                mbar_wait_idle(tempty + 8 * b, bph ^ 1u);
+                mbar_wait_idle(full + 8 * s, ph);
                 tc_fence_after();
                 const uint32_t sa = smem0 + s * K5_STAGE_BYTES;
                 tc_mma_i8(tmem_base + (uint32_t)(b * BUF_COLS), adesc0 | (uint64_t)((sa & 0x3FFFFu) >> 4), bdesc, IDESC, 0u);
