@@ -78,6 +78,20 @@ int ozaki2_dgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, doub
                    int num_moduli, int scaling_mode, void *stream);
 
 /*
+ * The full BLAS shape (the paper states C = A B only).  `layout`: 'C' column-major or 'R'
+ * row-major (any case; the CBLAS enums 102 / 101 are accepted too).  `transa`, `transb`: 'N', 'T' or 'C' (any case;
+ * 'C' = 'T' for real matrices; CBLAS 111 / 112 / 113).  Column-major: exactly ozaki2_dgemm_t.  Row-major: A is stored
+ * m x k (transa = 'N', lda >= k) or k x m ('T', lda >= m), B is k x n (ldb >= n) or n x k (ldb >= k), C is m x n with
+ * ldc >= n, all with the column index fastest.  A row-major problem is run as the column-major problem
+ * C^T = op(B)^T op(A)^T on the same memory; the scaled vectors (rows of op(A), columns of op(B)) are the same in both
+ * views, so the result equals ozaki2_dgemm on the logical matrices bit for bit.  Errors: -1 / -2 / -3 for a bad flag,
+ * then -(i + 3) for argument i of ozaki2_dgemm (of the caller's A, B: the internal operand swap is undone).
+ */
+int ozaki2_dgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha, const double *A,
+                      int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli,
+                      int scaling_mode, void *stream);
+
+/*
  * SGEMM variant (Fig. 6): A, B, C are FP32 (4-byte aligned device pointers, same
  * column-major conventions).  Every FP32 input is an FP64 number, so S1-S4 are the steps above on
  * the promoted inputs; S5 rounds the exact integer once to FP32, C = RN_32(C'' 2^-(e_i+f_j)), and
@@ -87,6 +101,14 @@ int ozaki2_dgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, doub
 int ozaki2_sgemm(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
                  const float *B, int64_t ldb, float beta, float *C, int64_t ldc,
                  int num_moduli, int scaling_mode, void *stream);
+
+/* The transposed-operand and full-BLAS entry points of the SGEMM variant (same conventions as the FP64 ones). */
+int ozaki2_sgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
+                   const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode,
+                   void *stream);
+int ozaki2_sgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha, const float *A,
+                      int64_t lda, const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli,
+                      int scaling_mode, void *stream);
 
 /* Bytes of device workspace ozaki2_dgemm / ozaki2_sgemm needs for this problem (0 for an invalid one). */
 size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
@@ -108,11 +130,16 @@ int ozaki2_set_workspace(void *device_ptr, size_t bytes);
  * next panel and the D2H copy of the previous one overlap the kernels (same results bit for bit:
  * e_i depends on row i of A only, f_j on column j of B only).
  * `device_scratch` is a caller-owned device buffer of at least
- * ozaki2_host_scratch_bytes(m, n, k) bytes that receives the device copies of A, B, C.
- * Host buffers should be page-locked for the copies to run at link speed.
+ * ozaki2_host_scratch_bytes(m, n, k) bytes that receives the device copies of A, B, C (the FP32 variant needs
+ * half of it); a missing or short buffer is error -14.  Host buffers should be page-locked for the copies to run
+ * at link speed.  The call returns only after every copy it enqueued has finished, also when it returns an error.
  */
 int ozaki2_dgemm_host(int64_t m, int64_t n, int64_t k, double alpha, const double *A_host, int64_t lda,
                       const double *B_host, int64_t ldb, double beta, double *C_host, int64_t ldc,
+                      int num_moduli, int scaling_mode, void *device_scratch, size_t scratch_bytes,
+                      void *stream);
+int ozaki2_sgemm_host(int64_t m, int64_t n, int64_t k, float alpha, const float *A_host, int64_t lda,
+                      const float *B_host, int64_t ldb, float beta, float *C_host, int64_t ldc,
                       int num_moduli, int scaling_mode, void *device_scratch, size_t scratch_bytes,
                       void *stream);
 size_t ozaki2_host_scratch_bytes(int64_t m, int64_t n, int64_t k);
@@ -170,10 +197,22 @@ int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64
 
 /* One INT8 product resA_l resB_l^T mod p_l for canonical planes (same layouts as above) on the
  * tensor-core kernel (use_tensor_cores = 1: one CTA per 128 x 256 tile, what ozaki2_dgemm runs;
- * 2: the cta_group::2 variant, CTA pairs on 256 x 256 tiles, a measured alternative) or on a
- * plain CUDA-core check kernel (0) that ozaki2_dgemm never uses.  None needs a workspace. */
+ * 2: the cta_group::2 variant, CTA pairs on 256 x 256 tiles, a measured alternative; 3: the kernel
+ * of 1 with its epilogue reduced to handing the accumulator back, U untouched -- the INT8 ceiling
+ * of this loop that bench.py measures) or on a plain CUDA-core check kernel (0) that ozaki2_dgemm
+ * never uses.  k must be a multiple of 128 and m of 16 (the planes are used in place).  None
+ * needs a workspace. */
 int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA,
                               const int8_t *resB, uint8_t *U, int use_tensor_cores, void *stream);
+
+/* S4 + S5 on caller-made residue planes (eq. (2)(3); Step 4): runs the CRT kernel of
+ * ozaki2_dgemm on U [N][n][m] (uint8, m fastest, m a multiple of 16; U_l < p_l), exponents e[m], f[n] (device),
+ * and writes C := alpha RN(C'') 2^-(e_i+f_j) + beta C (FP64, or FP32 if is_f32) with leading dimension ldc.
+ * Cpp == NULL: the production code path (branch-free common case, exact routine for the rare ones);
+ * Cpp != NULL ([n][m][4] u64): the exact routine for every element, which also stores C''.
+ * alpha, beta are rounded to FP32 when is_f32.  Errors: -i for argument i. */
+int ozaki2_debug_crt(int num_moduli, int64_t m, int64_t n, const uint8_t *U, const int32_t *e, const int32_t *f,
+                     double alpha, double beta, void *C, int64_t ldc, uint64_t *Cpp, int is_f32, void *stream);
 
 /* Number of kernels this library has launched in this process so far (all devices, all entry
  * points; memsets and copies are not counted). */

@@ -210,6 +210,19 @@ def unscale(Cpp, e, f, alpha: float = 1.0, beta: float = 0.0, C_in=None):
     return out
 
 
+def unscale_f32(Cpp, e, f, alpha: float = 1.0, beta: float = 0.0, C_in=None):
+    """FP32 tail of the SGEMM variant (marshalling of oz2o_unscale_f32): RN_32(C'' 2^-(e_i+f_j)), alpha / beta in FP32."""
+    n, m, _ = Cpp.shape
+    out = np.zeros((m, n), np.float32, order="F") if C_in is None else np.array(C_in, np.float32, order="F")
+    e = np.ascontiguousarray(e, np.int32)
+    f = np.ascontiguousarray(f, np.int32)
+    rc = lib().oz2o_unscale_f32(C.c_long(m), C.c_long(n), _p(Cpp), _p(e), _p(f), C.c_float(alpha), C.c_float(beta),
+                                _p(out), C.c_long(max(1, m)))
+    if rc:
+        raise ValueError(f"oz2o_unscale_f32 -> {rc}")
+    return out
+
+
 def words_to_double(words, sh: int) -> float:
     words = np.ascontiguousarray(words, np.uint64)
     return float(lib().oz2o_words_to_double(_p(words), C.c_long(sh)))

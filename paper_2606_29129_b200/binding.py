@@ -56,6 +56,17 @@ def lib() -> C.CDLL:
         L.ozaki2_sgemm_stages.restype = ci
         L.ozaki2_dgemm_host.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, ci, ci, vp, C.c_size_t, vp]
         L.ozaki2_dgemm_host.restype = ci
+        L.ozaki2_sgemm_host.argtypes = [i64, i64, i64, C.c_float, vp, i64, vp, i64, C.c_float, vp, i64, ci, ci, vp,
+                                        C.c_size_t, vp]
+        L.ozaki2_sgemm_host.restype = ci
+        L.ozaki2_sgemm_t.argtypes = [ci, ci] + sgemm_args
+        L.ozaki2_sgemm_t.restype = ci
+        L.ozaki2_dgemm_blas.argtypes = [ci, ci, ci] + gemm_args
+        L.ozaki2_dgemm_blas.restype = ci
+        L.ozaki2_sgemm_blas.argtypes = [ci, ci, ci] + sgemm_args
+        L.ozaki2_sgemm_blas.restype = ci
+        L.ozaki2_debug_crt.argtypes = [ci, i64, i64, vp, vp, vp, dbl, dbl, vp, i64, vp, ci, vp]
+        L.ozaki2_debug_crt.restype = ci
         L.ozaki2_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
         L.ozaki2_workspace_bytes.restype = C.c_size_t
         L.ozaki2_host_scratch_bytes.argtypes = [i64, i64, i64]
@@ -157,6 +168,39 @@ def ozaki2_dgemm_host(m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ld
                       device_scratch, scratch_bytes, stream=None) -> int:
     return int(lib().ozaki2_dgemm_host(m, n, k, alpha, _ptr(A_host), lda, _ptr(B_host), ldb, beta, _ptr(C_host), ldc,
                                        num_moduli, scaling_mode, _ptr(device_scratch), scratch_bytes, _stream(stream)))
+
+
+def ozaki2_sgemm_host(m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ldc, num_moduli, scaling_mode,
+                      device_scratch, scratch_bytes, stream=None) -> int:
+    return int(lib().ozaki2_sgemm_host(m, n, k, alpha, _ptr(A_host), lda, _ptr(B_host), ldb, beta, _ptr(C_host), ldc,
+                                       num_moduli, scaling_mode, _ptr(device_scratch), scratch_bytes, _stream(stream)))
+
+
+def ozaki2_sgemm_t(transa, transb, m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None) -> int:
+    return int(lib().ozaki2_sgemm_t(transa, transb, m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc,
+                                    num_moduli, scaling_mode, _stream(stream)))
+
+
+def _flag(c):
+    """'N' / 'T' / 'C' / 'R' (str or bytes) or a CBLAS enum -> int"""
+    return c if isinstance(c, int) else ord(c)
+
+
+def ozaki2_dgemm_blas(layout, transa, transb, m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode,
+                      stream=None) -> int:
+    return int(lib().ozaki2_dgemm_blas(_flag(layout), _flag(transa), _flag(transb), m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb,
+                                       beta, _ptr(Cm), ldc, num_moduli, scaling_mode, _stream(stream)))
+
+
+def ozaki2_sgemm_blas(layout, transa, transb, m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode,
+                      stream=None) -> int:
+    return int(lib().ozaki2_sgemm_blas(_flag(layout), _flag(transa), _flag(transb), m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb,
+                                       beta, _ptr(Cm), ldc, num_moduli, scaling_mode, _stream(stream)))
+
+
+def ozaki2_debug_crt(num_moduli, m, n, U, e, f, alpha, beta, Cm, ldc, Cpp=None, is_f32=False, stream=None) -> int:
+    return int(lib().ozaki2_debug_crt(num_moduli, m, n, _ptr(U), _ptr(e), _ptr(f), alpha, beta, _ptr(Cm), ldc, _ptr(Cpp),
+                                      1 if is_f32 else 0, _stream(stream)))
 
 
 def ozaki2_get_constants(num_moduli: int) -> dict:

@@ -311,7 +311,11 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
     int8_t *RA = reinterpret_cast<int8_t *>(ws + L.off_RA), *RB = reinterpret_cast<int8_t *>(ws + L.off_RB);
     uint8_t *U = ws + L.off_U;
 
-    cudaEvent_t ev[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };
+    struct StageEvents {                                    // destroyed on every exit path
+        cudaEvent_t ev[5] = { nullptr, nullptr, nullptr, nullptr, nullptr };
+        ~StageEvents() { for (int t = 0; t < 5; t++) if (ev[t]) cudaEventDestroy(ev[t]); }
+    } sev;
+    cudaEvent_t *ev = sev.ev;
     const bool timing = out && out->stage_ms;
     cudaEvent_t *uev = out && out->stage_events ? reinterpret_cast<cudaEvent_t *>(out->stage_events) : nullptr;
     if (timing) {
@@ -326,7 +330,7 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
         OZ2_CUDA_TRY(cudaMemsetAsync(colmax, 0, sizeof(int32_t) * (size_t)n, st));
         if ((rc = oz2_launch_scale_accu_side(f32, strided_a, m, k, A, lda, amax, EA, Abar, L.kp, st))) return rc;
         if ((rc = oz2_launch_scale_accu_side(f32, strided_b, n, k, B, ldb, amax, EB, Bbar, L.kp, st))) return rc;
-        if ((rc = oz2_launch_gemm_tc(1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
+        if ((rc = oz2_launch_gemm_tc(OZ2_GEMM_PATH, 1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
         if ((rc = oz2_launch_scale_accu_finish(N, m, n, EA, EB, rowmax, colmax, e, f, st))) return rc;
     } else {
         if (strided_a) rc = oz2_launch_scale_rows(mode, N, f32, m, k, A, lda, amax, ssq, e, st);
@@ -345,7 +349,7 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[2], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[2], st));
     // ---- S3 residue GEMMs
-    if ((rc = oz2_launch_gemm_tc(N, 0, m, n, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
+    if ((rc = oz2_launch_gemm_tc(OZ2_GEMM_PATH, N, 0, m, n, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[3], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[3], st));
     // ---- S4 + S5
@@ -371,7 +375,6 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
             OZ2_CUDA_TRY(cudaStreamSynchronize(st));
             for (int t = 0; t < 4; t++) OZ2_CUDA_TRY(cudaEventElapsedTime(out->stage_ms + t, ev[t], ev[t + 1]));
             OZ2_CUDA_TRY(cudaEventElapsedTime(out->stage_ms + 4, ev[0], ev[4]));
-            for (int t = 0; t < 5; t++) cudaEventDestroy(ev[t]);
         }
     }
     return 0;
@@ -385,6 +388,7 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
 // ---------------------------------------------------------------------------------------------
 static int ensure_host_streams(DeviceState *d)
 {
+    std::lock_guard<std::mutex> lk(g_mu);
     if (d->host_ready) return 0;
     OZ2_CUDA_TRY(cudaStreamCreateWithFlags(&d->s_h2d, cudaStreamNonBlocking));
     OZ2_CUDA_TRY(cudaStreamCreateWithFlags(&d->s_d2h, cudaStreamNonBlocking));
@@ -399,12 +403,13 @@ static int ensure_host_streams(DeviceState *d)
     return 0;
 }
 
-static int host_pipelined(int64_t m, int64_t n, int64_t k, double alpha, const double *A_host, int64_t lda,
-                          const double *B_host, int64_t ldb, double beta, double *C_host, int64_t ldc, int N, int mode,
-                          double *dA, double *dB, double *dC, cudaStream_t st, DeviceState *dev)
+// the enqueue part of the panel pipeline; esz = bytes per element (8: FP64, 4: FP32)
+static int host_pipelined_enqueue(int f32, int64_t m, int64_t n, int64_t k, double alpha, const uint8_t *A_host, int64_t lda,
+                                  const uint8_t *B_host, int64_t ldb, double beta, uint8_t *C_host, int64_t ldc, int N, int mode,
+                                  uint8_t *dA, uint8_t *dB, uint8_t *dC, cudaStream_t st, DeviceState *dev)
 {
     int rc;
-    if ((rc = ensure_host_streams(dev))) return rc;
+    const size_t esz = f32 ? 4 : 8;
     const Layout L = make_layout(m, n, k, N, mode);
     if (!dev->ws || dev->ws_bytes < L.total) return OZAKI2_ERR_WORKSPACE;
     uint8_t *ws = static_cast<uint8_t *>(dev->ws);
@@ -422,38 +427,126 @@ static int host_pipelined(int64_t m, int64_t n, int64_t k, double alpha, const d
     OZ2_CUDA_TRY(cudaStreamWaitEvent(sh, dev->ev0, 0));
     OZ2_CUDA_TRY(cudaStreamWaitEvent(sd, dev->ev0, 0));
     // ---- copies in: A, then the panels of B (and of C if it is read)
-    OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, 8 * (size_t)m, A_host, 8 * (size_t)lda, 8 * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, sh));
+    OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, esz * (size_t)m, A_host, esz * (size_t)lda, esz * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, sh));
     OZ2_CUDA_TRY(cudaEventRecord(dev->evA, sh));
     for (int p = 0; p < panels; p++) {
         const int64_t j0 = p * np, nc = (j0 + np < n ? np : n - j0);
-        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB + j0 * k, 8 * (size_t)k, B_host + j0 * ldb, 8 * (size_t)ldb, 8 * (size_t)k, (size_t)nc,
-                                       cudaMemcpyHostToDevice, sh));
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB + esz * (size_t)(j0 * k), esz * (size_t)k, B_host + esz * (size_t)(j0 * ldb), esz * (size_t)ldb,
+                                       esz * (size_t)k, (size_t)nc, cudaMemcpyHostToDevice, sh));
         if (beta != 0.0)
-            OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC + j0 * m, 8 * (size_t)m, C_host + j0 * ldc, 8 * (size_t)ldc, 8 * (size_t)m, (size_t)nc,
-                                           cudaMemcpyHostToDevice, sh));
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC + esz * (size_t)(j0 * m), esz * (size_t)m, C_host + esz * (size_t)(j0 * ldc), esz * (size_t)ldc,
+                                           esz * (size_t)m, (size_t)nc, cudaMemcpyHostToDevice, sh));
         OZ2_CUDA_TRY(cudaEventRecord(dev->evB[p], sh));
     }
     // ---- rows of A: S1, S2
     OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evA, 0));
-    if ((rc = oz2_launch_scale_rows(mode, N, 0, m, k, dA, m, amax, ssq, e, st))) return rc;
-    if ((rc = oz2_launch_convert(0, N, wide, 0, m, k, dA, m, e, RA, L.kp, st))) return rc;
+    if ((rc = oz2_launch_scale_rows(mode, N, f32, m, k, dA, m, amax, ssq, e, st))) return rc;
+    if ((rc = oz2_launch_convert(0, N, wide, f32, m, k, dA, m, e, RA, L.kp, st))) return rc;
     // ---- panels: S1, S2 of the columns, S3, S4 + S5, copy out
     for (int p = 0; p < panels; p++) {
         const int64_t j0 = p * np, nc = (j0 + np < n ? np : n - j0);
         OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evB[p], 0));
-        if ((rc = oz2_launch_scale_cols(mode, N, 0, nc, k, dB + j0 * k, k, f, st))) return rc;
-        if ((rc = oz2_launch_convert(1, N, wide, 0, nc, k, dB + j0 * k, k, f, RB, L.kp, st))) return rc;
-        if ((rc = oz2_launch_gemm_tc(N, 0, m, nc, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
-        if ((rc = oz2_launch_crt(N, 0, m, nc, U, L.mp, e, f, alpha, beta, dC + j0 * m, m, nullptr, st))) return rc;
+        if ((rc = oz2_launch_scale_cols(mode, N, f32, nc, k, dB + esz * (size_t)(j0 * k), k, f, st))) return rc;
+        if ((rc = oz2_launch_convert(1, N, wide, f32, nc, k, dB + esz * (size_t)(j0 * k), k, f, RB, L.kp, st))) return rc;
+        if ((rc = oz2_launch_gemm_tc(OZ2_GEMM_PATH, N, 0, m, nc, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
+        if ((rc = oz2_launch_crt(N, f32, m, nc, U, L.mp, e, f, alpha, beta, dC + esz * (size_t)(j0 * m), m, nullptr, st))) return rc;
         OZ2_CUDA_TRY(cudaEventRecord(dev->evC[p], st));
         OZ2_CUDA_TRY(cudaStreamWaitEvent(sd, dev->evC[p], 0));
-        OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host + j0 * ldc, 8 * (size_t)ldc, dC + j0 * m, 8 * (size_t)m, 8 * (size_t)m, (size_t)nc,
-                                       cudaMemcpyDeviceToHost, sd));
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host + esz * (size_t)(j0 * ldc), esz * (size_t)ldc, dC + esz * (size_t)(j0 * m), esz * (size_t)m,
+                                       esz * (size_t)m, (size_t)nc, cudaMemcpyDeviceToHost, sd));
     }
     OZ2_CUDA_TRY(cudaEventRecord(dev->evEnd, sd));
     OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evEnd, 0));
-    OZ2_CUDA_TRY(cudaStreamSynchronize(st));
     return 0;
+}
+
+static int host_pipelined(int f32, int64_t m, int64_t n, int64_t k, double alpha, const uint8_t *A_host, int64_t lda,
+                          const uint8_t *B_host, int64_t ldb, double beta, uint8_t *C_host, int64_t ldc, int N, int mode,
+                          uint8_t *dA, uint8_t *dB, uint8_t *dC, cudaStream_t st, DeviceState *dev)
+{
+    int rc;
+    if ((rc = ensure_host_streams(dev))) return rc;
+    rc = host_pipelined_enqueue(f32, m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ldc, N, mode, dA, dB, dC, st, dev);
+    // success or not, nothing may still be reading or writing the caller's host buffers when this returns
+    const cudaError_t e1 = cudaStreamSynchronize(dev->s_h2d), e2 = cudaStreamSynchronize(dev->s_d2h), e3 = cudaStreamSynchronize(st);
+    if (rc) return rc;
+    if (e1 != cudaSuccess) return (int)e1;
+    if (e2 != cudaSuccess) return (int)e2;
+    return (int)e3;
+}
+
+// ozaki2_dgemm_host / ozaki2_sgemm_host
+static int host_entry(int f32, int64_t m, int64_t n, int64_t k, double alpha, const void *A_host, int64_t lda, const void *B_host,
+                      int64_t ldb, double beta, void *C_host, int64_t ldc, int num_moduli, int scaling_mode, void *device_scratch,
+                      size_t scratch_bytes, cudaStream_t st)
+{
+    int rc = check_args(m, n, k, A_host, lda, B_host, ldb, C_host, ldc, num_moduli, scaling_mode);
+    if (rc) return rc;
+    if (m == 0 || n == 0) return 0;
+    const size_t esz = f32 ? 4 : 8;
+    const size_t need = align_up(esz * (size_t)m * k) + align_up(esz * (size_t)k * n) + align_up(esz * (size_t)m * n);
+    if (!device_scratch || scratch_bytes < need) return -14;
+    uint8_t *base = static_cast<uint8_t *>(device_scratch);
+    uint8_t *dA = base, *dB = base + align_up(esz * (size_t)m * k), *dC = dB + align_up(esz * (size_t)k * n);
+    const uint8_t *Ah = static_cast<const uint8_t *>(A_host), *Bh = static_cast<const uint8_t *>(B_host);
+    uint8_t *Ch = static_cast<uint8_t *>(C_host);
+    if (k > 0 && alpha != 0.0 && scaling_mode != OZAKI2_MODE_ACCURATE && n >= 512) {
+        DeviceState *dev = nullptr;
+        if ((rc = ensure_device(&dev))) return rc;
+        return host_pipelined(f32, m, n, k, alpha, Ah, lda, Bh, ldb, beta, Ch, ldc, num_moduli, scaling_mode, dA, dB, dC, st, dev);
+    }
+    auto enqueue = [&]() -> int {
+        if (k > 0) {
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, esz * (size_t)m, Ah, esz * (size_t)lda, esz * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, st));
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB, esz * (size_t)k, Bh, esz * (size_t)ldb, esz * (size_t)k, (size_t)n, cudaMemcpyHostToDevice, st));
+        }
+        if (beta != 0.0)
+            OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC, esz * (size_t)m, Ch, esz * (size_t)ldc, esz * (size_t)m, (size_t)n, cudaMemcpyHostToDevice, st));
+        const int r = run_path(f32, m, n, k, alpha, dA, m > 1 ? m : 1, dB, k > 1 ? k : 1, beta, dC, m > 1 ? m : 1, num_moduli, scaling_mode, st, nullptr);
+        if (r) return r;
+        OZ2_CUDA_TRY(cudaMemcpy2DAsync(Ch, esz * (size_t)ldc, dC, esz * (size_t)m, esz * (size_t)m, (size_t)n, cudaMemcpyDeviceToHost, st));
+        return 0;
+    };
+    rc = enqueue();
+    const cudaError_t es = cudaStreamSynchronize(st);      // also on error: the host buffers must be quiescent on return
+    if (rc) return rc;
+    return (int)es;
+}
+
+// BLAS-style flags: 'N' / 'T' / 'C' (any case; 'C' = 'T' for real matrices) or the CBLAS enums 111 / 112 / 113
+static int parse_trans(int c)
+{
+    if (c == 'N' || c == 'n' || c == 111) return 0;
+    if (c == 'T' || c == 't' || c == 'C' || c == 'c' || c == 112 || c == 113) return 1;
+    return -1;
+}
+// 'C' column-major / 'R' row-major (any case) or the CBLAS enums 102 / 101
+static int parse_layout(int c)
+{
+    if (c == 'C' || c == 'c' || c == 102) return 0;
+    if (c == 'R' || c == 'r' || c == 101) return 1;
+    return -1;
+}
+
+// The full BLAS shape.  A row-major problem is the column-major problem C^T = op(B)^T op(A)^T on the same memory:
+// the operands swap places and m, n swap, the flags stay with their matrices.  The vectors the method scales --
+// rows of op(A), columns of op(B) -- are the same vectors in both views, so the result is the oracle's on the
+// logical matrices bit for bit.
+static int blas_entry(int f32, int layout, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha, const void *A,
+                      int64_t lda, const void *B, int64_t ldb, double beta, void *C, int64_t ldc, int N, int mode, cudaStream_t st)
+{
+    const int lay = parse_layout(layout), ta = parse_trans(transa), tb = parse_trans(transb);
+    if (lay < 0) return -1;
+    if (ta < 0) return -2;
+    if (tb < 0) return -3;
+    int rc;
+    if (!lay) rc = run_path(f32, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, N, mode, st, nullptr, ta, tb);
+    else rc = run_path(f32, n, m, k, alpha, B, ldb, A, lda, beta, C, ldc, N, mode, st, nullptr, tb, ta);
+    if (rc >= 0 || rc <= -100) return rc;
+    // argument numbers of run_path (m n k alpha A lda B ldb beta C ldc N mode stream) -> this prototype
+    static const int col[15] = { 0, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17 };
+    static const int row[15] = { 0, 5, 4, 6, 7, 10, 11, 8, 9, 12, 13, 14, 15, 16, 17 };
+    return -(lay ? row[-rc] : col[-rc]);
 }
 
 extern "C" {
@@ -530,44 +623,60 @@ int ozaki2_dgemm_host(int64_t m, int64_t n, int64_t k, double alpha, const doubl
                       const double *B_host, int64_t ldb, double beta, double *C_host, int64_t ldc, int num_moduli,
                       int scaling_mode, void *device_scratch, size_t scratch_bytes, void *stream)
 {
-    int rc = check_args(m, n, k, A_host, lda, B_host, ldb, C_host, ldc, num_moduli, scaling_mode);
-    if (rc) return rc;
-    if (m == 0 || n == 0) return 0;
-    if (!device_scratch || scratch_bytes < ozaki2_host_scratch_bytes(m, n, k)) return -15;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    uint8_t *base = static_cast<uint8_t *>(device_scratch);
-    double *dA = reinterpret_cast<double *>(base);
-    double *dB = reinterpret_cast<double *>(base + align_up(8 * (size_t)m * k));
-    double *dC = reinterpret_cast<double *>(base + align_up(8 * (size_t)m * k) + align_up(8 * (size_t)k * n));
-    if (k > 0 && alpha != 0.0 && scaling_mode != OZAKI2_MODE_ACCURATE && n >= 512) {
-        DeviceState *dev = nullptr;
-        if ((rc = ensure_device(&dev))) return rc;
-        return host_pipelined(m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ldc, num_moduli, scaling_mode, dA, dB, dC,
-                              st, dev);
-    }
-    if (k > 0) {
-        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dA, 8 * (size_t)m, A_host, 8 * (size_t)lda, 8 * (size_t)m, (size_t)k, cudaMemcpyHostToDevice, st));
-        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dB, 8 * (size_t)k, B_host, 8 * (size_t)ldb, 8 * (size_t)k, (size_t)n, cudaMemcpyHostToDevice, st));
-    }
-    if (beta != 0.0)
-        OZ2_CUDA_TRY(cudaMemcpy2DAsync(dC, 8 * (size_t)m, C_host, 8 * (size_t)ldc, 8 * (size_t)m, (size_t)n, cudaMemcpyHostToDevice, st));
-    rc = run_path(0, m, n, k, alpha, dA, m > 1 ? m : 1, dB, k > 1 ? k : 1, beta, dC, m > 1 ? m : 1, num_moduli, scaling_mode, st, nullptr);
-    if (rc) return rc;
-    OZ2_CUDA_TRY(cudaMemcpy2DAsync(C_host, 8 * (size_t)ldc, dC, 8 * (size_t)m, 8 * (size_t)m, (size_t)n, cudaMemcpyDeviceToHost, st));
-    OZ2_CUDA_TRY(cudaStreamSynchronize(st));
-    return 0;
+    return host_entry(0, m, n, k, alpha, A_host, lda, B_host, ldb, beta, C_host, ldc, num_moduli, scaling_mode, device_scratch,
+                      scratch_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int ozaki2_sgemm_host(int64_t m, int64_t n, int64_t k, float alpha, const float *A_host, int64_t lda, const float *B_host,
+                      int64_t ldb, float beta, float *C_host, int64_t ldc, int num_moduli, int scaling_mode,
+                      void *device_scratch, size_t scratch_bytes, void *stream)
+{
+    return host_entry(1, m, n, k, (double)alpha, A_host, lda, B_host, ldb, (double)beta, C_host, ldc, num_moduli, scaling_mode,
+                      device_scratch, scratch_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int ozaki2_sgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
+                   const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream)
+{
+    if (transa != 0 && transa != 1) return -1;
+    if (transb != 0 && transb != 1) return -2;
+    const int rc = run_path(1, m, n, k, (double)alpha, A, lda, B, ldb, (double)beta, C, ldc, num_moduli, scaling_mode,
+                            static_cast<cudaStream_t>(stream), nullptr, transa, transb);
+    return rc < 0 && rc > -100 ? rc - 2 : rc;
+}
+
+int ozaki2_dgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha, const double *A,
+                      int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli,
+                      int scaling_mode, void *stream)
+{
+    return blas_entry(0, layout, transa, transb, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+                      static_cast<cudaStream_t>(stream));
+}
+
+int ozaki2_sgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha, const float *A,
+                      int64_t lda, const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli,
+                      int scaling_mode, void *stream)
+{
+    return blas_entry(1, layout, transa, transb, m, n, k, (double)alpha, A, lda, B, ldb, (double)beta, C, ldc, num_moduli,
+                      scaling_mode, static_cast<cudaStream_t>(stream));
 }
 
 const char *ozaki2_status_string(int status)
 {
+    // names in the numbering of ozaki2_dgemm / ozaki2_dgemm_host (other entry points shift them as their
+    // headers say; the number is always the position in the prototype that was called)
     static const char *arg_names[] = { "",      "m",   "n",    "k", "alpha",      "A",           "lda",   "B",
-                                       "ldb",   "beta", "C",   "ldc", "num_moduli", "scaling_mode", "stream", "scratch" };
-    static thread_local char buf[96];
+                                       "ldb",   "beta", "C",   "ldc", "num_moduli", "scaling_mode", "stream / device_scratch" };
+    static thread_local char buf[128];
     if (status == 0) return "success";
     if (status == OZAKI2_ERR_WORKSPACE) return "workspace missing or too small (ozaki2_set_workspace)";
     if (status == OZAKI2_ERR_DEVICE) return "current device is not sm_100 (B200)";
-    if (status < 0 && status >= -15) {
-        snprintf(buf, sizeof buf, "invalid argument %d (%s)", -status, arg_names[-status]);
+    if (status < 0 && status >= -14) {
+        snprintf(buf, sizeof buf, "invalid argument %d (ozaki2_dgemm numbering: %s)", -status, arg_names[-status]);
+        return buf;
+    }
+    if (status < 0 && status > -100) {
+        snprintf(buf, sizeof buf, "invalid argument %d", -status);
         return buf;
     }
     if (status > 0) return cudaGetErrorString(static_cast<cudaError_t>(status));
@@ -629,13 +738,31 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
     if (k <= 0 || k % 128 != 0 || k > OZAKI2_MAX_K) return -4;      // canonical planes are used in place: pitch = k
     if (m % 16 != 0) return -2;                                     // U pitch = m
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (use_tensor_cores < 0 || use_tensor_cores > 3) return -8;
     if (use_tensor_cores) {
-        oz2_gemm_set_pair_mode(use_tensor_cores == 2 ? 1 : 0);      // 1: one CTA per tile (the ozaki2_dgemm path), 2: CTA pairs
-        const int rc2 = oz2_launch_gemm_tc(num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
-        oz2_gemm_set_pair_mode(0);
-        return rc2;
+        // 1: one CTA per tile (the ozaki2_dgemm path), 2: CTA pairs, 3: the path kernel without its epilogue
+        const int variant = use_tensor_cores == 2 ? OZ2_GEMM_PAIR : use_tensor_cores == 3 ? OZ2_GEMM_MMA_ONLY : OZ2_GEMM_PATH;
+        return oz2_launch_gemm_tc(variant, num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
     }
     return oz2_launch_gemm_check(num_moduli, m, n, k, resA, resB, k, U, m, st);
+}
+
+int ozaki2_debug_crt(int num_moduli, int64_t m, int64_t n, const uint8_t *U, const int32_t *e, const int32_t *f, double alpha,
+                     double beta, void *C, int64_t ldc, uint64_t *Cpp, int is_f32, void *stream)
+{
+    DeviceState *dev = nullptr;
+    int rc = ensure_device(&dev);
+    if (rc) return rc;
+    if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return -1;
+    if (m < 0 || m % 16 != 0) return -2;                            // the planes are used in place: pitch = m
+    if (n < 0) return -3;
+    if (m == 0 || n == 0) return 0;
+    if (!U) return -4;
+    if (!e) return -5;
+    if (!f) return -6;
+    if (!C) return -9;
+    if (ldc < m) return -10;
+    return oz2_launch_crt(num_moduli, is_f32 ? 1 : 0, m, n, U, m, e, f, alpha, beta, C, ldc, Cpp, static_cast<cudaStream_t>(stream));
 }
 
 uint64_t ozaki2_kernel_launches(void) { return g_launches.load(std::memory_order_relaxed); }

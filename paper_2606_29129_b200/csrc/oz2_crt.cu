@@ -413,18 +413,12 @@ template <int NW, typename TO>
 int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const int32_t *e, const int32_t *f, TO alpha,
               TO beta, TO *C, int64_t ldc, uint64_t *Cpp, cudaStream_t st)
 {
-    EncodeTiledFn enc = get_encode_fn();
-    if (!enc) return (int)cudaErrorNotSupported;
     // U planes [N][n][mp] -> 3-D map (i, j, l), box (128, 1, 32): rows i >= mp and planes l >= N are zero filled
     CUtensorMap map;
-    cuuint64_t dims[3] = { (cuuint64_t)mp, (cuuint64_t)n, (cuuint64_t)N };
-    cuuint64_t strides[2] = { (cuuint64_t)mp, (cuuint64_t)(n * mp) };
-    cuuint32_t box[3] = { 128u, 1u, (cuuint32_t)K5_KPAD };
-    cuuint32_t estr[3] = { 1u, 1u, 1u };
-    CUresult r = enc(&map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint8_t *>(U), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    const TensorMapKey key = { U, (uint64_t)mp, (uint64_t)n, (uint64_t)N, (uint64_t)mp, (uint64_t)(n * mp),
+                               128u, 1u, (uint32_t)K5_KPAD, (uint32_t)CU_TENSOR_MAP_SWIZZLE_128B };
+    const int erc = encode_u8_3d_cached(&map, key);
+    if (erc) return erc;
     static int sms = 0;
     if (!sms) {
         int dev = 0;

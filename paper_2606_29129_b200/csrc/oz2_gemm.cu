@@ -8,8 +8,8 @@
 //     SWIZZLE_128B shared-memory tiles (A 128 x 128 B, B 256 x 128 B per stage),
 //   * math: tcgen05.mma.cta_group::1.kind::i8, M = 128, N = 256, K = 32 per instruction, issued by one thread;
 //     INT32 accumulators live in tensor memory (2 x 256 columns, double buffered), they never touch HBM,
-//   * epilogue: 8 warps (two per TMEM lane quarter) read the accumulator with tcgen05.ld, reduce mod p_l and write one byte per element,
-//     overlapping the MMAs of the next tile,
+//   * epilogue: 16 warps (four per TMEM lane quarter, 64 accumulator columns each) read the accumulator with
+//     tcgen05.ld, reduce mod p_l and write one byte per element, overlapping the MMAs of the next tile,
 //   * persistent grid (one CTA per SM), static tile order: modulus-major, then groups of 32 M-tiles so that the
 //     148 tiles in flight share A / B panels in L2.
 // INT32 accumulation wraps (never saturates): with reading R6 that keeps k <= 2^17 exact for p = 256.
@@ -97,8 +97,10 @@ __device__ __forceinline__ TileCoord decode_tile(int64_t t, int tiles_m, int til
     return c;
 }
 
-// MAXEPI = false: U[plane][j][mp] = acc mod p_(mod_base + plane);  true: rowmax / colmax of the accumulators
-template <bool MAXEPI>
+// EPI = EPI_MODP: U[plane][j][mp] = acc mod p_(mod_base + plane);  EPI_MAX: rowmax / colmax of the accumulators;
+// EPI_NONE: the accumulator is handed back unread (the measured INT8 ceiling of this very loop, bench.py)
+enum { EPI_MODP = 0, EPI_MAX = 1, EPI_NONE = 2 };
+template <int EPI>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, int nplanes,
                 int mod_base, int m, int n, int kb0, int num_kb, int accum, uint8_t *__restrict__ U, int64_t mp,
@@ -175,9 +177,9 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             }
         }
     } else {
-        // ===================== epilogue: warps 2..9, TMEM lane quarter = warp % 4, column half = (warp - 2) / 4 =====================
+        // ===================== epilogue: warps 2..17, TMEM lane quarter = warp % 4, column slice = (warp - 2) / 4 =====================
         const int q = warp & 3;                                // TMEM lane quarter
-        const int half = (warp - 2) >> 2;                      // column slice of the tile
+        const int half = (warp - 2) >> 2;                      // column slice of the tile (64 columns)
         int as = 0;
         uint32_t aphase = 0;
         for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
@@ -186,7 +188,9 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             tc_fence_after();
             const int i = c.m0 + q * 32 + lane;                // output row of this thread
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TILE_N);
-            if (!MAXEPI) {
+            if (EPI == EPI_NONE) {
+                // nothing: MMA-only ceiling run
+            } else if (EPI == EPI_MODP) {
                 const int l = mod_base + c.plane;
                 const Oz2ModTab tb = c_mod[l];
                 if (!accum) {
@@ -517,16 +521,9 @@ __global__ void k_mod_p(int l, const int32_t *__restrict__ in, uint8_t *__restri
 // planes [nplanes][rows][kp] INT8 -> 3-D map (k, row, plane), box (128, box_rows, 1), 128B swizzle, zero OOB fill
 int make_plane_map(CUtensorMap *map, const int8_t *base, int64_t kp, int64_t rows, int nplanes, int box_rows)
 {
-    EncodeTiledFn enc = get_encode_fn();
-    if (!enc) return (int)cudaErrorNotSupported;
-    cuuint64_t dims[3] = { (cuuint64_t)kp, (cuuint64_t)rows, (cuuint64_t)nplanes };
-    cuuint64_t strides[2] = { (cuuint64_t)kp, (cuuint64_t)(rows * kp) };
-    cuuint32_t box[3] = { (cuuint32_t)TILE_K, (cuuint32_t)box_rows, 1u };
-    cuuint32_t estr[3] = { 1u, 1u, 1u };
-    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<int8_t *>(base), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? 0 : (int)cudaErrorInvalidValue;
+    const TensorMapKey key = { base, (uint64_t)kp, (uint64_t)rows, (uint64_t)nplanes, (uint64_t)kp, (uint64_t)(rows * kp),
+                               (uint32_t)TILE_K, (uint32_t)box_rows, 1u, (uint32_t)CU_TENSOR_MAP_SWIZZLE_128B };
+    return encode_u8_3d_cached(map, key);
 }
 
 int num_sms()
@@ -545,28 +542,26 @@ int num_sms()
 int oz2_gemm_upload_tables(const Oz2HostTables &t)
 {
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_mod, t.mod, sizeof(t.mod)));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<EPI_MODP>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<EPI_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<EPI_NONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
     return 0;
 }
 
-// 0: one CTA per 128 x 256 tile (default); 1: CTA pairs on 256 x 256 tiles.  Measured at 8192^3, N = 16 on random
-// residues, 20 calls back to back: 5.98 / 6.06 ms single vs 6.29 / 6.15 ms pairs -- the kernel is bound by the
-// power cap and the operand toggling, not by shared-memory or L2 traffic, so the pair variant stays a tested
-// alternative (ozaki2_debug_residue_gemm, use_tensor_cores = 2) and is not on the ozaki2_dgemm path.
-static int g_gemm_pair = 0;
-void oz2_gemm_set_pair_mode(int on) { g_gemm_pair = on; }
-
-int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA, const int8_t *RB,
-                       int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
+// variant OZ2_GEMM_PATH: one CTA per 128 x 256 tile -- what ozaki2_dgemm runs.  OZ2_GEMM_PAIR: CTA pairs on 256 x 256
+// tiles (cta_group::2); measured at 8192^3, N = 16 on random residues, 20 calls back to back: 5.98 / 6.06 ms single vs
+// 6.29 / 6.15 ms pairs, so it stays a tested alternative behind ozaki2_debug_residue_gemm.  OZ2_GEMM_MMA_ONLY: the
+// path kernel with the epilogue reduced to handing the accumulator back (INT8 ceiling of this loop; U untouched).
+int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA,
+                       const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
 {
     (void)k;
     if (m <= 0 || n <= 0 || nplanes <= 0) return 0;
     CUtensorMap mapA, mapB;
     const int num_kb = (int)(kp / TILE_K);
-    if (g_gemm_pair && m > TILE_M && kp <= (1 << 17)) {
+    if (variant == OZ2_GEMM_PAIR && m > TILE_M && kp <= (1 << 17)) {
         int rc = make_plane_map(&mapA, RA, kp, m, nplanes, 128);
         if (rc) return rc;
         rc = make_plane_map(&mapB, RB, kp, n, nplanes, 128);
@@ -594,16 +589,20 @@ int oz2_launch_gemm_tc(int nplanes, int mod_base, int64_t m, int64_t n, int64_t 
     if (tiles < grid) grid = (int)tiles;
     if (rowmax) {
         // accurate mode's auxiliary product: entries <= 64, the API keeps k <= 2^18 so that 2^12 k fits INT32
-        k3_residue_gemm<true><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, 0, num_kb,
-                                                                   0, nullptr, mp, rowmax, colmax);
+        k3_residue_gemm<EPI_MAX><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, 0, num_kb,
+                                                                      0, nullptr, mp, rowmax, colmax);
         oz2_count_launches(1);
     } else {
         // the INT32 accumulator holds k <= 2^17; longer products are blocked and summed mod p_l in the epilogue
         constexpr int KB_MAX = (1 << 17) / TILE_K;
         for (int kb0 = 0; kb0 < num_kb; kb0 += KB_MAX) {
             const int nkb = num_kb - kb0 < KB_MAX ? num_kb - kb0 : KB_MAX;
-            k3_residue_gemm<false><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, kb0, nkb,
-                                                                        kb0 > 0 ? 1 : 0, U, mp, nullptr, nullptr);
+            if (variant == OZ2_GEMM_MMA_ONLY)
+                k3_residue_gemm<EPI_NONE><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, kb0,
+                                                                               nkb, 0, nullptr, mp, nullptr, nullptr);
+            else
+                k3_residue_gemm<EPI_MODP><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, kb0,
+                                                                               nkb, kb0 > 0 ? 1 : 0, U, mp, nullptr, nullptr);
             oz2_count_launches(1);
         }
     }

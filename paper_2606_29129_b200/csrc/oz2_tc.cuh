@@ -4,10 +4,45 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
+#include <mutex>
 
 namespace {
 
-constexpr uint32_t SPIN_LIMIT = 1u << 24;         // polls before a stuck barrier traps instead of hanging
+// A stuck mbarrier must not hang the GPU box, and a legitimately long stall (debugger, MPS time slicing, deep clock
+// throttling) must not kill the context: the waits below spin freely for SPIN_FAST polls, then back off with
+// __nanosleep and give up (trap) only after STALL_NS of wall time by %globaltimer.  -DOZ2_TRAP_ON_STALL=0 removes
+// the trap altogether.
+#ifndef OZ2_TRAP_ON_STALL
+#define OZ2_TRAP_ON_STALL 1
+#endif
+constexpr uint32_t SPIN_FAST = 1u << 14;
+constexpr unsigned long long STALL_NS = 20ull * 1000ull * 1000ull * 1000ull;     // 20 s
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+// slow side of every wait: called once the fast spin budget is used up
+__device__ __noinline__ void mbar_wait_slow(uint32_t addr, uint32_t parity)
+{
+    const unsigned long long t0 = globaltimer_ns();
+    uint32_t done = 0;
+    while (true) {
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(addr), "r"(parity)
+                     : "memory");
+        if (done) return;
+        __nanosleep(1000);
+#if OZ2_TRAP_ON_STALL
+        if (globaltimer_ns() - t0 > STALL_NS) __trap();
+#endif
+    }
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -35,7 +70,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
                      : "r"(addr), "r"(parity)
                      : "memory");
         if (done) break;
-        if (++spins > SPIN_LIMIT) __trap();
+        if (++spins > SPIN_FAST) { mbar_wait_slow(addr, parity); break; }
     }
 }
 __device__ __forceinline__ void tma_load_3d(const CUtensorMap *map, uint64_t *bar, void *dst, int c0, int c1, int c2)
@@ -72,7 +107,7 @@ __device__ __forceinline__ void mbar_wait_a(uint32_t addr, uint32_t parity)
                      : "r"(addr), "r"(parity)
                      : "memory");
         if (done) break;
-        if (++spins > SPIN_LIMIT) __trap();
+        if (++spins > SPIN_FAST) { mbar_wait_slow(addr, parity); break; }
     }
 }
 // wait of a warp that is expected to idle for a long time (an epilogue warp waiting for the next accumulator):
@@ -89,7 +124,7 @@ __device__ __forceinline__ void mbar_wait_idle(uint32_t addr, uint32_t parity)
                      : "memory");
         if (done) break;
         __nanosleep(200);
-        if (++spins > SPIN_LIMIT) __trap();
+        if (++spins > SPIN_FAST) { mbar_wait_slow(addr, parity); break; }
     }
 }
 __device__ __forceinline__ void mbar_arrive_a(uint32_t addr)
@@ -128,5 +163,40 @@ inline EncodeTiledFn get_encode_fn()
     return fn;
 }
 
+// Encoded tensor maps are pure functions of (base, dims, strides, box, swizzle): a small cache keeps the host from
+// re-encoding the same three maps on every ozaki2_dgemm call (cuTensorMapEncodeTiled costs a few microseconds,
+// which shows at small sizes).  Uniform key: 3-D UINT8 maps only, which is all this library uses.
+struct TensorMapKey {
+    const void *base;
+    uint64_t d0, d1, d2, s1, s2;
+    uint32_t b0, b1, b2, swizzle;
+};
+inline int encode_u8_3d_cached(CUtensorMap *out, const TensorMapKey &key)
+{
+    constexpr int SLOTS = 16;
+    static TensorMapKey keys[SLOTS];
+    static CUtensorMap maps[SLOTS];
+    static int used = 0, next = 0;
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lk(mu);
+    for (int t = 0; t < used; t++)
+        if (memcmp(&keys[t], &key, sizeof(key)) == 0) { *out = maps[t]; return 0; }
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return (int)cudaErrorNotSupported;
+    cuuint64_t dims[3] = { key.d0, key.d1, key.d2 };
+    cuuint64_t strides[2] = { key.s1, key.s2 };
+    cuuint32_t box[3] = { key.b0, key.b1, key.b2 };
+    cuuint32_t estr[3] = { 1u, 1u, 1u };
+    CUtensorMap m;
+    CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(key.base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, (CUtensorMapSwizzle)key.swizzle, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return (int)cudaErrorInvalidValue;
+    const int slot = used < SLOTS ? used++ : (next = (next + 1) % SLOTS);
+    keys[slot] = key;
+    maps[slot] = m;
+    *out = m;
+    return 0;
+}
 
 } // namespace

@@ -1,0 +1,168 @@
+"""GPU parity of the remaining entry points (-m gpu): the plain ozaki2_dgemm / ozaki2_sgemm calls (production CRT code
+path, no stage outputs) on inputs whose results are subnormal, overflowing or spread over the whole exponent range;
+the full BLAS shape (row-major, 'N' / 'T' / 'C'); ozaki2_sgemm_t; ozaki2_sgemm_host.  Expected values: the oracle on
+the LOGICAL matrices."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import ozaki2_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_29129_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def plain_dgemm(B, A, Bm, N, mode):
+    import torch
+    Ad, Bd = B.colmajor_to_device(A), B.colmajor_to_device(Bm)
+    Cd = B.dgemm(Ad, Bd, N, mode)
+    torch.cuda.synchronize()
+    return B.device_to_colmajor(Cd)
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("N", [8, 14, 17, 20])
+def test_plain_call_on_wide_exponent_inputs(B, mode, N):
+    A, Bm = W.wide_exponent_matrices(300, 130, 260, seed=31 + N)
+    with np.errstate(all="ignore"):
+        assert np.array_equal(plain_dgemm(B, A, Bm, N, mode), O.dgemm(A, Bm, N, mode))
+
+
+@pytest.mark.parametrize("sa,sb", [(-600, -500), (600, 500), (-530, -520), (-1000, -40), (500, 523)])
+@pytest.mark.parametrize("N", [12, 16, 19])
+def test_plain_call_with_subnormal_and_overflowing_results(B, sa, sb, N):
+    # C = A B 2^(sa+sb): subnormal, partly flushed to zero, or overflowing; the production CRT path must hand these
+    # elements to its exact routine (one rounding in total, also when the result is subnormal)
+    A, Bm = W.eq15_matrices(260, 70, 200, 1.0, 900 + N)
+    A, Bm = np.ldexp(A, sa), np.ldexp(Bm, sb)
+    with np.errstate(all="ignore"):
+        want = O.dgemm(A, Bm, N, 2)
+        got = plain_dgemm(B, A, Bm, N, 2)
+        assert np.array_equal(got, want)
+    if sa + sb < -1000:
+        assert np.any((want != 0) & (np.abs(want) < 2.3e-308))          # subnormal results are really exercised
+    if sa + sb > 1000:
+        assert np.any(np.isinf(want))
+
+
+@pytest.mark.parametrize("sa,sb", [(-80, -60), (70, 55)])
+def test_plain_sgemm_with_subnormal_and_overflowing_results(B, sa, sb):
+    import torch
+    A, Bm = W.eq15_matrices(260, 70, 200, 1.0, 77)
+    A = np.asfortranarray(np.ldexp(A, sa).astype(np.float32))
+    Bm = np.asfortranarray(np.ldexp(Bm, sb).astype(np.float32))
+    m, k = A.shape
+    n = Bm.shape[1]
+    Ad, Bd = B.colmajor_to_device(A, np.float32), B.colmajor_to_device(Bm, np.float32)
+    Cd = torch.empty((n, m), dtype=torch.float32, device="cuda")
+    B.ensure_workspace(m, n, k, 8, 2)
+    assert B.ozaki2_sgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, 8, 2) == 0
+    torch.cuda.synchronize()
+    with np.errstate(all="ignore"):
+        want = O.sgemm(A, Bm, 8, 2)
+        assert np.array_equal(B.device_to_colmajor(Cd), want)
+    assert np.any(np.isinf(want)) or np.any((want != 0) & (np.abs(want) < 1.2e-38))
+
+
+def _stored(X, trans, row_major, pad):
+    """memory image of logical matrix X under (trans, layout) as a numpy array whose C-order bytes are the buffer,
+    and its leading dimension"""
+    S = X.T if trans else X                        # the stored matrix
+    if row_major:
+        ld = S.shape[1] + pad
+        buf = np.zeros((S.shape[0], ld), X.dtype)
+        buf[:, :S.shape[1]] = S
+    else:
+        ld = S.shape[0] + pad
+        buf = np.zeros((S.shape[1], ld), X.dtype)   # column-major: columns are contiguous
+        buf[:, :S.shape[0]] = S.T
+    return buf, ld
+
+
+@pytest.mark.parametrize("layout", ["C", "R", 101])
+@pytest.mark.parametrize("ta,tb", [("N", "N"), ("T", "n"), ("n", "C"), ("t", "T"), (111, 112)])
+@pytest.mark.parametrize("f32", [False, True])
+def test_full_blas_signature(B, layout, ta, tb, f32):
+    import torch
+    m, n, k, N, mode = 150, 90, 260, (8 if f32 else 15), 2
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 321)
+    dt = np.float32 if f32 else np.float64
+    A, Bm = np.asfortranarray(A.astype(dt)), np.asfortranarray(Bm.astype(dt))
+    rm = layout in ("R", "r", 101)
+    tra = ta in ("T", "t", "C", "c", 112, 113)
+    trb = tb in ("T", "t", "C", "c", 112, 113)
+    bufA, lda = _stored(A, tra, rm, 3)
+    bufB, ldb = _stored(Bm, trb, rm, 5)
+    rng = np.random.Generator(np.random.PCG64(1))
+    Cin = rng.standard_normal((m, n)).astype(dt)
+    bufC, ldc = _stored(Cin, False, rm, 2)
+    Ad, Bd, Cd = torch.from_numpy(bufA).cuda(), torch.from_numpy(bufB).cuda(), torch.from_numpy(bufC.copy()).cuda()
+    B.ensure_workspace(max(m, n), max(m, n), k, N, mode)
+    call = B.ozaki2_sgemm_blas if f32 else B.ozaki2_dgemm_blas
+    alpha, beta = 0.5, -2.0
+    assert call(layout, ta, tb, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == 0
+    torch.cuda.synchronize()
+    got = Cd.cpu().numpy()
+    got = got[:, :n] if rm else got[:, :m].T
+    want = (O.sgemm if f32 else O.dgemm)(A, Bm, N, mode, alpha=alpha, beta=beta, C_in=Cin.copy())
+    assert np.array_equal(got, want)
+    # errors are reported in the numbering of this prototype, for the caller's own A and B
+    assert call("X", ta, tb, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == -1
+    assert call(layout, "Q", tb, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == -2
+    assert call(layout, ta, 7, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == -3
+    assert call(layout, ta, tb, -1, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == -4
+    assert call(layout, ta, tb, m, -1, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == -5
+    assert call(layout, ta, tb, m, n, k, alpha, Ad, 1, Bd, ldb, beta, Cd, ldc, N, mode) == -9
+    assert call(layout, ta, tb, m, n, k, alpha, Ad, lda, Bd, 1, beta, Cd, ldc, N, mode) == -11
+    assert call(layout, ta, tb, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, 1, N, mode) == -14
+    assert call(layout, ta, tb, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, 1, mode) == -15
+    assert call(layout, ta, tb, m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, 9) == -16
+
+
+@pytest.mark.parametrize("transa,transb", [(0, 0), (1, 0), (0, 1), (1, 1)])
+def test_sgemm_transposed_operands(B, transa, transb):
+    import torch
+    m, n, k, N, mode = 130, 70, 200, 9, 0
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 11)
+    A, Bm = np.asfortranarray(A.astype(np.float32)), np.asfortranarray(Bm.astype(np.float32))
+    bufA, lda = _stored(A, transa, False, 1)
+    bufB, ldb = _stored(Bm, transb, False, 4)
+    Ad, Bd = torch.from_numpy(bufA).cuda(), torch.from_numpy(bufB).cuda()
+    Cd = torch.full((n, m), float("nan"), dtype=torch.float32, device="cuda")
+    B.ensure_workspace(m, n, k, N, mode)
+    assert B.ozaki2_sgemm_t(transa, transb, m, n, k, 1.0, Ad, lda, Bd, ldb, 0.0, Cd, m, N, mode) == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(B.device_to_colmajor(Cd), O.sgemm(A, Bm, N, mode))
+    assert B.ozaki2_sgemm_t(3, 0, m, n, k, 1.0, Ad, lda, Bd, ldb, 0.0, Cd, m, N, mode) == -1
+
+
+@pytest.mark.parametrize("n,mode", [(80, 2), (1100, 2), (1100, 1), (600, 0)])
+def test_sgemm_host_buffer_entry_point(B, n, mode):
+    # n >= 512 in modes 1, 2: column panels with the copies overlapped; otherwise the plain route
+    import torch
+    m, k, N = 200, 300, 9
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 55)
+    lda, ldb, ldc = m + 4, k + 2, m + 6
+    Ah = np.zeros((lda, k), np.float32, order="F"); Ah[:m] = A
+    Bh = np.zeros((ldb, n), np.float32, order="F"); Bh[:k] = Bm
+    rng = np.random.Generator(np.random.PCG64(4))
+    Cin = np.asfortranarray(rng.standard_normal((ldc, n)).astype(np.float32))
+    Ch = Cin.copy(order="F")
+    B.ensure_workspace(m, n, k, N, mode)
+    nbytes = B.ozaki2_host_scratch_bytes(m, n, k)
+    scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    assert B.ozaki2_sgemm_host(m, n, k, 0.5, Ah, lda, Bh, ldb, 1.5, Ch, ldc, N, mode, scratch, nbytes) == 0
+    want = O.sgemm(Ah[:m], Bh[:k], N, mode, alpha=0.5, beta=1.5, C_in=Cin[:m].copy())
+    assert np.array_equal(Ch[:m], want)
+    assert np.array_equal(Ch[m:], Cin[m:])
+    assert B.ozaki2_sgemm_host(m, n, k, 0.5, Ah, lda, Bh, ldb, 1.5, Ch, ldc, N, mode, scratch, 16) == -14
+    assert "14" in B.ozaki2_status_string(-14)

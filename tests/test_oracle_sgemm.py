@@ -92,3 +92,26 @@ def test_accuracy_reaches_fp32_level_with_few_moduli():
     errs = {N: np.max(np.abs(O.sgemm(A, B, N, PROP).astype(np.float64) - ref) / np.abs(ref)) for N in (4, 6, 8, 10)}
     assert errs[4] > 10 * errs[6] > 10 * errs[8]
     assert errs[10] <= 2.0 ** -24
+
+
+def test_unscale_f32_is_rn32_of_the_scaled_integer_then_fp32_alpha_beta():
+    # the FP32 tail on its own (used by the GPU CRT boundary tests): RN_32(z 2^-(e+f)) from exact rationals,
+    # then t = RN_32(alpha c), out = RN_32(beta C_in + t) (fmaf)
+    rng = np.random.Generator(np.random.PCG64(17))
+    n, m = 3, 7
+    zs = [[int(rng.integers(-2 ** 62, 2 ** 62)) * (1 << int(rng.integers(0, 60))) + int(rng.integers(-5, 5)) for _ in range(m)]
+          for _ in range(n)]
+    Cpp = np.stack([np.stack([O.int_to_words(z) for z in row]) for row in zs])
+    e = rng.integers(20, 90, size=m).astype(np.int32)
+    f = rng.integers(20, 90, size=n).astype(np.int32)
+    got = O.unscale_f32(Cpp, e, f)
+    assert np.all(np.isfinite(got))
+    for j in range(n):
+        for i in range(m):
+            assert got[i, j] == rn32(Fraction(zs[j][i]) / Fraction(2) ** (int(e[i]) + int(f[j]))), (i, j)
+    Cin = rng.standard_normal((m, n)).astype(np.float32)
+    out = O.unscale_f32(Cpp, e, f, alpha=0.75, beta=-1.5, C_in=Cin)
+    for j in range(n):
+        for i in range(m):
+            t = rn32(Fraction(0.75) * Fraction(float(got[i, j])))
+            assert out[i, j] == rn32(Fraction(-1.5) * Fraction(float(Cin[i, j])) + Fraction(float(t))), (i, j)
