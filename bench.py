@@ -1,16 +1,28 @@
 #!/usr/bin/env python
-"""bench.py -- emulated FP64 TFLOPS (2mnk/t) of ozaki2_dgemm on BASELINE.json configs[2] (8192^3, eq. (15) inputs
-with phi = 0.5, N = 14..18 moduli, revised fast mode), one JSON line on stdout.
+"""bench.py -- emulated FP64 TFLOPS (2mnk/t, eq. (19)) of ozaki2_dgemm on the BASELINE.json workloads, one JSON
+line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--moduli 16] [--mode 2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4] [--moduli 16] [--mode 2]
+                    [--protocol paper] [--impl reference]
+
+Workload (default): BASELINE configs[2], m = n = k = 8192, eq. (15) inputs with phi = 0.5, N = 16 moduli, revised
+fast mode.  --config 3: 16384^3, phi = 4 (default N = 20); --config 4: 4096 x 4096 x 65536, phi = 1 (default N = 16).
 
 A "step" is one pass of the whole hot path S1..S5 (one ozaki2_dgemm call) over one pair of synthetic matrices.
-`value` is measured with A, B, C resident in HBM; `e2e` goes through ozaki2_dgemm_host with pinned HOST buffers
-(H2D of A and B and D2H of C inside the timed region).  `roofline` is for the dominant kernel, the batched
-tcgen05 INT8 GEMM (S3), timed live with CUDA events that the library records on the launching stream at the
-stage boundaries of every timed step; `stages` carries the same for the HBM-bound stages; `path` is the
-north-star roofline max(N 2mnk / INT8 peak, bytes / HBM bandwidth) over the whole step.  `cpu_baseline` is the
-oracle as it stands, timed on this box's host cores on a bounded slab of the same workload.
+Timing follows the paper's protocol: every step is bracketed by CUDA events that the library records on
+the launching stream, `ms_per_step` is the MEDIAN over the K timed steps and `value` = 2mnk / that median; the mean
+over the whole timed region (one event pair around all K steps, barrier + synchronize on both sides, max over ranks)
+is printed beside it.  `--protocol paper` sets the paper's iteration caps (warm-up until 3 s or 100 iterations,
+timed until 12 s or 100).  `value` is measured with A, B, C resident in HBM; `e2e` goes through ozaki2_dgemm_host
+with pinned HOST buffers (H2D of A and B and D2H of C inside the timed region).
+
+`roofline` is for the dominant kernel, the batched tcgen05 INT8 GEMM (S3): achieved = N 2mnk / its median launch
+duration (stage events); peak = 2 x the measured bf16 BURST figure of MEASURED_PEAKS.json (a step is milliseconds
+long, not seconds), with the sustained and nominal figures and a ceiling measured in this very process -- the same
+kernel with its epilogue reduced to handing the accumulator back, on random and on all-zero residue planes --
+beside it.  `stages` carries ms, algorithmic bytes and GB/s against the measured HBM bandwidth for the streaming
+stages; `path` is the north-star figure max(N 2mnk / INT8 peak, bytes / HBM bandwidth) / step time with the same peak.
+`cpu_baseline` is the oracle as it stands, timed on this box's host cores on a bounded slab of the same workload.
 
 Multi-GPU: replicas only -- every rank runs the same-shaped problem on its own GPU, no collective on
 the data path; `value` is the aggregate.  `--impl reference` times the CPU oracle (rank 0 only).
@@ -35,6 +47,8 @@ if ROOT not in sys.path:
 MODE_NAMES = {0: "accurate", 1: "fast", 2: "prop"}
 NOMINAL_INT8_TOPS = 4500.0          # P:30 (B200 spec sheet, dense)
 INT8_OVER_BF16 = 2.0                # guide's nominal ratio 4.5 / 2.25 PFLOP/s
+DEFAULT_MODULI = {2: 16, 3: 20, 4: 16}
+TRAFFIC_CSV = os.path.join("profiles", "r02_dram_traffic.csv")      # ncu dram bytes per launch, see the .md beside it
 
 
 def parse_args():
@@ -43,14 +57,36 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--moduli", type=int, default=16, help="number of moduli N (BASELINE configs[2]: 14..18)")
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4], help="BASELINE.json configs[] index")
+    ap.add_argument("--moduli", type=int, default=0, help="number of moduli N (default: 16 / 20 / 16 for config 2 / 3 / 4)")
     ap.add_argument("--mode", type=int, default=2, help="0 accurate, 1 original fast, 2 revised fast (headline)")
-    ap.add_argument("--size", type=int, default=8192, help="m = n = k (8192 is the BASELINE workload)")
-    ap.add_argument("--sgemm", action="store_true", help="SURVEY 8(f) #1: the FP32 in / FP32 out variant (paper: N = 3..12); "
-                    "no host-buffer entry point exists for it, so e2e is null")
+    ap.add_argument("--size", type=int, default=0, help="m = n = k override (keeps the config's distribution)")
+    ap.add_argument("--protocol", default="fixed", choices=["fixed", "paper"],
+                    help="paper: P:387-392 iteration caps (warm-up 3 s / 100, timed 12 s / 100) instead of --steps / --warmup")
+    ap.add_argument("--sgemm", action="store_true", help="SURVEY 8(f) #1: the FP32 in / FP32 out variant (paper: N = 3..12)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: leave out the oracle leg")
-    return ap.parse_args()
+    ap.add_argument("--skip-ceiling", action="store_true", help="profiling runs only: leave out the MMA-only ceiling runs")
+    ap.add_argument("--accuracy", action="store_true", help="add max relative error vs the double-double reference "
+                    "(P:268) on a sampled slab, and max |R_l| on it (INT32 headroom, P:113)")
+    a = ap.parse_args()
+    if not a.moduli:
+        a.moduli = DEFAULT_MODULI[a.config]
+    return a
+
+
+def workload_shape(args):
+    import workloads as W
+    c = W.CONFIGS[args.config]
+    if args.size:
+        return args.size, args.size, args.size, c["phi"]
+    return c["m"], c["n"], c["k"], c["phi"]
+
+
+def workload_name(args, m, n, k, phi, N, mode, f32=False):
+    shape = f"m=n=k={m}" if m == n == k else f"m={m}, n={n}, k={k}"
+    return (f"BASELINE configs[{args.config}]%s: {shape}, eq.(15) phi={phi}, N={N} moduli, mode={MODE_NAMES[mode]}"
+            % (" as SGEMM (SURVEY 8(f) #1)" if f32 else ""))
 
 
 def measured_peaks():
@@ -85,6 +121,11 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.lines.append((time.time(), line))
 
+    def wait_first_sample(self, timeout=10.0):
+        t0 = time.time()
+        while self.proc is not None and not self.lines and time.time() - t0 < timeout:
+            time.sleep(0.02)
+
     def stop(self):
         if self.proc is None:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
@@ -111,27 +152,29 @@ class ClockSampler:
                     reasons.add(nm)
         if not sm:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
-        return dict(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), power_w_max=max(pw), samples=len(sm),
+        return dict(sm_mhz=statistics.median(sm), sm_min_mhz=min(sm), sm_max_mhz=max(mx), power_w_max=max(pw),
+                    power_w_median=statistics.median(pw), samples=len(sm), samples_in_timed_region=len(inside),
                     reasons=sorted(reasons))
 
 
-def profiled_traffic(m, N, mode):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), only for
-    the workload that capture was taken on; None otherwise."""
-    path = os.path.join(ROOT, "profiles", "r01c_dram_traffic.csv")
-    if not (os.path.exists(path) and m == 8192 and N == 16 and mode == 2):
+def profiled_traffic(args, m, n, k, N, mode, f32):
+    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (TRAFFIC_CSV; the .md
+    beside it names the command and the commit it was taken at), only for the workload of that capture."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not (os.path.exists(path) and (m, n, k) == (8192, 8192, 8192) and N == 16 and mode == 2 and not f32):
         return None
     with open(path) as fh:
         for line in fh:
-            if line.startswith('"k3_residue_gemm<0>"'):
+            if line.startswith('"k3_residue_gemm'):
                 return float(line.rsplit(",", 1)[1])
     return None
 
 
 def cpu_slab_shape(m, n, k):
-    """Bounded sample of the workload for the oracle: 512 rows of A against 4096 columns of B at the full k
-    (about 15 s on the GPU box's 16 host threads at k = 8192, N = 16)."""
-    return min(m, 512), min(n, 4096), k
+    """Bounded sample of the workload for the oracle: about 1.4e11 residue MACs at N = 16, i.e. 512 rows of A against
+    4096 columns of B at k = 8192 (about 7 s on the GPU box's 16 host threads), fewer columns at longer k."""
+    ns = max(256, min(n, 4096 * 8192 // max(k, 1)))
+    return min(m, 512), min(n, ns), k
 
 
 def time_oracle_slab(A, B, N, mode, shape):
@@ -150,11 +193,11 @@ def run_reference(args):
     if rank != 0:
         return 0
     import workloads as W
-    m = n = k = args.size
+    m, n, k, phi = workload_shape(args)
     N, mode = args.moduli, args.mode
     ms, ns, _ = cpu_slab_shape(m, n, k)
     # the slab keeps the workload's distribution: same generator, same phi, shape (ms, ns, k)
-    A, B = W.config_matrices(2, 0, shape=(ms, ns, k))
+    A, B = W.config_matrices(args.config, 0, shape=(ms, ns, k))
     steps, warm = max(1, min(args.steps, 3)), max(0, min(args.warmup, 1))
     threads = 0
     for _ in range(warm):
@@ -163,15 +206,15 @@ def run_reference(args):
     for _ in range(steps):
         _, dt, threads = time_oracle_slab(A, B, N, mode, (ms, ns, k))
         t.append(dt)
-    dt = sum(t) / len(t)
+    dt = statistics.median(t)
     val = 2.0 * ms * ns * k / dt / 1e12
-    sample = f"oracle dgemm on a {ms}x{ns}x{k} slab (eq. 15, phi=0.5) per step; steps capped at 3, warmup at 1"
+    sample = f"oracle dgemm on a {ms}x{ns}x{k} slab (eq. 15, phi={phi}) per step; steps capped at 3, warmup at 1"
     line = dict(impl="reference", metric="emulated_fp64_tflops", value=val, unit="TFLOPS", n_gpus=args.gpus,
                 steps=steps, warmup=warm, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="int8xint8->int32 residues, fp64 in/out (CPU: int64 / 256-bit integers)",
                 data="synthetic",
-                config=dict(workload=f"BASELINE configs[2]: m=n=k={m}, eq.(15) phi=0.5, N={N} moduli, mode={MODE_NAMES[mode]}",
-                            moduli=N, scaling_mode=MODE_NAMES[mode], sample=sample),
+                config=dict(workload=workload_name(args, m, n, k, phi, N, mode), moduli=N, scaling_mode=MODE_NAMES[mode],
+                            sample=sample),
                 cpu_baseline=dict(value=val, unit="TFLOPS", cores=threads, kind="oracle", sample=sample),
                 e2e=dict(value=val, unit="TFLOPS", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
@@ -179,12 +222,47 @@ def run_reference(args):
     return 0
 
 
+def measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=10):
+    """The path's GEMM kernel with the epilogue reduced to handing the accumulator back (ozaki2_debug_residue_gemm,
+    variant 3), on uniform random symmetric residues and on all-zero planes: what this MMA / TMA loop can deliver on
+    this board at the clocks it gets, next to which the mod-p epilogue and the real data are judged."""
+    if k % 128 or m % 16 or k > (1 << 17):
+        return None
+    out = {}
+    RA = torch.empty((N, m, k), dtype=torch.int8, device="cuda")
+    RB = torch.empty((N, n, k), dtype=torch.int8, device="cuda")
+    U = torch.empty((16,), dtype=torch.uint8, device="cuda")          # untouched by variant 3
+    for name in ("random", "zero"):
+        if name == "random":
+            g = torch.Generator(device="cuda")
+            g.manual_seed(29129)
+            for t in (RA, RB):
+                for l in range(N):                                     # |r| <= 86 is inside every modulus' symmetric range
+                    t[l].copy_(torch.randint(-86, 87, t[l].shape, dtype=torch.int8, device="cuda", generator=g))
+        else:
+            RA.zero_(); RB.zero_()
+        for _ in range(3):
+            rc = pkg.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, U, 3, stream)
+            if rc:
+                raise pkg.Ozaki2Error(rc, "ozaki2_debug_residue_gemm(3)")
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+        evs[0].record(stream)
+        for r in range(reps):
+            pkg.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, U, 3, stream)
+            evs[r + 1].record(stream)
+        torch.cuda.synchronize()
+        ms = statistics.median(evs[r].elapsed_time(evs[r + 1]) for r in range(reps))
+        out[name] = dict(tops=N * 2.0 * m * n * k / (ms * 1e-3) / 1e12, ms=ms)
+    del RA, RB
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
 
-    import numpy as np
     import torch
     import torch.distributed as dist
 
@@ -203,13 +281,13 @@ def main():
     pkg.lib()
     peaks = measured_peaks()
 
-    m = n = k = args.size
+    m, n, k, phi = workload_shape(args)
     N, mode = args.moduli, args.mode
     K, Wm = args.steps, max(args.warmup, 3)
     flops = 2.0 * m * n * k
 
     # ---- inputs: eq. (15), seeded, one variant per rank (replicas)
-    A, B = W.config_matrices(2, rank, shape=(m, n, k))
+    A, B = W.config_matrices(args.config, rank, shape=(m, n, k))
     f32 = bool(args.sgemm)
     npdt, tdt, esz = (np.float32, torch.float32, 4) if f32 else (np.float64, torch.float64, 8)
     if f32:
@@ -232,7 +310,17 @@ def main():
         if rc:
             raise pkg.Ozaki2Error(rc, "ozaki2_dgemm")
 
-    for _ in range(Wm):
+    sampler = ClockSampler(local)
+    sampler.start()                       # nvidia-smi takes a moment to come up: started before the warm-up
+    for _ in range(3):
+        step()
+    if args.protocol == "paper":          # warm-up until 3 s or 100 iterations, timed until 12 s or 100 (>= 5)
+        t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+        t0.record(stream); step(); t1.record(stream); torch.cuda.synchronize()
+        est = max(t0.elapsed_time(t1) * 1e-3, 1e-6)
+        Wm = int(max(3, min(100, 3.0 / est)))
+        K = int(max(5, min(100, 12.0 / est)))
+    for _ in range(max(0, Wm - 3)):
         step()
     # stage events: created by one record each (torch creates lazily), re-recorded by the library
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(K)]
@@ -240,10 +328,7 @@ def main():
         for ev in row:
             ev.record(stream)
     t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local)
-    sampler.start()                       # nvidia-smi takes a moment to come up: started before the last warm-ups
-    for _ in range(2):
-        step()
+    sampler.wait_first_sample()
     barrier()
     launches0 = pkg.ozaki2_kernel_launches()
     sampler.window[0] = time.time()
@@ -256,27 +341,38 @@ def main():
     launches = pkg.ozaki2_kernel_launches() - launches0
     clocks = sampler.stop()
     total_ms = t0.elapsed_time(t1)
+    step_ms = [evs[s][0].elapsed_time(evs[s][4]) for s in range(K)]
+    med_ms = statistics.median(step_ms)
     if world > 1:
-        tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        tt = torch.tensor([total_ms, med_ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
-    ms_per_step = total_ms / K
-    value = world * flops / (ms_per_step * 1e-3) / 1e12
+        total_ms, med_ms = float(tt[0].item()), float(tt[1].item())
+    mean_ms = total_ms / K
+    value = world * flops / (med_ms * 1e-3) / 1e12
 
-    stage_ms = [statistics.fmean(evs[s][t].elapsed_time(evs[s][t + 1]) for s in range(K)) for t in range(4)]
+    stage_ms = [statistics.median(evs[s][t].elapsed_time(evs[s][t + 1]) for s in range(K)) for t in range(4)]
     X, Y = float(m) * k + float(k) * n, float(m) * n
     # algorithmic work per launch / stage
-    s3_ops = N * flops + (flops if mode == 0 else 0.0)
-    int8_peak = INT8_OVER_BF16 * peaks["bf16_sustained"]
-    s3_ms = stage_ms[2] if mode != 0 else stage_ms[2]            # mode 0: the auxiliary GEMM sits in S1
+    s3_ops = N * flops + (flops if mode == 0 else 0.0)          # mode 0: the auxiliary GEMM sits in S1
+    int8_peak = INT8_OVER_BF16 * peaks["bf16"]
+    s3_ms = stage_ms[2]
     achieved = N * flops / (s3_ms * 1e-3) / 1e12
-    roofline = dict(bound="tensor", kernel="k3_residue_gemm<false> (tcgen05.mma kind::i8, batched over N moduli)",
+    ceiling = None
+    if not args.skip_ceiling and not f32:
+        ceiling = measure_int8_ceiling(pkg, torch, m, n, k, N, stream)
+    roofline = dict(bound="tensor", kernel="k3_residue_gemm<EPI_MODP> (tcgen05.mma kind::i8, batched over N moduli)",
                     achieved=achieved, peak=int8_peak, unit="TFLOP/s", frac=achieved / int8_peak,
-                    peak_source=f"2 x bf16_tflops_sustained ({peaks['source']}); INT8 has no measured entry",
-                    frac_of_burst=achieved / (INT8_OVER_BF16 * peaks["bf16"]),
+                    peak_source=f"2 x bf16_tflops burst ({peaks['source']}): another dtype's measured peak x the nominal "
+                                "ratio 4.5 / 2.25; MEASURED_PEAKS.json has no INT8 entry",
+                    frac_of_2x_sustained=achieved / (INT8_OVER_BF16 * peaks["bf16_sustained"]),
                     frac_of_nominal_4500=achieved / NOMINAL_INT8_TOPS, ms_per_launch=s3_ms,
-                    traffic=profiled_traffic(m, N, mode), traffic_unit="bytes per launch (ncu dram read + write, profiles/r01c)",
+                    int8_ceiling_tops=ceiling,
+                    frac_of_ceiling_random=(achieved / ceiling["random"]["tops"]) if ceiling else None,
+                    traffic=profiled_traffic(args, m, n, k, N, mode, f32),
+                    traffic_unit=f"bytes per launch (ncu dram read + write, {TRAFFIC_CSV})",
                     algorithmic_bytes=N * X + N * Y)
+    if roofline["frac"] > 1.0:
+        roofline["note"] = "frac > 1: the kernel beats 2 x the cuBLAS bf16 burst figure; see int8_ceiling_tops"
     stage_bytes = [esz * X if mode != 0 else esz * X + 2 * X, (esz + N) * X, N * X + N * Y, (N + esz) * Y]
     stages = {}
     for nm, ms_, by in zip(("S1_scaling", "S2_conversion", "S3_residue_gemm", "S4S5_crt_unscale"), stage_ms, stage_bytes):
@@ -284,53 +380,55 @@ def main():
                           hbm_frac=by / (ms_ * 1e-3) / 1e9 / peaks["hbm_gbs"])
     stages["S3_residue_gemm"]["int8_tops"] = achieved
     total_bytes = (2 * esz + 2 * N) * X + (2 * N + esz) * Y
-    t_roof_ms = max(s3_ops / (int8_peak * 1e12), total_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
-    t_roof_nominal_ms = max(s3_ops / (NOMINAL_INT8_TOPS * 1e12), total_bytes / (peaks["hbm_gbs"] * 1e9)) * 1e3
-    path = dict(roofline_ms=t_roof_ms, frac=t_roof_ms / ms_per_step, roofline_ms_nominal_4500=t_roof_nominal_ms,
-                frac_nominal_4500=t_roof_nominal_ms / ms_per_step, total_algorithmic_gb=total_bytes / 1e9,
-                int8_ops=s3_ops)
+    t_hbm_ms = total_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
+    t_roof_ms = max(s3_ops / (int8_peak * 1e12) * 1e3, t_hbm_ms)
+    t_roof_nominal_ms = max(s3_ops / (NOMINAL_INT8_TOPS * 1e12) * 1e3, t_hbm_ms)
+    path = dict(roofline_ms=t_roof_ms, frac=t_roof_ms / med_ms, peak_tops=int8_peak, roofline_ms_nominal_4500=t_roof_nominal_ms,
+                frac_nominal_4500=t_roof_nominal_ms / med_ms, hbm_ms=t_hbm_ms, total_algorithmic_gb=total_bytes / 1e9,
+                int8_ops=s3_ops, stage_sum_ms=sum(stage_ms))
 
-    # ---- e2e: host buffers through ozaki2_dgemm_host (pinned), copies inside the timed region
+    # ---- e2e: host buffers through ozaki2_dgemm_host / ozaki2_sgemm_host (pinned), copies inside the timed region
     e2e = None
-    if not args.skip_e2e and not f32:
-        Ah = torch.empty((k, m), dtype=torch.float64, pin_memory=True)
-        Bh = torch.empty((n, k), dtype=torch.float64, pin_memory=True)
-        Ch = torch.empty((n, m), dtype=torch.float64, pin_memory=True)
+    if not args.skip_e2e:
+        Ah = torch.empty((k, m), dtype=tdt, pin_memory=True)
+        Bh = torch.empty((n, k), dtype=tdt, pin_memory=True)
+        Ch = torch.empty((n, m), dtype=tdt, pin_memory=True)
         Ah.numpy()[...] = A.T
         Bh.numpy()[...] = B.T
         nbytes = pkg.ozaki2_host_scratch_bytes(m, n, k)
         scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
         Ke = max(1, min(K, 5))
+        host_call = pkg.ozaki2_sgemm_host if f32 else pkg.ozaki2_dgemm_host
 
         def host_step():
-            rc = pkg.ozaki2_dgemm_host(m, n, k, 1.0, Ah.data_ptr(), m, Bh.data_ptr(), k, 0.0, Ch.data_ptr(), m, N, mode,
-                                       scratch, nbytes, stream)
+            rc = host_call(m, n, k, 1.0, Ah.data_ptr(), m, Bh.data_ptr(), k, 0.0, Ch.data_ptr(), m, N, mode, scratch, nbytes,
+                           stream)
             if rc:
                 raise pkg.Ozaki2Error(rc, "ozaki2_dgemm_host")
 
         host_step()
         barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(Ke):
+        ee = [torch.cuda.Event(enable_timing=True) for _ in range(Ke + 1)]
+        ee[0].record(stream)
+        for r in range(Ke):
             host_step()
-        e1.record(stream)
+            ee[r + 1].record(stream)
         barrier()
-        e_ms = e0.elapsed_time(e1) / Ke
+        e_ms = statistics.median(ee[r].elapsed_time(ee[r + 1]) for r in range(Ke))
         if world > 1:
             tt = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             e_ms = float(tt.item())
         e2e = dict(value=world * flops / (e_ms * 1e-3) / 1e12, unit="TFLOPS", ms_per_step=e_ms, steps=Ke,
-                   h2d_bytes_per_step=int(8 * X), d2h_bytes_per_step=int(8 * Y),
-                   api="ozaki2_dgemm_host (pinned host A, B, C)")
+                   h2d_bytes_per_step=int(esz * X), d2h_bytes_per_step=int(esz * Y),
+                   api="ozaki2_%sgemm_host (pinned host A, B, C)" % ("s" if f32 else "d"))
         # the host-buffer result must be the device-resident one
-        same = bool(torch.equal(Ch.cuda(), Cd))
-        e2e["matches_device_path"] = same
+        e2e["matches_device_path"] = bool(torch.equal(Ch.cuda(), Cd))
         del scratch
 
     # ---- cpu_baseline: the oracle on a slab of the same matrices (rank 0, N = 1 only), compared with the GPU's C
     cpu = None
+    accuracy = None
     if rank == 0 and world == 1 and not args.skip_cpu_baseline:
         ms_, ns_, _ = cpu_slab_shape(m, n, k)
         Cs, dt, threads = time_oracle_slab(A, B, N, mode, (ms_, ns_, k))
@@ -340,20 +438,42 @@ def main():
         if mode != 0:       # e_i, f_j of modes 1, 2 depend on their own row / column only: the slab of C is comparable
             Cg = Cd[:ns_, :ms_].cpu().numpy().T
             cpu["gpu_slab_bit_exact_vs_oracle"] = bool(np.array_equal(Cg, Cs))
+    if rank == 0 and world == 1 and args.accuracy and not f32:
+        # max elementwise relative error against a double-double reference, on a sampled slab of the GPU's C
+        from oracle import ozaki2_oracle as O
+        ra, ca = min(m, 256), min(n, 512)
+        hi, lo = O.dd_reference(np.asfortranarray(A[:ra, :]), np.asfortranarray(B[:, :ca]))
+        Cg = Cd[:ca, :ra].cpu().numpy().T
+        nz = hi != 0
+        accuracy = dict(max_rel_err=float(np.max(np.abs((Cg[nz] - hi[nz]) - lo[nz]) / np.abs(hi[nz]))),
+                        sample=f"rows 0..{ra - 1} x columns 0..{ca - 1} of C vs oracle double-double AB",
+                        zero_reference_entries=int(np.sum(~nz)))
+        if mode != 0:
+            g = pkg.dgemm_stages(Ad, Bd, N, mode, C_dev=Cd, want=("e", "f"))
+            torch.cuda.synchronize()
+            e, f = g["e"].cpu().numpy(), g["f"].cpu().numpy()
+            rr, cc = min(m, 32), min(n, 64)
+            RA = O.residues(0, N, np.asfortranarray(A[:rr, :]), e[:rr])
+            RB = O.residues(1, N, np.asfortranarray(B[:, :cc]), f[:cc])
+            _, maxR = O.products(N, RA, RB)
+            accuracy["max_abs_residue_product"] = int(maxR)
+            accuracy["int32_headroom_bits"] = float(31 - np.log2(max(maxR, 1)))
 
     if rank == 0:
         line = dict(metric="emulated_fp32_tflops" if f32 else "emulated_fp64_tflops", value=value, unit="TFLOPS",
-                    n_gpus=world, steps=K, warmup=Wm,
-                    ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    n_gpus=world, steps=K, warmup=Wm, ms_per_step=med_ms, ms_per_step_stat="median of the K timed steps "
+                    "(P:387-392); ms_per_step_mean = one event pair around all K steps / K", ms_per_step_mean=mean_ms,
+                    value_mean=world * flops / (mean_ms * 1e-3) / 1e12, ms_per_step_min=min(step_ms), ms_per_step_max=max(step_ms),
+                    higher_is_better=True, scaling="weak", vs_baseline=None,
                     dtype="int8xint8->int32 (tcgen05 kind::i8), %s in/out" % ("fp32" if f32 else "fp64"), data="synthetic",
-                    config=dict(workload=f"BASELINE configs[2]%s: m=n=k={m}, eq.(15) phi=0.5, N={N} moduli, "
-                                         f"mode={MODE_NAMES[mode]}" % (" as SGEMM (SURVEY 8(f) #1)" if f32 else ""),
-                                moduli=N, scaling_mode=MODE_NAMES[mode],
+                    config=dict(workload=workload_name(args, m, n, k, phi, N, mode, f32), moduli=N, scaling_mode=MODE_NAMES[mode],
+                                protocol=args.protocol,
                                 l2="inputs larger than L2 (A + B = %.2f GB per step, residue planes %.2f GB)" %
                                    (esz * X / 1e9, N * X / 1e9), parallelism="replicas" if world > 1 else "single GPU"),
                     clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, stages=stages, path=path,
-                    cpu_baseline=cpu, peaks=dict(hbm_gbs=peaks["hbm_gbs"], bf16_tflops=peaks["bf16"],
-                                                 bf16_tflops_sustained=peaks["bf16_sustained"], source=peaks["source"]),
+                    cpu_baseline=cpu, accuracy=accuracy,
+                    peaks=dict(hbm_gbs=peaks["hbm_gbs"], bf16_tflops=peaks["bf16"],
+                               bf16_tflops_sustained=peaks["bf16_sustained"], source=peaks["source"]),
                     context="paper (GH200): cuBLAS DGEMM 60.9 TFLOPS, Ozaki-II DGEMM up to 80.2 TFLOPS (P:48); "
                             "FP64 tensor peak 67 (GH200) / 37 (B200) TFLOPS (P:30)")
         print(json.dumps(line))
