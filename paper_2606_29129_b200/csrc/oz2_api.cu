@@ -231,12 +231,13 @@ Layout make_layout(int64_t m, int64_t n, int64_t k, int N, int mode)
     return L;
 }
 
-// widths: fast / prop  <= floor(P'_prop) + 1 bits, accurate <= floor(P'_accu) + 7 bits; two words hold |a'| < 2^64
+// widths: fast / prop  <= floor(P'_prop) + 1 bits, accurate <= floor(P'_accu) + 7 bits; the narrow conversion format
+// holds a' as a signed 64-bit integer, |a'| < 2^63
 bool needs_wide_words(int N, int mode)
 {
     const float Pp = host_consts().tab.crt[N].Pprop;
     const int width = (int)floorf(Pp) + (mode == OZAKI2_MODE_ACCURATE ? 7 : 1);
-    return width > 64;
+    return width > 63;
 }
 
 int check_args(int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B, int64_t ldb,
@@ -738,10 +739,11 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
     if (k <= 0 || k % 128 != 0 || k > OZAKI2_MAX_K) return -4;      // canonical planes are used in place: pitch = k
     if (m % 16 != 0) return -2;                                     // U pitch = m
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (use_tensor_cores < 0 || use_tensor_cores > 3) return -8;
+    if (use_tensor_cores < 0 || use_tensor_cores > 4) return -8;
     if (use_tensor_cores) {
         // 1: one CTA per tile (the ozaki2_dgemm path), 2: CTA pairs, 3: the path kernel without its epilogue
-        const int variant = use_tensor_cores == 2 ? OZ2_GEMM_PAIR : use_tensor_cores == 3 ? OZ2_GEMM_MMA_ONLY : OZ2_GEMM_PATH;
+        const int variant = use_tensor_cores == 2 ? OZ2_GEMM_PAIR : use_tensor_cores == 3 ? OZ2_GEMM_MMA_ONLY
+                            : use_tensor_cores == 4 ? OZ2_GEMM_PAIR_MMA_ONLY : OZ2_GEMM_PATH;
         return oz2_launch_gemm_tc(variant, num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);
     }
     return oz2_launch_gemm_check(num_moduli, m, n, k, resA, resB, k, U, m, st);

@@ -68,7 +68,7 @@ int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k
 // S3: batched INT8 GEMM with mod-p epilogue (tcgen05).  nplanes GEMMs; modulus index of plane b is mod_base + b.
 // U: [plane][n][mp].  If rowmax/colmax != NULL the epilogue keeps maxima instead (accurate mode).
 // variant: OZ2_GEMM_PATH (what ozaki2_dgemm runs), OZ2_GEMM_PAIR (cta_group::2 alternative), OZ2_GEMM_MMA_ONLY (no epilogue)
-enum { OZ2_GEMM_PATH = 0, OZ2_GEMM_PAIR = 1, OZ2_GEMM_MMA_ONLY = 2 };
+enum { OZ2_GEMM_PATH = 0, OZ2_GEMM_PAIR = 1, OZ2_GEMM_MMA_ONLY = 2, OZ2_GEMM_PAIR_MMA_ONLY = 3 };
 int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA,
                        const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st);
 int oz2_launch_gemm_check(int nplanes, int64_t m, int64_t n, int64_t k, const int8_t *RA, const int8_t *RB, int64_t kp,

@@ -1,44 +1,109 @@
 // oz2_convert.cu -- S2: A' = trunc(diag(mu) A), B' = trunc(B diag(nu)) (Step 2) and the symmetric
 // INT8 residues rmod(., p_l) for all N moduli in ONE pass over A and B.
 //
-// Arithmetic.  |a'| (up to 84 bits, never written to memory) lives in registers as NB 32-bit words.  With d_i the
-// base-256 digits of |a'|, for an odd modulus p
-//     x = sum_i d_i (256^i mod p)                                       (NB dp4a; x < 2^20, congruent to |a'|)
-// and the symmetric residue is r = sign(a') (x - p round(x / p)).  The reduction runs in FP32 on exact small
-// integers, so that it can use both halves of the FMA pipe (integer multiplies only run on one):
-//     the dp4a chain starts from 0x4B000000, the bit pattern of 2^23, so its result read as a float is 2^23 + x;
-//     q = RN(x (1/p)~ + 1.5 2^23) - 1.5 2^23 is round(x / p) exactly: |x (1/p)~ - x/p| < 2^-11, while x / p is at
-//     least 1/(2p) > 2^-9 away from every half-integer (p odd);
-//     x - q p is then exact, and RN(sign (x - q p) + 1.5 2^23) holds r in two's complement in its low byte.
-// p = 256: the low byte of a' in two's complement (reading R5).
+// The reduction of an up-to-84-bit integer modulo N small moduli is a dense contraction, so it runs on the tensor
+// cores: with d_i the base-256 digits of a non-negative image a'' of a',
+//     a'' = sum_i d_i 256^i      =>      a'' mod p_l  =  ( sum_i d_i (256^i mod p_l) ) mod p_l ,
+// i.e. (elements x digits) x (digits x moduli).  One tcgen05.mma kind::i8 (unsigned x unsigned, M = 128, K = 32,
+// N = up to 64) handles 128 "quads" = 512 elements: a K row of 32 bytes carries the 8-byte digit strings of the 4
+// consecutive elements of a quad side by side (two 16-byte strings when |a'| needs more than 63 bits), and the B
+// operand is a constant block-diagonal image of the byte weights 256^i mod p_l, so that accumulator column
+// (l, slot) holds  Y = sum_i d_i(slot) (256^i mod p_l) < 2^20.  A second MMA with a constant all-ones operand adds a
+// per-modulus bias.  What is left for the CUDA cores is 2 multiplies per element and modulus and a packed store:
+//     a''  = a' + 2^63 (two's complement of a' with the top bit flipped: non-negative, sign handled for free),
+//     bias = (p-1)/2 - 2^63 mod p,  Y ~ a' + (p-1)/2 (mod p),  u = Y mod p = Y - umulhi(Y, magic) p  in [0, p),
+//     r    = u - (p-1)/2  in [-(p-1)/2, (p-1)/2]  is the symmetric residue (reading R5 for p = 256, where the
+//     byte is simply the low byte of a'); four u bytes are packed, the per-byte offset 128 - (p-1)/2 is added to the
+//     packed word (no carries: u + 128 - (p-1)/2 <= 255) and 0x80808080 is XORed to give the four INT8 values.
+// trunc(a 2^e) is one exponent-field addition and one FP64 -> INT64 conversion (round toward zero, exact because
+// |a'| < 2^63); subnormal inputs and the wide (N >= 17 or accurate-mode) format take integer shifts.
 //
-// Data movement (the stage is bound by HBM traffic 8 + N bytes per element and by ~7 integer instructions per
-// element and modulus).  Planes are [l][row][kp], k fastest (K-major for the tensor-core GEMM),
-// kp = round_up(k, 128), zero padded.  Work unit everywhere: a "quad" = 4 consecutive h of one row, held by one
-// lane, so that a warp stores 128 contiguous bytes per row and modulus.
-//   * B is column-major = already K-major: a warp streams 256 consecutive h of one column with 16-byte loads.
-//   * A is column-major = M-major: a CTA stages a 32-row x 128-h tile through shared memory (coalesced 256-byte
-//     reads along the rows, transposed on the way in), then every warp converts whole rows of the tile.
-// The same two movers serve accurate mode's Abar / Bbar = ceil(mu' |.|), one plane.
+// Data movement (the stage is bound by HBM traffic 8 + N bytes per element).  Planes are [l][row][kp], k fastest
+// (K-major for the GEMM), kp = round_up(k, 128), zero padded.  A thread owns a quad (4 consecutive h of one vector)
+// from the global load to the 4-byte store, so a warp stores 128 contiguous bytes per modulus.
+//   * contiguous vectors (columns of B, or rows of A^T): 32-byte loads straight from global memory;
+//   * strided vectors (rows of a column-major A): a CTA brings 16 rows x 64 h into shared memory with cp.async
+//     (128-byte coalesced reads along the rows, transposed on the way in, double buffered).
+// The same two movers, without the tensor-core part, serve accurate mode's Abar / Bbar = ceil(mu' |.|).
 #include "oz2_common.cuh"
+#include "oz2_tc.cuh"
 
 namespace {
 
-struct ConvTab {
-    float invp, negp;          // RN(1 / p), -p
-    uint32_t wb[3];            // byte weights 256^(4t+b) mod p, packed
-    uint32_t pad[3];
-};
-__constant__ ConvTab c_conv[OZ2_MAX_MODULI];
+// eq. (14), P:252-255 as compile-time constants (the epilogue is fully unrolled over the moduli)
+__host__ __device__ constexpr uint32_t modulus_of(int l)
+{
+    constexpr uint32_t t[OZ2_MAX_MODULI] = OZ2_MODULI_LIST;
+    return t[l];
+}
 
-constexpr int TI = 32;             // rows of A per tile
-constexpr int TH = 128;            // h per tile
-constexpr int SROW = TH + 2;       // padded row of the staging tile in doubles (16-byte aligned rows)
-constexpr int CONV_THREADS = 256;
+constexpr int CV_THREADS = 128;                    // one MMA tile row (quad) per thread
+constexpr int CV_TILE_BYTES = 128 * 32;            // A operand: 128 rows x 32 K bytes
+constexpr int CV_IMG_BYTES = 64 * 32;              // B operand: 64 columns x 32 K bytes
+constexpr int CV_ONES_BYTES = 256;                 // all-ones A operand of the bias MMA: one 8-row group, re-read for all 16 (SBO = 0)
+constexpr int CV_TMEM_COLS = 64;
+constexpr int CV_CHUNK_H = 4 * CV_THREADS;         // contiguous side: h per round
 
-// magnitude words of trunc(|a| 2^ex); returns the sign mask of a (0 or 0xFFFFFFFF)
-template <int NB>
-__device__ __forceinline__ uint32_t scaled_words(double a, int ex, uint32_t (&w)[NB])
+// operand images: [wide][0: byte weights, 1: bias][2048], canonical no-swizzle K-major layout (see tile_off)
+__device__ uint8_t g_conv_img[2][2][CV_IMG_BYTES];
+
+// byte offset of (row r, K byte kb) in a K-major, no-swizzle operand: 8 x 16-byte core matrices,
+// K-direction core-matrix stride (LBO) 128 B, 8-row group stride (SBO) 256 B
+__host__ __device__ constexpr int tile_off(int r, int kb) { return (r >> 3) * 256 + (kb >> 4) * 128 + (r & 7) * 16 + (kb & 15); }
+
+__device__ __forceinline__ uint64_t kmajor_desc(uint32_t saddr, uint32_t sbo)
+{
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(128u >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
+}
+
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// trunc(a 2^ex)
+// ---------------------------------------------------------------------------------------------
+// zero / subnormal input (rare): integer shifts of the 52-bit mantissa; value = +-M 2^(ex - 1074)
+__device__ __noinline__ long long trunc_subnormal(long long bits, int ex)
+{
+    const unsigned long long M = (unsigned long long)bits & 0x000FFFFFFFFFFFFFull;
+    const int sh = ex - 1074;
+    unsigned long long mag;
+    if (sh >= 0) mag = M << (sh > 63 ? 63 : sh);
+    else mag = (-sh < 64) ? (M >> (-sh)) : 0ull;
+    return bits < 0 ? -(long long)mag : (long long)mag;
+}
+
+// narrow format: |a'| < 2^63.  Returns a' + 2^63 as an unsigned 64-bit integer (its bytes are the 8 digits).
+__device__ __forceinline__ unsigned long long digits_narrow(double a, int ex)
+{
+    const long long bits = __double_as_longlong(a);
+    const int hi = (int)(bits >> 32);
+    const int be = (hi >> 20) & 0x7FF;
+    long long t;
+    if (be == 0) {
+        t = (bits << 1) == 0 ? 0ll : trunc_subnormal(bits, ex);
+    } else {
+        const int ne = be + ex;                                   // biased exponent of a 2^ex
+        const double x = __hiloint2double(hi + ex * 1048576, (int)bits);
+        t = ne < 1023 ? 0ll : __double2ll_rz(x);                  // |a 2^ex| < 1 truncates to 0; else exact (< 2^63)
+    }
+    return (unsigned long long)t ^ 0x8000000000000000ull;
+}
+
+// wide format: |a'| < 2^95 as three 32-bit words of a' + 2^95 (two's complement, top bit flipped)
+__device__ __forceinline__ void digits_wide(double a, int ex, uint32_t (&w)[3])
 {
     const unsigned long long b = (unsigned long long)__double_as_longlong(a);
     const uint32_t hi = (uint32_t)(b >> 32), lo = (uint32_t)b;
@@ -46,81 +111,441 @@ __device__ __forceinline__ uint32_t scaled_words(double a, int ex, uint32_t (&w)
     const int be = (int)((hi >> 20) & 0x7FFu);
     const uint32_t m1 = (hi & 0x000FFFFFu) | (be ? 0x00100000u : 0u), m0 = lo;
     const unsigned long long M = ((unsigned long long)m1 << 32) | m0;
-    const int sh = (be ? be : 1) - 1075 + ex;          // |a| 2^ex = M 2^sh, M < 2^53
-    if (NB == 2) {
-        // |a'| < 2^64: a non-zero M is shifted left by at most 63
-        unsigned long long v;
-        if (sh >= 0) v = M << (sh > 63 ? 63 : sh);
-        else v = (-sh < 64) ? (M >> (-sh)) : 0ull;      // dropping magnitude bits = toward zero
+    const int sh = (be ? be : 1) - 1075 + ex;                     // |a| 2^ex = M 2^sh, M < 2^53
+    if (sh >= 0) {
+        const int s = sh > 95 ? 95 : sh;
+        const int ws = s >> 5, bs = s & 31;
+        const uint32_t t0 = m0 << bs, t1 = __funnelshift_l(m0, m1, bs), t2 = __funnelshift_l(m1, 0u, bs);
+        w[0] = ws == 0 ? t0 : 0u;
+        w[1] = ws == 0 ? t1 : (ws == 1 ? t0 : 0u);
+        w[2] = ws == 0 ? t2 : (ws == 1 ? t1 : t0);
+    } else {
+        const int r = -sh;
+        const unsigned long long v = r < 64 ? (M >> r) : 0ull;    // dropping magnitude bits = toward zero
         w[0] = (uint32_t)v;
         w[1] = (uint32_t)(v >> 32);
-    } else {
-        if (sh >= 0) {
-            // |a'| < 2^96: word shift ws = sh / 32 (<= 2 for a non-zero M), bit shift bs
-            const int s = sh > 95 ? 95 : sh;
-            const int ws = s >> 5, bs = s & 31;
-            const uint32_t t0 = m0 << bs, t1 = __funnelshift_l(m0, m1, bs), t2 = __funnelshift_l(m1, 0u, bs);
-            w[0] = ws == 0 ? t0 : 0u;
-            w[1] = ws == 0 ? t1 : (ws == 1 ? t0 : 0u);
-            w[2] = ws == 0 ? t2 : (ws == 1 ? t1 : t0);
-        } else {
-            const int r = -sh;
-            const unsigned long long v = r < 64 ? (M >> r) : 0ull;
-            w[0] = (uint32_t)v;
-            w[1] = (uint32_t)(v >> 32);
-            w[2] = 0u;
-        }
+        w[2] = 0u;
     }
-    return negm;
+    // two's complement over 96 bits, then + 2^95
+    w[0] ^= negm; w[1] ^= negm; w[2] ^= negm;
+    asm("add.cc.u32 %0, %0, %3;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.u32 %2, %2, 0;"
+        : "+r"(w[0]), "+r"(w[1]), "+r"(w[2]) : "r"(negm & 1u));
+    w[2] ^= 0x80000000u;
 }
 
-// Two quads at once (8 elements, exponents ex0 / ex1): residues for every modulus, one 4-byte store per quad and
-// modulus.  The per-modulus constants are loaded once for the 8 elements; `ok1` guards the second quad's stores.
-template <int NB>
-__device__ __forceinline__ void oct_residues(const double (&a)[2][4], int ex0, int ex1, int N, int8_t *dst0,
-                                             int64_t dst1_off, bool ok1, int64_t plane_stride)
+// ---------------------------------------------------------------------------------------------
+// per-round tensor-core step and epilogue
+// ---------------------------------------------------------------------------------------------
+struct ConvSmem {                                   // dynamic shared memory, 128-byte aligned base
+    uint8_t tile[CV_TILE_BYTES];
+    uint8_t ones[CV_ONES_BYTES];
+    uint8_t imgw[CV_IMG_BYTES];
+    uint8_t imgb[CV_IMG_BYTES];
+    uint64_t mbar;
+    uint32_t tmem_slot;
+    uint32_t pad;
+};
+
+struct ConvCtx {
+    uint32_t tile_row;          // shared address of this thread's 32-byte K row (first 16 bytes; +128 for the rest)
+    uint32_t mbar;              // shared address of the MMA-done barrier
+    uint32_t phase;
+    uint32_t tmem;              // TMEM address of this thread's lane, column 0
+    uint32_t tmem_base;
+    uint64_t adesc, bdesc, odesc, biasdesc;
+    uint32_t idesc;
+};
+
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
 {
-    constexpr float MAGIC = 12582912.0f;               // 1.5 2^23: RN(y + MAGIC) - MAGIC = round(y) for |y| < 2^22
-    uint32_t w[8][NB];
-    float sg[8];                                       // +1.0f / -1.0f
-    uint32_t b256[8];                                  // a' in two's complement, low word
-#pragma unroll
-    for (int u = 0; u < 8; u++) {
-        const uint32_t negm = scaled_words<NB>(a[u >> 2][u & 3], u < 4 ? ex0 : ex1, w[u]);
-        sg[u] = __uint_as_float(0x3F800000u | (negm & 0x80000000u));
-        b256[u] = (w[u][0] ^ negm) - negm;
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+
+// all 128 K rows are in place: run the two MMAs (digits x weights, ones x bias) and wait for the accumulator
+__device__ __forceinline__ void conv_mma(ConvCtx &cx)
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy stores -> tensor-core reads
+    tc_fence_before();                                                // my tcgen05.ld of the previous round is done
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        tc_fence_after();
+        tc_mma_i8(cx.tmem_base, cx.adesc, cx.bdesc, cx.idesc, 0u);
+        tc_mma_i8(cx.tmem_base, cx.odesc, cx.biasdesc, cx.idesc, 1u);
+        tc_commit_a(cx.mbar);
     }
-    int8_t *out = dst0;
-    {   // p = 256: low bytes
-        const uint32_t lo = __byte_perm(b256[0], b256[1], 0x0040), hi = __byte_perm(b256[2], b256[3], 0x0040);
-        *reinterpret_cast<uint32_t *>(out) = __byte_perm(lo, hi, 0x5410);
-        const uint32_t lo1 = __byte_perm(b256[4], b256[5], 0x0040), hi1 = __byte_perm(b256[6], b256[7], 0x0040);
-        if (ok1) *reinterpret_cast<uint32_t *>(out + dst1_off) = __byte_perm(lo1, hi1, 0x5410);
-    }
-#pragma unroll 1
-    for (int l = 1; l < N; l++) {
-        const float invp = c_conv[l].invp, negp = c_conv[l].negp;
-        const uint32_t wb0 = c_conv[l].wb[0], wb1 = c_conv[l].wb[1], wb2 = c_conv[l].wb[2];
-        uint32_t r[8];
-#pragma unroll
-        for (int u = 0; u < 8; u++) {
-            uint32_t xb = __dp4a(w[u][0], wb0, 0x4B000000u);
-            xb = __dp4a(w[u][1], wb1, xb);
-            if (NB == 3) xb = __dp4a(w[u][2], wb2, xb);
-            const float x = __fadd_rn(__uint_as_float(xb), -8388608.0f);        // exact
-            const float q = __fadd_rn(__fmaf_rn(x, invp, MAGIC), -MAGIC);       // round(x / p), exact
-            const float rm = __fmaf_rn(q, negp, x);                             // x - q p in [-(p-1)/2, (p-1)/2]
-            r[u] = __float_as_uint(__fmaf_rn(rm, sg[u], MAGIC));                // low byte = sign * rm
-        }
-        out += plane_stride;
-        const uint32_t lo = __byte_perm(r[0], r[1], 0x0040), hi = __byte_perm(r[2], r[3], 0x0040);
-        *reinterpret_cast<uint32_t *>(out) = __byte_perm(lo, hi, 0x5410);
-        const uint32_t lo1 = __byte_perm(r[4], r[5], 0x0040), hi1 = __byte_perm(r[6], r[7], 0x0040);
-        if (ok1) *reinterpret_cast<uint32_t *>(out + dst1_off) = __byte_perm(lo1, hi1, 0x5410);
+}
+__device__ __forceinline__ void conv_wait(ConvCtx &cx)
+{
+    mbar_wait_a(cx.mbar, cx.phase);
+    cx.phase ^= 1u;
+    tc_fence_after();
+}
+
+// u = Y mod p for Y < 2^24 (exact: magic = floor(2^32 / p) + 1, Y (magic p - 2^32) < 2^32)
+template <int L>
+__device__ __forceinline__ uint32_t umod(uint32_t y)
+{
+    constexpr uint32_t p = modulus_of(L), magic = (uint32_t)(0x100000000ull / p) + 1u;
+    return y - __umulhi(y, magic) * p;
+}
+
+// four residues of modulus L (accumulator values y0..y3 of the quad's four elements) -> one packed word of INT8
+template <int L>
+__device__ __forceinline__ uint32_t pack_quad(uint32_t y0, uint32_t y1, uint32_t y2, uint32_t y3)
+{
+    if constexpr (L == 0) {                                           // p = 256: the low bytes of a' (reading R5)
+        return __byte_perm(__byte_perm(y0, y1, 0x0040), __byte_perm(y2, y3, 0x0040), 0x5410);
+    } else {
+        constexpr uint32_t half = (modulus_of(L) - 1) / 2, c = (128u - half) * 0x01010101u;
+        const uint32_t u0 = umod<L>(y0), u1 = umod<L>(y1), u2 = umod<L>(y2), u3 = umod<L>(y3);
+        const uint32_t w = __byte_perm(__byte_perm(u0, u1, 0x0040), __byte_perm(u2, u3, 0x0040), 0x5410);
+        return (w + c) ^ 0x80808080u;                                 // per byte: u + 128 - half <= 255, then offset-128 -> INT8
     }
 }
 
-// accurate mode: ceil(|a| 2^(5-E)) in [0, 64]
+// narrow epilogue: accumulator column = 4 l + slot.  One LDTM per 8 moduli; moduli in groups of 4 with one uniform
+// guard per group (and per-modulus guards in the last, partial group).
+template <int L0>
+__device__ __forceinline__ void store_group4(const uint32_t *v, int N, int8_t *dst, int64_t plane_stride)
+{
+    // v: 16 accumulator values (4 moduli x 4 slots) of moduli L0 .. L0 + 3
+    if (L0 + 4 <= N) {
+        *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 0) * plane_stride) = pack_quad<L0 + 0>(v[0], v[1], v[2], v[3]);
+        *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 1) * plane_stride) = pack_quad<L0 + 1>(v[4], v[5], v[6], v[7]);
+        *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 2) * plane_stride) = pack_quad<L0 + 2>(v[8], v[9], v[10], v[11]);
+        *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 3) * plane_stride) = pack_quad<L0 + 3>(v[12], v[13], v[14], v[15]);
+    } else {
+        if (L0 + 0 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 0) * plane_stride) = pack_quad<L0 + 0>(v[0], v[1], v[2], v[3]);
+        if (L0 + 1 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 1) * plane_stride) = pack_quad<L0 + 1>(v[4], v[5], v[6], v[7]);
+        if (L0 + 2 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 2) * plane_stride) = pack_quad<L0 + 2>(v[8], v[9], v[10], v[11]);
+    }
+}
+
+__device__ __forceinline__ void epilogue_narrow(const ConvCtx &cx, int N, int8_t *dst, int64_t plane_stride, bool ok)
+{
+    uint32_t v[32];
+    tc_ld32(cx.tmem, v);
+    if (ok) {
+        store_group4<0>(v, N, dst, plane_stride);
+        if (N > 4) store_group4<4>(v + 16, N, dst, plane_stride);
+    }
+    if (N > 8) {                                                      // uniform
+        tc_ld32(cx.tmem + 32u, v);
+        if (ok) {
+            store_group4<8>(v, N, dst, plane_stride);
+            if (N > 12) store_group4<12>(v + 16, N, dst, plane_stride);
+        }
+    }
+}
+
+// wide epilogue: accumulator column = 2 l + slot; a round has two MMA passes (elements 0, 1 and 2, 3 of the quad).
+// Pass 0 keeps u0 | u1 << 8 per modulus in H[], pass 1 completes the words.
+template <int L>
+__device__ __forceinline__ uint32_t half_word(uint32_t y0, uint32_t y1)
+{
+    if constexpr (L == 0) return __byte_perm(y0, y1, 0x0040) & 0xFFFFu;
+    else return __byte_perm(umod<L>(y0), umod<L>(y1), 0x0040) & 0xFFFFu;
+}
+template <int L>
+__device__ __forceinline__ uint32_t finish_word(uint32_t h)
+{
+    if constexpr (L == 0) return h;
+    else {
+        constexpr uint32_t half = (modulus_of(L) - 1) / 2, c = (128u - half) * 0x01010101u;
+        return (h + c) ^ 0x80808080u;
+    }
+}
+template <int L0, int PASS>
+__device__ __forceinline__ void wide_group4(const uint32_t *v, int N, uint32_t *H, int8_t *dst, int64_t plane_stride, bool ok)
+{
+    // v: 8 accumulator values (4 moduli x 2 slots) of moduli L0 .. L0 + 3
+    if (L0 >= N) return;
+    uint32_t h0 = half_word<L0 + 0>(v[0], v[1]), h1 = half_word<L0 + 1 < OZ2_MAX_MODULI ? L0 + 1 : 0>(v[2], v[3]);
+    uint32_t h2 = half_word<L0 + 2 < OZ2_MAX_MODULI ? L0 + 2 : 0>(v[4], v[5]), h3 = half_word<L0 + 3 < OZ2_MAX_MODULI ? L0 + 3 : 0>(v[6], v[7]);
+    if (PASS == 0) {
+        H[L0 + 0] = h0; H[L0 + 1] = h1; H[L0 + 2] = h2; H[L0 + 3] = h3;
+    } else if (ok) {
+        *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 0) * plane_stride) = finish_word<L0 + 0>(H[L0 + 0] | (h0 << 16));
+        if (L0 + 1 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 1) * plane_stride) = finish_word<L0 + 1 < OZ2_MAX_MODULI ? L0 + 1 : 0>(H[L0 + 1] | (h1 << 16));
+        if (L0 + 2 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 2) * plane_stride) = finish_word<L0 + 2 < OZ2_MAX_MODULI ? L0 + 2 : 0>(H[L0 + 2] | (h2 << 16));
+        if (L0 + 3 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 3) * plane_stride) = finish_word<L0 + 3 < OZ2_MAX_MODULI ? L0 + 3 : 0>(H[L0 + 3] | (h3 << 16));
+    }
+}
+template <int PASS>
+__device__ __forceinline__ void epilogue_wide(const ConvCtx &cx, int N, uint32_t *H, int8_t *dst, int64_t plane_stride, bool ok)
+{
+    uint32_t v[32];
+    tc_ld32(cx.tmem, v);                                              // moduli 0 .. 15
+    wide_group4<0, PASS>(v, N, H, dst, plane_stride, ok);
+    wide_group4<4, PASS>(v + 8, N, H, dst, plane_stride, ok);
+    wide_group4<8, PASS>(v + 16, N, H, dst, plane_stride, ok);
+    wide_group4<12, PASS>(v + 24, N, H, dst, plane_stride, ok);
+    if (N > 16) {                                                     // uniform; moduli 16 .. 19 (columns 32 .. 39)
+        tc_ld32(cx.tmem + 32u, v);
+        wide_group4<16, PASS>(v, N, H, dst, plane_stride, ok);
+    }
+}
+
+// one quad: digits -> K row -> MMA -> residues of all N moduli -> 4-byte stores
+template <int WIDE>
+__device__ __forceinline__ void convert_quad(ConvCtx &cx, const double (&a)[4], const int (&ex)[4], int N, int8_t *dst,
+                                             int64_t plane_stride, bool ok)
+{
+    if (!WIDE) {
+        const unsigned long long d0 = digits_narrow(a[0], ex[0]), d1 = digits_narrow(a[1], ex[1]);
+        const unsigned long long d2 = digits_narrow(a[2], ex[2]), d3 = digits_narrow(a[3], ex[3]);
+        sts128(cx.tile_row, (uint32_t)d0, (uint32_t)(d0 >> 32), (uint32_t)d1, (uint32_t)(d1 >> 32));
+        sts128(cx.tile_row + 128u, (uint32_t)d2, (uint32_t)(d2 >> 32), (uint32_t)d3, (uint32_t)(d3 >> 32));
+        conv_mma(cx);
+        conv_wait(cx);
+        epilogue_narrow(cx, N, dst, plane_stride, ok);
+    } else {
+        uint32_t H[OZ2_MAX_MODULI + 4];
+        uint32_t w[3];
+        digits_wide(a[0], ex[0], w);
+        sts128(cx.tile_row, w[0], w[1], w[2], 0u);
+        digits_wide(a[1], ex[1], w);
+        sts128(cx.tile_row + 128u, w[0], w[1], w[2], 0u);
+        conv_mma(cx);
+        conv_wait(cx);
+        epilogue_wide<0>(cx, N, H, dst, plane_stride, ok);
+        digits_wide(a[2], ex[2], w);
+        sts128(cx.tile_row, w[0], w[1], w[2], 0u);
+        digits_wide(a[3], ex[3], w);
+        sts128(cx.tile_row + 128u, w[0], w[1], w[2], 0u);
+        conv_mma(cx);
+        conv_wait(cx);
+        epilogue_wide<1>(cx, N, H, dst, plane_stride, ok);
+    }
+}
+
+// CTA prologue: operand images, barrier, tensor memory
+template <int WIDE>
+__device__ __forceinline__ void conv_setup(ConvSmem *S, ConvCtx &cx, int N)
+{
+    const int tid = threadIdx.x;
+    for (int t = tid; t < CV_IMG_BYTES / 16; t += CV_THREADS) {
+        reinterpret_cast<uint4 *>(S->imgw)[t] = reinterpret_cast<const uint4 *>(g_conv_img[WIDE][0])[t];
+        reinterpret_cast<uint4 *>(S->imgb)[t] = reinterpret_cast<const uint4 *>(g_conv_img[WIDE][1])[t];
+    }
+    if (tid < CV_ONES_BYTES / 16)                                     // K byte 0 of every row = 1: first byte of the 8 core rows of K chunk 0
+        reinterpret_cast<uint4 *>(S->ones)[tid] = make_uint4(tid < 8 ? 1u : 0u, 0u, 0u, 0u);
+    if (tid == 0) {
+        mbar_init(&S->mbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (tid < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&S->tmem_slot)), "n"(CV_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    cx.tmem_base = S->tmem_slot;
+    cx.tmem = cx.tmem_base + ((uint32_t)(tid & ~31) << 16);          // lane quarter of this warp
+    cx.tile_row = smem_u32(S->tile) + (uint32_t)tile_off(tid, 0);
+    cx.mbar = smem_u32(&S->mbar);
+    cx.phase = 0;
+    cx.adesc = kmajor_desc(smem_u32(S->tile), 256u);
+    cx.odesc = kmajor_desc(smem_u32(S->ones), 0u);                    // every 8-row group reads the same 256 bytes
+    cx.bdesc = kmajor_desc(smem_u32(S->imgw), 256u);
+    cx.biasdesc = kmajor_desc(smem_u32(S->imgb), 256u);
+    // accumulator columns in use: 4 per modulus (narrow) / 2 per modulus (wide), rounded up to the MMA's N granule of 16
+    const int cols = WIDE ? 2 * N : 4 * N;
+    const uint32_t nmma = (uint32_t)((cols + 15) & ~15);
+    // kind::i8: D = S32, A = B = unsigned 8 bit, both K-major, M = 128
+    cx.idesc = (2u << 4) | ((nmma >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+
+__device__ __forceinline__ void conv_teardown(const ConvCtx &cx)
+{
+    tc_fence_before();
+    __syncthreads();
+    if (threadIdx.x < 32)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(cx.tmem_base), "n"(CV_TMEM_COLS) : "memory");
+}
+
+__device__ __forceinline__ ConvSmem *conv_smem(uint8_t *raw)
+{
+    return reinterpret_cast<ConvSmem *>((reinterpret_cast<uintptr_t>(raw) + 127) & ~(uintptr_t)127);   // no swizzle: 16 B would do
+}
+
+// four consecutive elements of a contiguous vector as doubles: two 16-byte loads (FP64) or one (FP32)
+__device__ __forceinline__ void ld4(const double *p, double (&a)[4])
+{
+    const double2 v0 = __ldg(reinterpret_cast<const double2 *>(p)), v1 = __ldg(reinterpret_cast<const double2 *>(p + 2));
+    a[0] = v0.x; a[1] = v0.y; a[2] = v1.x; a[3] = v1.y;
+}
+__device__ __forceinline__ void ld4(const float *p, double (&a)[4])
+{
+    const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
+    a[0] = (double)v.x; a[1] = (double)v.y; a[2] = (double)v.z; a[3] = (double)v.w;
+}
+template <typename T>
+__device__ __forceinline__ void load_quad(const T *vec, int64_t h, int64_t k, bool vec_ok, double (&a)[4])
+{
+    if (vec_ok && h + 3 < k) ld4(vec + h, a);
+    else {
+#pragma unroll
+        for (int u = 0; u < 4; u++) a[u] = (h + u < k) ? (double)__ldg(vec + h + u) : 0.0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// contiguous vectors: vector j is X[h + j ldx].  Work item = (vector, chunk of 512 h); every CTA of the persistent
+// grid takes one contiguous run of items, so that its pointers advance by a constant between rounds.
+// ---------------------------------------------------------------------------------------------
+template <int WIDE, typename T>
+__global__ void __launch_bounds__(CV_THREADS, WIDE ? 6 : 8)
+k2_tc_cols(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx, const int32_t *__restrict__ ex,
+           int8_t *__restrict__ planes, int64_t kp)
+{
+    extern __shared__ uint8_t smem_raw[];
+    ConvSmem *S = conv_smem(smem_raw);
+    ConvCtx cx;
+    conv_setup<WIDE>(S, cx, N);
+    const int tid = threadIdx.x;
+    const int chunks = (int)((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);      // k <= 2^22: fits 32 bits
+    const int64_t items = rows * chunks;
+    const int64_t it0 = items * blockIdx.x / gridDim.x, it1 = items * (blockIdx.x + 1) / gridDim.x;
+    const int64_t plane_stride = rows * kp;
+    const int k32 = (int)k, kp32 = (int)kp;
+    int64_t j = it0 / chunks;
+    int c = (int)(it0 - j * chunks);
+    int h = c * CV_CHUNK_H + 4 * tid;                                  // first h of this thread's quad
+    const T *src = X + j * ldx + h;
+    int8_t *dst = planes + j * kp + h;
+    bool vec_ok = (((uintptr_t)(X + j * ldx)) & 15) == 0;
+    double a[4] = { 0.0, 0.0, 0.0, 0.0 };
+    int e = 0;
+    if (it0 < it1) {
+        if (vec_ok && h + 3 < k32) ld4(src, a);
+        else {
+#pragma unroll
+            for (int u = 0; u < 4; u++) a[u] = (h + u < k32) ? (double)__ldg(src + u) : 0.0;
+        }
+        e = __ldg(ex + j);
+    }
+    for (int64_t item = it0; item < it1; item++) {
+        const double cur[4] = { a[0], a[1], a[2], a[3] };
+        const int exq[4] = { e, e, e, e };
+        int8_t *dcur = dst;
+        const bool ok = h < kp32;
+        // next item: its loads are in flight while this one runs through the tensor core and the epilogue
+        c++; h += CV_CHUNK_H; src += CV_CHUNK_H; dst += CV_CHUNK_H;
+        if (c == chunks) {
+            c = 0; j++; h = 4 * tid;
+            src = X + j * ldx + h;
+            dst = planes + j * kp + h;
+            vec_ok = (((uintptr_t)(X + j * ldx)) & 15) == 0;
+            if (item + 1 < it1) e = __ldg(ex + j);
+        }
+        if (item + 1 < it1) {
+            if (vec_ok && h + 3 < k32) ld4(src, a);
+            else {
+#pragma unroll
+                for (int u = 0; u < 4; u++) a[u] = (h + u < k32) ? (double)__ldg(src + u) : 0.0;
+            }
+        }
+        convert_quad<WIDE>(cx, cur, exq, N, dcur, plane_stride, ok);
+    }
+    conv_teardown(cx);
+}
+
+// ---------------------------------------------------------------------------------------------
+// strided vectors: vector i is X[i + h ldx] (rows of a column-major matrix).  Work item = block of 16 vectors x 64 h,
+// brought into shared memory by cp.async (128-byte coalesced reads along the rows, transposed on the way in, two
+// buffers: the next block lands while this one is converted); two rounds of 8 vectors x 64 h per block, half a warp
+// per vector, so that a warp stores two runs of 64 contiguous bytes per modulus.
+// ---------------------------------------------------------------------------------------------
+constexpr int ST_ROWS = 16, ST_H = 64;
+template <typename T>
+struct StageRow { static constexpr int PITCH = ST_H + 16 / (int)sizeof(T); };      // 16-byte aligned rows, odd in 16-byte units
+
+__device__ __forceinline__ void cp_async_zfill(uint32_t dst, const void *src, bool valid, int bytes)
+{
+    // copies `bytes` (4 or 8) or, if !valid, writes zeros (src-size 0); src must be a valid address either way
+    if (bytes == 8)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(valid ? 8 : 0) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(valid ? 4 : 0) : "memory");
+}
+
+template <int WIDE, typename T>
+__global__ void __launch_bounds__(CV_THREADS, WIDE ? 6 : 8)
+k2_tc_rows(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx, const int32_t *__restrict__ ex,
+           int8_t *__restrict__ planes, int64_t kp)
+{
+    extern __shared__ uint8_t smem_raw[];
+    ConvSmem *S = conv_smem(smem_raw);
+    constexpr int PITCH = StageRow<T>::PITCH, BUF = ST_ROWS * PITCH;
+    T *stage = reinterpret_cast<T *>(S + 1);                               // two buffers of BUF elements
+    ConvCtx cx;
+    conv_setup<WIDE>(S, cx, N);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nib = (int)((rows + ST_ROWS - 1) / ST_ROWS), nhb = (int)(kp / ST_H);
+    const int64_t items = (int64_t)nib * nhb;
+    const int64_t it0 = items * blockIdx.x / gridDim.x, it1 = items * (blockIdx.x + 1) / gridDim.x;
+    const int64_t plane_stride = rows * kp;
+    const int k32 = (int)k;
+    // copy pattern: thread = (row r = tid % 16, h = tid / 16 + 8 s), s = 0 .. 7
+    const int r = tid & 15, hs = tid >> 4;
+    const uint32_t stage_s = smem_u32(stage) + (uint32_t)((r * PITCH + hs) * sizeof(T));
+    auto issue = [&](int64_t item, int buf) {
+        const int hb = (int)(item / nib), ib = (int)(item - (int64_t)hb * nib);   // row blocks fastest: concurrent CTAs read whole columns
+        const int64_t i = (int64_t)ib * ST_ROWS + r;
+        const int h0 = hb * ST_H + hs;
+        const bool rok = i < rows;
+        const T *srcp = X + (rok ? i : 0) + (int64_t)h0 * ldx;
+        const uint32_t d = stage_s + (uint32_t)(buf * BUF * sizeof(T));
+#pragma unroll
+        for (int s = 0; s < 8; s++) {
+            const bool v = rok && h0 + 8 * s < k32;
+            cp_async_zfill(d + (uint32_t)(8 * s * sizeof(T)), v ? srcp + (int64_t)(8 * s) * ldx : X, v, (int)sizeof(T));
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if (it0 < it1) issue(it0, 0);
+    int buf = 0;
+    for (int64_t item = it0; item < it1; item++, buf ^= 1) {
+        if (item + 1 < it1) {
+            issue(item + 1, buf ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncthreads();                                                   // every thread's copies of this block have landed
+        const int hb = (int)(item / nib), ib = (int)(item - (int64_t)hb * nib);
+        const T *sb = stage + buf * BUF;
+#pragma unroll 1
+        for (int rr = 0; rr < 2; rr++) {
+            const int rl = 8 * rr + 2 * warp + (lane >> 4), ql = lane & 15;
+            const int64_t i = (int64_t)ib * ST_ROWS + rl;
+            const bool ok = i < rows;
+            double a[4];
+            if constexpr (sizeof(T) == 8) {
+                const double2 lo = *reinterpret_cast<const double2 *>(&sb[rl * PITCH + 4 * ql]);
+                const double2 hi = *reinterpret_cast<const double2 *>(&sb[rl * PITCH + 4 * ql + 2]);
+                a[0] = lo.x; a[1] = lo.y; a[2] = hi.x; a[3] = hi.y;
+            } else {
+                const float4 q = *reinterpret_cast<const float4 *>(&sb[rl * PITCH + 4 * ql]);
+                a[0] = (double)q.x; a[1] = (double)q.y; a[2] = (double)q.z; a[3] = (double)q.w;
+            }
+            const int e = ok ? __ldg(ex + i) : 0;
+            const int exq[4] = { e, e, e, e };
+            int8_t *dst = planes + i * kp + hb * ST_H + 4 * ql;
+            convert_quad<WIDE>(cx, a, exq, N, dst, plane_stride, ok);
+        }
+        // the buffer is free again once every thread has passed the barrier inside the NEXT block's first round;
+        // the copy that reuses it is issued one block later still
+    }
+    conv_teardown(cx);
+}
+
+// ---------------------------------------------------------------------------------------------
+// accurate mode: Abar / Bbar = ceil(|a| 2^(5-E)) in [0, 64], one INT8 plane, CUDA cores only
+// ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t ceil_scaled(double a, int E)
 {
     const unsigned long long b = (unsigned long long)__double_as_longlong(a) & 0x7FFFFFFFFFFFFFFFull;
@@ -143,18 +568,16 @@ __device__ __forceinline__ void quad_bar(const double (&a)[4], int E, int8_t *ds
     *reinterpret_cast<uint32_t *>(dst) = o;
 }
 
-// ---------------------------------------------------------------------------------------------
-// A path.  MODE 0: residues (NB words)   MODE 1: Abar
-// ---------------------------------------------------------------------------------------------
-template <int NB, int MODE, typename T>
-__global__ void __launch_bounds__(CONV_THREADS)
-k2_rows(int N, int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, const int32_t *__restrict__ e,
-        int8_t *__restrict__ planes, int64_t kp)
+constexpr int BAR_TI = 32, BAR_TH = 128, BAR_SROW = BAR_TH + 2, BAR_THREADS = 256;
+
+template <typename T>
+__global__ void __launch_bounds__(BAR_THREADS)
+k2_bar_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, const int32_t *__restrict__ E, int8_t *__restrict__ plane,
+            int64_t kp)
 {
-    __shared__ __align__(16) double tile[TI * SROW];
+    __shared__ __align__(16) double tile[BAR_TI * BAR_SROW];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t i0 = (int64_t)blockIdx.x * TI, h0 = (int64_t)blockIdx.y * TH;
-    // ---- stage: thread (lane = row, warp = h mod 8), 16 loads in flight, transposed into tile[i][h]
+    const int64_t i0 = (int64_t)blockIdx.x * BAR_TI, h0 = (int64_t)blockIdx.y * BAR_TH;
     {
         const int64_t i = i0 + lane;
         const bool iok = i < m;
@@ -166,122 +589,120 @@ k2_rows(int N, int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, const
             v[s] = (iok && h < k) ? (double)__ldg(src + (int64_t)(8 * s) * lda) : 0.0;
         }
 #pragma unroll
-        for (int s = 0; s < 16; s++) tile[lane * SROW + warp + 8 * s] = v[s];
+        for (int s = 0; s < 16; s++) tile[lane * BAR_SROW + warp + 8 * s] = v[s];
     }
     __syncthreads();
-    // ---- convert: warp w owns rows 4w .. 4w+3, lane owns the quad h = 4 lane .. 4 lane + 3
-    const int64_t plane_stride = m * kp;
 #pragma unroll 1
-    for (int rr = 0; rr < TI / 8; rr += 2) {
-        const int il = warp * (TI / 8) + rr;
+    for (int rr = 0; rr < BAR_TI / 8; rr++) {
+        const int il = warp * (BAR_TI / 8) + rr;
         const int64_t i = i0 + il;
         if (i >= m) break;
-        const bool ok1 = i + 1 < m;
-        double a[2][4];
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-            const double2 lo = *reinterpret_cast<const double2 *>(&tile[(il + t) * SROW + 4 * lane]);
-            const double2 hi = *reinterpret_cast<const double2 *>(&tile[(il + t) * SROW + 4 * lane + 2]);
-            a[t][0] = lo.x; a[t][1] = lo.y; a[t][2] = hi.x; a[t][3] = hi.y;
-        }
-        int8_t *dst = planes + i * kp + h0 + 4 * lane;
-        const int ex0 = __ldg(e + i), ex1 = ok1 ? __ldg(e + i + 1) : 0;
-        if (MODE == 0) oct_residues<NB>(a, ex0, ex1, N, dst, kp, ok1, plane_stride);
-        else {
-            quad_bar(a[0], ex0, dst);
-            if (ok1) quad_bar(a[1], ex1, dst + kp);
-        }
+        const double2 lo = *reinterpret_cast<const double2 *>(&tile[il * BAR_SROW + 4 * lane]);
+        const double2 hi = *reinterpret_cast<const double2 *>(&tile[il * BAR_SROW + 4 * lane + 2]);
+        const double a[4] = { lo.x, lo.y, hi.x, hi.y };
+        quad_bar(a, __ldg(E + i), plane + i * kp + h0 + 4 * lane);
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// B path: warp = 256 consecutive h of column j; lane holds the quads at 4 lane and 128 + 4 lane
-// ---------------------------------------------------------------------------------------------
-// four consecutive elements of a column as doubles: two 16-byte loads (FP64) or one (FP32)
-__device__ __forceinline__ void ld4(const double *p, double (&a)[4])
-{
-    const double2 v0 = __ldg(reinterpret_cast<const double2 *>(p)), v1 = __ldg(reinterpret_cast<const double2 *>(p + 2));
-    a[0] = v0.x; a[1] = v0.y; a[2] = v1.x; a[3] = v1.y;
-}
-__device__ __forceinline__ void ld4(const float *p, double (&a)[4])
-{
-    const float4 v = __ldg(reinterpret_cast<const float4 *>(p));
-    a[0] = (double)v.x; a[1] = (double)v.y; a[2] = (double)v.z; a[3] = (double)v.w;
-}
-
-template <int NB, int MODE, typename T>
-__global__ void __launch_bounds__(CONV_THREADS)
-k2_cols(int N, int64_t n, int64_t k, const T *__restrict__ B, int64_t ldb, const int32_t *__restrict__ f,
-        int8_t *__restrict__ planes, int64_t kp)
-{
-    const int lane = threadIdx.x & 31;
-    const int64_t chunks = (kp + 255) / 256;
-    const int64_t item = (int64_t)blockIdx.x * (CONV_THREADS / 32) + (threadIdx.x >> 5);
-    if (item >= n * chunks) return;
-    const int64_t j = item / chunks, c = item - j * chunks;
-    const T *col = B + j * ldb;
-    const int ex = __ldg(f + j);
-    const bool vec = ((((uintptr_t)col) & 15) == 0);
-    const int64_t plane_stride = n * kp;
-    double a[2][4];
-#pragma unroll
-    for (int t = 0; t < 2; t++) {
-        const int64_t h = c * 256 + 128 * t + 4 * lane;
-        if (vec && h + 3 < k) {
-            ld4(col + h, a[t]);
-        } else {
-#pragma unroll
-            for (int u = 0; u < 4; u++) a[t][u] = (h + u < k) ? (double)__ldg(col + h + u) : 0.0;
-        }
-    }
-    const int64_t h = c * 256 + 4 * lane;           // first quad; kp is a multiple of 128, so it is inside
-    int8_t *dst = planes + j * kp + h;
-    const bool ok1 = h + 128 < kp;
-    if (MODE == 0) oct_residues<NB>(a, ex, ex, N, dst, 128, ok1, plane_stride);
-    else {
-        quad_bar(a[0], ex, dst);
-        if (ok1) quad_bar(a[1], ex, dst + 128);
-    }
-}
-
-} // namespace
-
-int oz2_convert_upload_tables(const Oz2HostTables &t)
-{
-    ConvTab h[OZ2_MAX_MODULI];
-    for (int l = 0; l < OZ2_MAX_MODULI; l++) {
-        const uint32_t p = t.mod[l].p;
-        h[l].invp = (float)(1.0 / (double)p);
-        h[l].negp = -(float)p;
-        for (int i = 0; i < 3; i++) { h[l].wb[i] = t.mod[l].wb[i]; h[l].pad[i] = 0; }
-    }
-    OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_conv, h, sizeof(h)));
-    return 0;
 }
 
 template <typename T>
-static int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *X, int64_t ldx, const int32_t *ex,
-                            int8_t *planes, int64_t kp, cudaStream_t st)
+__global__ void __launch_bounds__(BAR_THREADS)
+k2_bar_cols(int64_t n, int64_t k, const T *__restrict__ B, int64_t ldb, const int32_t *__restrict__ E, int8_t *__restrict__ plane,
+            int64_t kp)
 {
-    if (op == 0) {
-        dim3 grid((unsigned)((rows + TI - 1) / TI), (unsigned)(kp / TH));
-        if (N == 0) k2_rows<2, 1, T><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else if (wide) k2_rows<3, 0, T><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else k2_rows<2, 0, T><<<grid, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+    const int64_t quads = kp / 4;
+    const int64_t t = (int64_t)blockIdx.x * BAR_THREADS + threadIdx.x;
+    if (t >= n * quads) return;
+    const int64_t j = t / quads, h = (t - j * quads) * 4;
+    const T *col = B + j * ldb;
+    double a[4];
+    load_quad(col, h, k, (((uintptr_t)col) & 15) == 0, a);
+    quad_bar(a, __ldg(E + j), plane + j * kp + h);
+}
+
+int num_sms()
+{
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    return sms;
+}
+
+template <typename T>
+constexpr size_t rows_smem() { return sizeof(ConvSmem) + 128 + 2 * (size_t)ST_ROWS * StageRow<T>::PITCH * sizeof(T); }
+constexpr size_t cols_smem() { return sizeof(ConvSmem) + 128; }
+
+template <typename T>
+int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *X, int64_t ldx, const int32_t *ex,
+                     int8_t *planes, int64_t kp, cudaStream_t st)
+{
+    if (N == 0) {                                     // accurate mode's single plane
+        if (op == 0) {
+            dim3 grid((unsigned)((rows + BAR_TI - 1) / BAR_TI), (unsigned)(kp / BAR_TH));
+            k2_bar_rows<T><<<grid, BAR_THREADS, 0, st>>>(rows, k, X, ldx, ex, planes, kp);
+        } else {
+            const int64_t total = rows * (kp / 4);
+            k2_bar_cols<T><<<(unsigned)((total + BAR_THREADS - 1) / BAR_THREADS), BAR_THREADS, 0, st>>>(rows, k, X, ldx, ex, planes, kp);
+        }
     } else {
-        const int64_t items = rows * ((kp + 255) / 256);
-        const unsigned gx = (unsigned)((items + CONV_THREADS / 32 - 1) / (CONV_THREADS / 32));
-        if (N == 0) k2_cols<2, 1, T><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else if (wide) k2_cols<3, 0, T><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
-        else k2_cols<2, 0, T><<<gx, CONV_THREADS, 0, st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        const int per_sm = wide ? 6 : 8;              // tensor memory: 64 columns per CTA
+        if (op == 0) {
+            const int64_t items = ((rows + ST_ROWS - 1) / ST_ROWS) * (kp / ST_H);
+            int64_t grid = (int64_t)num_sms() * per_sm;
+            if (grid > items) grid = items;
+            if (wide) k2_tc_rows<1, T><<<(unsigned)grid, CV_THREADS, rows_smem<T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            else k2_tc_rows<0, T><<<(unsigned)grid, CV_THREADS, rows_smem<T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        } else {
+            const int64_t items = rows * ((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);
+            int64_t grid = (int64_t)num_sms() * per_sm;
+            if (grid > items) grid = items;
+            if (wide) k2_tc_cols<1, T><<<(unsigned)grid, CV_THREADS, cols_smem(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            else k2_tc_cols<0, T><<<(unsigned)grid, CV_THREADS, cols_smem(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+        }
     }
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
 }
 
-// op 0: rows of A, op 1: columns of B.  N >= 1: residue planes [N][rows][kp] with exponents `ex`.  N == 0: the
-// single plane ceil(mu' |.|) of accurate mode; `ex` then holds E = floor(log2 max |.|) per row.
+} // namespace
+
+int oz2_convert_upload_tables(const Oz2HostTables &t)
+{
+    static uint8_t img[2][2][CV_IMG_BYTES];
+    memset(img, 0, sizeof(img));
+    for (int wide = 0; wide < 2; wide++) {
+        const int slots = wide ? 2 : 4, digits = wide ? 12 : 8, kstride = wide ? 16 : 8, topbit = wide ? 95 : 63;
+        for (int l = 0; l < OZ2_MAX_MODULI; l++) {
+            const uint32_t p = t.mod[l].p;
+            uint32_t two = 1 % p;                                    // 2^topbit mod p
+            for (int b = 0; b < topbit; b++) two = (two * 2u) % p;
+            const uint32_t half = (p - 1) / 2;
+            const uint32_t bias = l == 0 ? 0u : (half + p - two) % p;      // Y ~ a' + half (mod p); p = 256 keeps the low byte
+            for (int s = 0; s < slots; s++) {
+                const int col = l * slots + s;
+                if (col >= 64) continue;
+                for (int i = 0; i < digits; i++) {
+                    const uint32_t w = (t.mod[l].wb[i / 4] >> (8 * (i % 4))) & 0xFFu;   // 256^i mod p
+                    img[wide][0][tile_off(col, kstride * s + i)] = (uint8_t)w;
+                }
+                img[wide][1][tile_off(col, 0)] = (uint8_t)bias;
+            }
+        }
+    }
+    OZ2_CUDA_TRY(cudaMemcpyToSymbol(g_conv_img, img, sizeof(img)));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<0, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<double>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<1, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<double>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<float>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<1, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<float>()));
+    return 0;
+}
+
+// op 0: strided vectors (rows of a column-major matrix), op 1: contiguous vectors (its columns).  N >= 1: residue
+// planes [N][rows][kp] with exponents `ex`; wide != 0 when |a'| may exceed 63 bits.  N == 0: the single plane
+// ceil(mu' |.|) of accurate mode; `ex` then holds E = floor(log2 max |.|) per vector.
 // f32 != 0: X is FP32 (SGEMM variant), promoted exactly on load.
 int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k, const void *X, int64_t ldx,
                        const int32_t *ex, int8_t *planes, int64_t kp, cudaStream_t st)

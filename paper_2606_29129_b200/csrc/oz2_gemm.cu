@@ -348,7 +348,7 @@ __device__ __forceinline__ TileCoord decode_tile_pair(int64_t t, int tiles_m, in
     return c;
 }
 
-template <bool MAXEPI>
+template <int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, int nplanes,
                      int mod_base, int m, int n, int num_kb, uint8_t *__restrict__ U, int64_t mp,
@@ -446,7 +446,8 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
             tc_fence_after();
             const int i = c.m0 + (int)rank * 128 + q * 32 + lane;
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TILE_N);
-            if (!MAXEPI) {
+            if (EPI == EPI_NONE) {
+            } else if (EPI == EPI_MODP) {
                 const int l = mod_base + c.plane;
                 const Oz2ModTab tb = c_mod[l];
                 uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
@@ -545,8 +546,9 @@ int oz2_gemm_upload_tables(const Oz2HostTables &t)
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<EPI_MODP>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<EPI_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
     OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm<EPI_NONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<EPI_MODP>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<EPI_MAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k3_residue_gemm_pair<EPI_NONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
     return 0;
 }
 
@@ -561,7 +563,7 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
     if (m <= 0 || n <= 0 || nplanes <= 0) return 0;
     CUtensorMap mapA, mapB;
     const int num_kb = (int)(kp / TILE_K);
-    if (variant == OZ2_GEMM_PAIR && m > TILE_M && kp <= (1 << 17)) {
+    if ((variant == OZ2_GEMM_PAIR || variant == OZ2_GEMM_PAIR_MMA_ONLY) && m > TILE_M && kp <= (1 << 17)) {
         int rc = make_plane_map(&mapA, RA, kp, m, nplanes, 128);
         if (rc) return rc;
         rc = make_plane_map(&mapB, RB, kp, n, nplanes, 128);
@@ -571,10 +573,13 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
         if (tiles < clusters) clusters = tiles;
         const unsigned grid = (unsigned)(2 * clusters);
         if (rowmax)
-            k3_residue_gemm_pair<true><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
+            k3_residue_gemm_pair<EPI_MAX><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
                                                                          nullptr, mp, rowmax, colmax);
+        else if (variant == OZ2_GEMM_PAIR_MMA_ONLY)
+            k3_residue_gemm_pair<EPI_NONE><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
+                                                                          nullptr, mp, nullptr, nullptr);
         else
-            k3_residue_gemm_pair<false><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
+            k3_residue_gemm_pair<EPI_MODP><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
                                                                           U, mp, nullptr, nullptr);
         oz2_count_launches(1);
         OZ2_CUDA_TRY(cudaGetLastError());

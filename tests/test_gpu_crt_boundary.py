@@ -57,7 +57,7 @@ def planes_from_integers(N, zs, m, n):
 @pytest.mark.parametrize("N", range(2, 21))
 def test_crt_kernel_on_boundary_residues(B, N):
     import torch
-    m, n = 272, 48                                    # 13056 elements, m = 16 * 17: ragged against the 256-row tile
+    m, n = 272, 72                                    # 19584 elements, m = 16 * 17: ragged against the 256-row tile
     zs, P = boundary_integers(N, 10000, 100 + N)
     assert len(zs) <= m * n
     U = planes_from_integers(N, zs, m, n)
