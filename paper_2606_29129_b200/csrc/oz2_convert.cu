@@ -22,8 +22,8 @@
 // (K-major for the GEMM), kp = round_up(k, 128), zero padded.  A thread owns a quad (4 consecutive h of one vector)
 // from the global load to the 4-byte store, so a warp stores 128 contiguous bytes per modulus.
 //   * contiguous vectors (columns of B, or rows of A^T): 32-byte loads straight from global memory;
-//   * strided vectors (rows of a column-major A): a CTA brings 16 rows x 64 h into shared memory with cp.async
-//     (128-byte coalesced reads along the rows, transposed on the way in, double buffered).
+//   * strided vectors (rows of a column-major A): a CTA brings 16 rows x 128 h into shared memory with cp.async
+//     (128-byte coalesced reads along the rows, transposed on the way in), refilled while the last round computes.
 // The same two movers, without the tensor-core part, serve accurate mode's Abar / Bbar = ceil(mu' |.|).
 #include "oz2_common.cuh"
 #include "oz2_tc.cuh"
@@ -286,32 +286,35 @@ __device__ __forceinline__ void epilogue_wide(const ConvCtx &cx, int N, uint32_t
     }
 }
 
-// one quad: digits -> K row -> MMA -> residues of all N moduli -> 4-byte stores
-template <int WIDE>
-__device__ __forceinline__ void convert_quad(ConvCtx &cx, const double (&a)[4], const int (&ex)[4], int N, int8_t *dst,
-                                             int64_t plane_stride, bool ok)
+// one quad: digits -> K row -> MMA -> residues of all N moduli -> 4-byte stores.  `overlap()` runs between the MMA
+// issue and the wait for its result (the callers put the loads of their next work item there).
+template <int WIDE, typename F>
+__device__ __forceinline__ void convert_quad(ConvCtx &cx, const double (&a)[4], int ex, int N, int8_t *dst,
+                                             int64_t plane_stride, bool ok, F overlap)
 {
     if (!WIDE) {
-        const unsigned long long d0 = digits_narrow(a[0], ex[0]), d1 = digits_narrow(a[1], ex[1]);
-        const unsigned long long d2 = digits_narrow(a[2], ex[2]), d3 = digits_narrow(a[3], ex[3]);
+        const unsigned long long d0 = digits_narrow(a[0], ex), d1 = digits_narrow(a[1], ex);
+        const unsigned long long d2 = digits_narrow(a[2], ex), d3 = digits_narrow(a[3], ex);
         sts128(cx.tile_row, (uint32_t)d0, (uint32_t)(d0 >> 32), (uint32_t)d1, (uint32_t)(d1 >> 32));
         sts128(cx.tile_row + 128u, (uint32_t)d2, (uint32_t)(d2 >> 32), (uint32_t)d3, (uint32_t)(d3 >> 32));
         conv_mma(cx);
+        overlap();
         conv_wait(cx);
         epilogue_narrow(cx, N, dst, plane_stride, ok);
     } else {
         uint32_t H[OZ2_MAX_MODULI + 4];
         uint32_t w[3];
-        digits_wide(a[0], ex[0], w);
+        digits_wide(a[0], ex, w);
         sts128(cx.tile_row, w[0], w[1], w[2], 0u);
-        digits_wide(a[1], ex[1], w);
+        digits_wide(a[1], ex, w);
         sts128(cx.tile_row + 128u, w[0], w[1], w[2], 0u);
         conv_mma(cx);
+        overlap();
         conv_wait(cx);
         epilogue_wide<0>(cx, N, H, dst, plane_stride, ok);
-        digits_wide(a[2], ex[2], w);
+        digits_wide(a[2], ex, w);
         sts128(cx.tile_row, w[0], w[1], w[2], 0u);
-        digits_wide(a[3], ex[3], w);
+        digits_wide(a[3], ex, w);
         sts128(cx.tile_row + 128u, w[0], w[1], w[2], 0u);
         conv_mma(cx);
         conv_wait(cx);
@@ -393,8 +396,7 @@ __device__ __forceinline__ void load_quad(const T *vec, int64_t h, int64_t k, bo
 }
 
 // ---------------------------------------------------------------------------------------------
-// contiguous vectors: vector j is X[h + j ldx].  Work item = (vector, chunk of 512 h); every CTA of the persistent
-// grid takes one contiguous run of items, so that its pointers advance by a constant between rounds.
+// contiguous vectors: vector j is X[h + j ldx].  Work item = (vector, chunk of 512 h), persistent CTAs.
 // ---------------------------------------------------------------------------------------------
 template <int WIDE, typename T>
 __global__ void __launch_bounds__(CV_THREADS, WIDE ? 6 : 8)
@@ -408,58 +410,46 @@ k2_tc_cols(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
     const int tid = threadIdx.x;
     const int chunks = (int)((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);      // k <= 2^22: fits 32 bits
     const int64_t items = rows * chunks;
-    const int64_t it0 = items * blockIdx.x / gridDim.x, it1 = items * (blockIdx.x + 1) / gridDim.x;
     const int64_t plane_stride = rows * kp;
     const int k32 = (int)k, kp32 = (int)kp;
-    int64_t j = it0 / chunks;
-    int c = (int)(it0 - j * chunks);
-    int h = c * CV_CHUNK_H + 4 * tid;                                  // first h of this thread's quad
-    const T *src = X + j * ldx + h;
-    int8_t *dst = planes + j * kp + h;
-    bool vec_ok = (((uintptr_t)(X + j * ldx)) & 15) == 0;
+    // items are dealt round-robin (item = blockIdx.x + t gridDim.x): at any time the CTAs work on neighbouring chunks, so
+    // that reads and the N write streams stay sequential across the chip.  (j, c) advance without a division.
+    const int step_j = (int)(gridDim.x / (unsigned)chunks), step_c = (int)(gridDim.x - (unsigned)step_j * (unsigned)chunks);
+    int j = (int)(blockIdx.x / (unsigned)chunks), c = (int)(blockIdx.x - (unsigned)j * (unsigned)chunks);
     double a[4] = { 0.0, 0.0, 0.0, 0.0 };
     int e = 0;
-    if (it0 < it1) {
-        if (vec_ok && h + 3 < k32) ld4(src, a);
+    auto fetch = [&](int jj, int cc) {
+        const T *vec = X + (int64_t)jj * ldx;
+        const int h = cc * CV_CHUNK_H + 4 * tid;
+        if (((((uintptr_t)vec) & 15) == 0) && h + 3 < k32) ld4(vec + h, a);
         else {
 #pragma unroll
-            for (int u = 0; u < 4; u++) a[u] = (h + u < k32) ? (double)__ldg(src + u) : 0.0;
+            for (int u = 0; u < 4; u++) a[u] = (h + u < k32) ? (double)__ldg(vec + h + u) : 0.0;
         }
-        e = __ldg(ex + j);
-    }
-    for (int64_t item = it0; item < it1; item++) {
+        e = __ldg(ex + jj);
+    };
+    if ((int64_t)blockIdx.x < items) fetch(j, c);
+    for (int64_t item = blockIdx.x; item < items; item += gridDim.x) {
         const double cur[4] = { a[0], a[1], a[2], a[3] };
-        const int exq[4] = { e, e, e, e };
-        int8_t *dcur = dst;
+        const int ecur = e;
+        const int h = c * CV_CHUNK_H + 4 * tid;
+        int8_t *dst = planes + (int64_t)j * kp + h;
         const bool ok = h < kp32;
+        c += step_c; j += step_j;
+        if (c >= chunks) { c -= chunks; j++; }
         // next item: its loads are in flight while this one runs through the tensor core and the epilogue
-        c++; h += CV_CHUNK_H; src += CV_CHUNK_H; dst += CV_CHUNK_H;
-        if (c == chunks) {
-            c = 0; j++; h = 4 * tid;
-            src = X + j * ldx + h;
-            dst = planes + j * kp + h;
-            vec_ok = (((uintptr_t)(X + j * ldx)) & 15) == 0;
-            if (item + 1 < it1) e = __ldg(ex + j);
-        }
-        if (item + 1 < it1) {
-            if (vec_ok && h + 3 < k32) ld4(src, a);
-            else {
-#pragma unroll
-                for (int u = 0; u < 4; u++) a[u] = (h + u < k32) ? (double)__ldg(src + u) : 0.0;
-            }
-        }
-        convert_quad<WIDE>(cx, cur, exq, N, dcur, plane_stride, ok);
+        convert_quad<WIDE>(cx, cur, ecur, N, dst, plane_stride, ok, [&] { if (item + gridDim.x < items) fetch(j, c); });
     }
     conv_teardown(cx);
 }
 
 // ---------------------------------------------------------------------------------------------
-// strided vectors: vector i is X[i + h ldx] (rows of a column-major matrix).  Work item = block of 16 vectors x 64 h,
-// brought into shared memory by cp.async (128-byte coalesced reads along the rows, transposed on the way in, two
-// buffers: the next block lands while this one is converted); two rounds of 8 vectors x 64 h per block, half a warp
-// per vector, so that a warp stores two runs of 64 contiguous bytes per modulus.
+// strided vectors: vector i is X[i + h ldx] (rows of a column-major matrix).  Work item = block of 16 vectors x 128 h,
+// brought into shared memory by cp.async (128-byte coalesced reads along the rows, transposed on the way in); four
+// rounds of 4 vectors x 128 h per block (a warp = one vector, 128 contiguous bytes per store).  The copy of the next
+// block is issued as soon as the last round has read the buffer, so it overlaps that round's MMA and epilogue.
 // ---------------------------------------------------------------------------------------------
-constexpr int ST_ROWS = 16, ST_H = 64;
+constexpr int ST_ROWS = 16, ST_H = 128;
 template <typename T>
 struct StageRow { static constexpr int PITCH = ST_H + 16 / (int)sizeof(T); };      // 16-byte aligned rows, odd in 16-byte units
 
@@ -479,66 +469,66 @@ k2_tc_rows(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
 {
     extern __shared__ uint8_t smem_raw[];
     ConvSmem *S = conv_smem(smem_raw);
-    constexpr int PITCH = StageRow<T>::PITCH, BUF = ST_ROWS * PITCH;
-    T *stage = reinterpret_cast<T *>(S + 1);                               // two buffers of BUF elements
+    constexpr int PITCH = StageRow<T>::PITCH;
+    T *stage = reinterpret_cast<T *>(S + 1);
     ConvCtx cx;
     conv_setup<WIDE>(S, cx, N);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nib = (int)((rows + ST_ROWS - 1) / ST_ROWS), nhb = (int)(kp / ST_H);
     const int64_t items = (int64_t)nib * nhb;
-    const int64_t it0 = items * blockIdx.x / gridDim.x, it1 = items * (blockIdx.x + 1) / gridDim.x;
     const int64_t plane_stride = rows * kp;
     const int k32 = (int)k;
-    // copy pattern: thread = (row r = tid % 16, h = tid / 16 + 8 s), s = 0 .. 7
+    // item = ib + nib hb (row blocks fastest: concurrent CTAs read whole columns), walked with stride gridDim.x
+    const int step_hb = (int)(gridDim.x / (unsigned)nib), step_ib = (int)(gridDim.x - (unsigned)step_hb * (unsigned)nib);
+    int hb = (int)(blockIdx.x / (unsigned)nib), ib = (int)(blockIdx.x - (unsigned)hb * (unsigned)nib);
+    // copy pattern: thread = (row r = tid % 16, h = tid / 16 + 8 s), s = 0 .. 15
     const int r = tid & 15, hs = tid >> 4;
     const uint32_t stage_s = smem_u32(stage) + (uint32_t)((r * PITCH + hs) * sizeof(T));
-    auto issue = [&](int64_t item, int buf) {
-        const int hb = (int)(item / nib), ib = (int)(item - (int64_t)hb * nib);   // row blocks fastest: concurrent CTAs read whole columns
-        const int64_t i = (int64_t)ib * ST_ROWS + r;
-        const int h0 = hb * ST_H + hs;
+    auto issue = [&](int ibn, int hbn) {
+        const int64_t i = (int64_t)ibn * ST_ROWS + r;
+        const int h0 = hbn * ST_H + hs;
         const bool rok = i < rows;
         const T *srcp = X + (rok ? i : 0) + (int64_t)h0 * ldx;
-        const uint32_t d = stage_s + (uint32_t)(buf * BUF * sizeof(T));
 #pragma unroll
-        for (int s = 0; s < 8; s++) {
+        for (int s = 0; s < ST_H / 8; s++) {
             const bool v = rok && h0 + 8 * s < k32;
-            cp_async_zfill(d + (uint32_t)(8 * s * sizeof(T)), v ? srcp + (int64_t)(8 * s) * ldx : X, v, (int)sizeof(T));
+            cp_async_zfill(stage_s + (uint32_t)(8 * s * sizeof(T)), v ? srcp + (int64_t)(8 * s) * ldx : X, v, (int)sizeof(T));
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    if (it0 < it1) issue(it0, 0);
-    int buf = 0;
-    for (int64_t item = it0; item < it1; item++, buf ^= 1) {
-        if (item + 1 < it1) {
-            issue(item + 1, buf ^ 1);
-            asm volatile("cp.async.wait_group 1;" ::: "memory");
-        } else {
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if ((int64_t)blockIdx.x < items) issue(ib, hb);
+    for (int64_t item = blockIdx.x; item < items; item += gridDim.x) {
+        const int ibc = ib, hbc = hb;
+        ib += step_ib; hb += step_hb;
+        if (ib >= nib) { ib -= nib; hb++; }
+        const bool more = item + gridDim.x < items;
+        // exponents of this thread's four vectors (one per round)
+        int e4[4];
+#pragma unroll
+        for (int rr = 0; rr < 4; rr++) {
+            const int64_t i = (int64_t)ibc * ST_ROWS + 4 * rr + warp;
+            e4[rr] = i < rows ? __ldg(ex + i) : 0;
         }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                                                   // every thread's copies of this block have landed
-        const int hb = (int)(item / nib), ib = (int)(item - (int64_t)hb * nib);
-        const T *sb = stage + buf * BUF;
-#pragma unroll 1
-        for (int rr = 0; rr < 2; rr++) {
-            const int rl = 8 * rr + 2 * warp + (lane >> 4), ql = lane & 15;
-            const int64_t i = (int64_t)ib * ST_ROWS + rl;
+#pragma unroll
+        for (int rr = 0; rr < ST_ROWS / 4; rr++) {
+            const int rl = 4 * rr + warp;
+            const int64_t i = (int64_t)ibc * ST_ROWS + rl;
             const bool ok = i < rows;
             double a[4];
             if constexpr (sizeof(T) == 8) {
-                const double2 lo = *reinterpret_cast<const double2 *>(&sb[rl * PITCH + 4 * ql]);
-                const double2 hi = *reinterpret_cast<const double2 *>(&sb[rl * PITCH + 4 * ql + 2]);
+                const double2 lo = *reinterpret_cast<const double2 *>(&stage[rl * PITCH + 4 * lane]);
+                const double2 hi = *reinterpret_cast<const double2 *>(&stage[rl * PITCH + 4 * lane + 2]);
                 a[0] = lo.x; a[1] = lo.y; a[2] = hi.x; a[3] = hi.y;
             } else {
-                const float4 q = *reinterpret_cast<const float4 *>(&sb[rl * PITCH + 4 * ql]);
+                const float4 q = *reinterpret_cast<const float4 *>(&stage[rl * PITCH + 4 * lane]);
                 a[0] = (double)q.x; a[1] = (double)q.y; a[2] = (double)q.z; a[3] = (double)q.w;
             }
-            const int e = ok ? __ldg(ex + i) : 0;
-            const int exq[4] = { e, e, e, e };
-            int8_t *dst = planes + i * kp + hb * ST_H + 4 * ql;
-            convert_quad<WIDE>(cx, a, exq, N, dst, plane_stride, ok);
+            int8_t *dst = planes + i * kp + hbc * ST_H + 4 * lane;
+            // after the barrier inside the last round every thread has read the buffer: refill it for the next block
+            convert_quad<WIDE>(cx, a, e4[rr], N, dst, plane_stride, ok, [&] { if (rr == ST_ROWS / 4 - 1 && more) issue(ib, hb); });
         }
-        // the buffer is free again once every thread has passed the barrier inside the NEXT block's first round;
-        // the copy that reuses it is issued one block later still
     }
     conv_teardown(cx);
 }
@@ -631,7 +621,7 @@ int num_sms()
 }
 
 template <typename T>
-constexpr size_t rows_smem() { return sizeof(ConvSmem) + 128 + 2 * (size_t)ST_ROWS * StageRow<T>::PITCH * sizeof(T); }
+constexpr size_t rows_smem() { return sizeof(ConvSmem) + 128 + (size_t)ST_ROWS * StageRow<T>::PITCH * sizeof(T); }
 constexpr size_t cols_smem() { return sizeof(ConvSmem) + 128; }
 
 template <typename T>
