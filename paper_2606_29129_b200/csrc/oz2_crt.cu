@@ -154,36 +154,92 @@ __device__ __noinline__ TO crt_exact(const uint32_t (&c)[NW + 1], const Oz2CrtTa
     }
 }
 
+// ---- multiword helpers: one PTX carry chain each (the C++ formulation costs about twice the instructions) ----------
+// r = a - b over W words (borrow out of the top word is dropped)
+template <int W>
+__device__ __forceinline__ void mp_sub(uint32_t (&r)[W], const uint32_t (&a)[W], const uint32_t (&b)[W])
+{
+    static_assert(W >= 2 && W <= 6, "word count");
+    if constexpr (W == 2)
+        asm("sub.cc.u32 %0, %2, %4;\n\tsubc.u32 %1, %3, %5;" : "=r"(r[0]), "=r"(r[1]) : "r"(a[0]), "r"(a[1]), "r"(b[0]), "r"(b[1]));
+    else if constexpr (W == 3)
+        asm("sub.cc.u32 %0, %3, %6;\n\tsubc.cc.u32 %1, %4, %7;\n\tsubc.u32 %2, %5, %8;"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(b[0]), "r"(b[1]), "r"(b[2]));
+    else if constexpr (W == 4)
+        asm("sub.cc.u32 %0, %4, %8;\n\tsubc.cc.u32 %1, %5, %9;\n\tsubc.cc.u32 %2, %6, %10;\n\tsubc.u32 %3, %7, %11;"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+            : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]));
+    else if constexpr (W == 5)
+        asm("sub.cc.u32 %0, %5, %10;\n\tsubc.cc.u32 %1, %6, %11;\n\tsubc.cc.u32 %2, %7, %12;\n\tsubc.cc.u32 %3, %8, %13;\n\t"
+            "subc.u32 %4, %9, %14;"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4])
+            : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]), "r"(b[4]));
+    else
+        asm("sub.cc.u32 %0, %6, %12;\n\tsubc.cc.u32 %1, %7, %13;\n\tsubc.cc.u32 %2, %8, %14;\n\tsubc.cc.u32 %3, %9, %15;\n\t"
+            "subc.cc.u32 %4, %10, %16;\n\tsubc.u32 %5, %11, %17;"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5])
+            : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]), "r"(b[4]),
+              "r"(b[5]));
+}
+// x += one (one = 0 or 1) over W words
+template <int W>
+__device__ __forceinline__ void mp_inc(uint32_t (&x)[W], uint32_t one)
+{
+    static_assert(W >= 1 && W <= 5, "word count");
+    if constexpr (W == 1) x[0] += one;
+    else if constexpr (W == 2) asm("add.cc.u32 %0, %0, %2;\n\taddc.u32 %1, %1, 0;" : "+r"(x[0]), "+r"(x[1]) : "r"(one));
+    else if constexpr (W == 3)
+        asm("add.cc.u32 %0, %0, %3;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.u32 %2, %2, 0;" : "+r"(x[0]), "+r"(x[1]), "+r"(x[2]) : "r"(one));
+    else if constexpr (W == 4)
+        asm("add.cc.u32 %0, %0, %4;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.cc.u32 %2, %2, 0;\n\taddc.u32 %3, %3, 0;"
+            : "+r"(x[0]), "+r"(x[1]), "+r"(x[2]), "+r"(x[3]) : "r"(one));
+    else
+        asm("add.cc.u32 %0, %0, %5;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.cc.u32 %2, %2, 0;\n\taddc.cc.u32 %3, %3, 0;\n\taddc.u32 %4, %4, 0;"
+            : "+r"(x[0]), "+r"(x[1]), "+r"(x[2]), "+r"(x[3]), "+r"(x[4]) : "r"(one));
+}
+
+// per-thread copy of the per-N constants the common case needs (kept in registers across the tile loop)
+template <int NW>
+struct CrtRegs {
+    uint32_t P[NW];
+    double invP;
+};
+
 // The common case of crt_exact without a branch: the quotient estimate is away from a half-integer and the result
 // is a normal number.  `rare` is set when that does not hold (the caller then takes crt_exact).
 template <int NW, typename TO>
-__device__ __forceinline__ TO crt_fast(const uint32_t (&c)[NW + 1], const Oz2CrtTab &T, int esum, bool &rare)
+__device__ __forceinline__ TO crt_fast(const uint32_t (&c)[NW + 1], const CrtRegs<NW> &T, int esum, bool &rare)
 {
+    // ---- Q = round(C' / P) from the top words (error of the estimate < 2^-30)
     double top = (double)(long long)(((unsigned long long)c[NW] << 32) | c[NW - 1]);
     if constexpr (NW >= 2) top = fma((double)c[NW - 2], 2.3283064365386963e-10, top);
     const double qd = top * T.invP;
-    const double qr = floor(qd + 0.5);
-    const uint32_t Q = (uint32_t)(int)qr;
-    rare = fabs(qd - qr) > 0.5 - 9.5367431640625e-07;
-    uint32_t r[NW + 1];
-    long long br = 0;
+    const double qr = rint(qd);
+    const uint32_t Q = (uint32_t)__double2int_rn(qd);
+    rare = fabs(qd - qr) > 0.5 - 9.5367431640625e-07;                 // within 2^-20 of a half-integer: exact compare needed
+    // ---- R = C' - Q P in two's complement: C' - lo(Q P_t) 2^(32 t) - hi(Q P_t) 2^(32 (t + 1))
+    uint32_t lo[NW + 1], hi[NW + 1], r[NW + 1];
+    hi[0] = 0u;
 #pragma unroll
-    for (int t = 0; t <= NW; t++) {
-        long long s = (long long)c[t] + br - (long long)((unsigned long long)Q * (t < NW ? T.P[t] : 0u));
-        r[t] = (uint32_t)s;
-        br = s >> 32;
+    for (int t = 0; t < NW; t++) {
+        const unsigned long long pr = (unsigned long long)Q * T.P[t];
+        lo[t] = (uint32_t)pr;
+        hi[t + 1] = (uint32_t)(pr >> 32);
     }
+    lo[NW] = 0u;
+    mp_sub<NW + 1>(r, c, lo);
+    mp_sub<NW + 1>(r, r, hi);
+    // ---- |R| (NW words: |C''| <= P/2 < 2^(32 NW - 1)), branch-free negate
     const uint32_t negm = (uint32_t)((int32_t)r[NW] >> 31);
-    const unsigned long long m64 = (unsigned long long)(long long)(int32_t)negm;
-    auto W = [&](int t) -> uint32_t { return t <= NW ? r[t <= NW ? t : 0] : negm; };
-    const unsigned long long R0 = ((unsigned long long)W(1) << 32) | W(0);
-    const unsigned long long R1 = ((unsigned long long)W(3) << 32) | W(2);
-    const unsigned long long R2 = ((unsigned long long)W(5) << 32) | W(4);
-    const unsigned long long X0 = (R0 ^ m64) + (m64 & 1ull);
-    const unsigned long long c0 = (m64 & 1ull) & (unsigned long long)(X0 == 0ull);
-    const unsigned long long X1 = (R1 ^ m64) + c0;
-    const unsigned long long c1 = c0 & (unsigned long long)(X1 == 0ull);
-    const unsigned long long X2 = (R2 ^ m64) + c1;
+    uint32_t x[NW];
+#pragma unroll
+    for (int t = 0; t < NW; t++) x[t] = r[t] ^ negm;
+    mp_inc<NW>(x, negm & 1u);
+    // ---- top 64 bits from the leading one, sticky bit
+    auto X = [&](int t) -> uint32_t { return t < NW ? x[t < NW ? t : 0] : 0u; };
+    const unsigned long long X0 = ((unsigned long long)X(1) << 32) | X(0);
+    const unsigned long long X1 = ((unsigned long long)X(3) << 32) | X(2);
+    const unsigned long long X2 = (unsigned long long)X(4);
     const bool use2 = NW >= 5 && X2 != 0ull, use1 = !use2 && NW >= 3 && X1 != 0ull;
     const unsigned long long ptop = use2 ? X2 : (use1 ? X1 : X0), pmid = use2 ? X1 : (use1 ? X0 : 0ull), plow = use2 ? X0 : 0ull;
     const int base = use2 ? 128 : (use1 ? 64 : 0);
@@ -194,15 +250,25 @@ __device__ __forceinline__ TO crt_fast(const uint32_t (&c)[NW + 1], const Oz2Crt
     const int pos = base + 63 - lz, sc = pos - 63 - esum, Ex = pos - esum;
     if constexpr (sizeof(TO) == 8) {
         rare |= !zero && (Ex < -1020 || Ex > 1021);
-        const double d = __ull2double_rn(mant | sticky);
-        const long long bits = (__double_as_longlong(d) + ((long long)sc << 52)) | (long long)(m64 << 63);
-        return __longlong_as_double(zero ? 0ll : bits);
+        const double d = __ull2double_rn(mant | sticky);              // the one rounding, ties to even
+        const int hw = (__double2hiint(d) + (sc << 20)) | (int)(negm & 0x80000000u);
+        return zero ? 0.0 : __hiloint2double(hw, __double2loint(d));
     } else {
         rare |= !zero && (Ex < -124 || Ex > 125);
         const float d = __ull2float_rn(mant | sticky);
         const int bits = (__float_as_int(d) + sc * 8388608) | (int)(negm & 0x80000000u);
         return __int_as_float(zero ? 0 : bits);
     }
+}
+
+// by-value gate to crt_exact: the words travel in a struct so that the hot path keeps them in registers (an array
+// passed by reference to a non-inlined function would live in local memory for the whole loop)
+template <int NW>
+struct CWords { uint32_t w[NW + 1]; };
+template <int NW, typename TO>
+__device__ __noinline__ TO crt_exact_v(CWords<NW> cw, int N, int esum, uint64_t *cpp_out)
+{
+    return crt_exact<NW, TO>(cw.w, c_crt[N], esum, cpp_out);
 }
 
 // =============================================================================================
@@ -251,42 +317,54 @@ __device__ __forceinline__ void k5_fold(const uint32_t *S, uint32_t (&c)[NW + 1]
     c[NW] = (uint32_t)carry;
 }
 
-template <typename TO>
+template <bool BETA0, typename TO>
 __device__ __forceinline__ void k5_store(TO cij, TO alpha, TO beta, TO *dst)
 {
     if constexpr (sizeof(TO) == 8) {
         const double tt = alpha * cij;
-        *dst = (beta == 0.0) ? tt : fma(beta, *dst, tt);
+        *dst = (BETA0 || beta == 0.0) ? tt : fma(beta, *dst, tt);
     } else {
         const float tt = __fmul_rn(alpha, cij);
-        *dst = (beta == 0.0f) ? tt : __fmaf_rn(beta, *dst, tt);
+        *dst = (BETA0 || beta == 0.0f) ? tt : __fmaf_rn(beta, *dst, tt);
     }
 }
 
 // the two elements (i, j) and (i + 128, j) of one thread: C'' -> C -> alpha / beta -> store.  Both go through the
 // branch-free crt_fast side by side (two independent dependency chains per thread); crt_exact is the rare path.
-template <int NW, bool WANT_CPP, typename TO>
-__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, const Oz2CrtTab &T, int64_t i, int64_t j,
-                                           int64_t m, int esum_a, int esum_b, TO alpha, TO beta, TO *__restrict__ C,
-                                           int64_t ldc, uint64_t *__restrict__ Cpp)
+template <int NW, bool WANT_CPP, bool BETA0, typename TO>
+__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, const CrtRegs<NW> &T, int N, bool ok_a, bool ok_b,
+                                           int esum_a, int esum_b, TO alpha, TO beta, TO *__restrict__ dst,
+                                           uint64_t *__restrict__ cpp)
 {
-    const bool ok_a = i < m, ok_b = i + 128 < m;
     uint32_t ca[NW + 1], cb[NW + 1];
     k5_fold<NW>(Sa, ca);
     k5_fold<NW>(Sb, cb);
-    bool rare_a, rare_b;
-    TO va = crt_fast<NW, TO>(ca, T, esum_a, rare_a);
-    TO vb = crt_fast<NW, TO>(cb, T, esum_b, rare_b);
-    if ((WANT_CPP || rare_a) && ok_a) va = crt_exact<NW, TO>(ca, T, esum_a, WANT_CPP ? Cpp + ((size_t)j * m + i) * 4 : nullptr);
-    if ((WANT_CPP || rare_b) && ok_b) vb = crt_exact<NW, TO>(cb, T, esum_b, WANT_CPP ? Cpp + ((size_t)j * m + i + 128) * 4 : nullptr);
-    TO *dst = C + i + j * ldc;
-    if (ok_a) k5_store<TO>(va, alpha, beta, dst);
-    if (ok_b) k5_store<TO>(vb, alpha, beta, dst + 128);
+    TO va, vb;
+    if constexpr (WANT_CPP) {
+        CWords<NW> wa, wb;
+#pragma unroll
+        for (int t = 0; t <= NW; t++) { wa.w[t] = ca[t]; wb.w[t] = cb[t]; }
+        va = ok_a ? crt_exact_v<NW, TO>(wa, N, esum_a, cpp) : (TO)0;
+        vb = ok_b ? crt_exact_v<NW, TO>(wb, N, esum_b, cpp + 128 * 4) : (TO)0;
+    } else {
+        bool rare_a, rare_b;
+        va = crt_fast<NW, TO>(ca, T, esum_a, rare_a);
+        vb = crt_fast<NW, TO>(cb, T, esum_b, rare_b);
+        if ((rare_a && ok_a) || (rare_b && ok_b)) {                   // rare: near-half quotient, subnormal or overflowing result
+            CWords<NW> wa, wb;
+#pragma unroll
+            for (int t = 0; t <= NW; t++) { wa.w[t] = ca[t]; wb.w[t] = cb[t]; }
+            if (rare_a && ok_a) va = crt_exact_v<NW, TO>(wa, N, esum_a, nullptr);
+            if (rare_b && ok_b) vb = crt_exact_v<NW, TO>(wb, N, esum_b, nullptr);
+        }
+    }
+    if (ok_a) k5_store<BETA0, TO>(va, alpha, beta, dst);
+    if (ok_b) k5_store<BETA0, TO>(vb, alpha, beta, dst + 128);
 }
 
-template <int NW, bool WANT_CPP, typename TO>
+template <int NW, bool WANT_CPP, bool BETA0, typename TO>
 __global__ void __launch_bounds__(K5_THREADS, NW <= 4 ? 3 : 2)
-k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n, const int32_t *__restrict__ e,
+k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const int32_t *__restrict__ e,
           const int32_t *__restrict__ f, TO alpha, TO beta, TO *__restrict__ C, int64_t ldc,
           uint64_t *__restrict__ Cpp)
 {
@@ -302,8 +380,10 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
     uint8_t *gen0 = smem_raw + (smem0 - smem_u32(smem_raw));                // generic pointer to the aligned base
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
-    const int64_t total = tiles_i * n;
+    // tile t = j * tiles_i + ib (ib fastest), walked with stride gridDim.x; (j, ib) advance without a division
+    const int tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
+    const int64_t total = (int64_t)tiles_i * n;
+    const int G = (int)gridDim.x;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < K5_STAGES; s++) {
@@ -333,16 +413,15 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
 
     if (warp == 0) {
         if (lane == 0) {
-            // tile t = j * tiles_i + ib, walked with stride gridDim.x without a division per tile
-            const int64_t step_j = (int64_t)gridDim.x / tiles_i, step_i = (int64_t)gridDim.x - step_j * tiles_i;
-            int64_t j = (int64_t)blockIdx.x / tiles_i, ib = (int64_t)blockIdx.x - j * tiles_i;
+            const int step_j = G / tiles_i, step_i = G - step_j * tiles_i;
+            int j = (int)blockIdx.x / tiles_i, ib = (int)blockIdx.x - j * tiles_i;
             int s = 0; uint32_t ph = 0;
-            for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+            for (int64_t t = blockIdx.x; t < total; t += G) {
                 mbar_wait_idle(empty + 8 * s, ph ^ 1u);          // the epilogue paces this kernel: poll lazily
                 mbar_expect_tx_a(full + 8 * s, K5_STAGE_BYTES);
                 const uint32_t dst = smem0 + s * K5_STAGE_BYTES;
-                tma_load_3d_a(&mapU, full + 8 * s, dst, (int)(ib * K5_TILE_I), (int)j, 0);
-                tma_load_3d_a(&mapU, full + 8 * s, dst + K5_STAGE_BYTES / 2, (int)(ib * K5_TILE_I + 128), (int)j, 0);
+                tma_load_3d_a(&mapU, full + 8 * s, dst, ib * K5_TILE_I, j, 0);
+                tma_load_3d_a(&mapU, full + 8 * s, dst + K5_STAGE_BYTES / 2, ib * K5_TILE_I + 128, j, 0);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
                 ib += step_i; j += step_j;
                 if (ib >= tiles_i) { ib -= tiles_i; j++; }
@@ -356,7 +435,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
                                    ((uint64_t)(256u >> 4) << 32) | (1ull << 46);
             // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
             const uint64_t adesc0 = ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
-            for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
+            for (int64_t t = blockIdx.x; t < total; t += G) {
                 mbar_wait_idle(tempty + 8 * b, bph ^ 1u);
                 mbar_wait_idle(full + 8 * s, ph);
                 tc_fence_after();
@@ -373,20 +452,32 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
     } else {
         const int q = warp & 3;                              // TMEM lane quarter of this warp
         const int set = (warp - 2) >> 2;                     // epilogue set 0 / 1 takes every second tile of the CTA
-        const Oz2CrtTab &T = c_crt[N];
+        CrtRegs<NW> T;
+#pragma unroll
+        for (int t = 0; t < NW; t++) T.P[t] = c_crt[N].P[t];
+        T.invP = c_crt[N].invP;
         int b = set; uint32_t bph = 0;
         // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
-        const int64_t t0 = (int64_t)blockIdx.x + (int64_t)set * gridDim.x;
-        int64_t j = t0 / tiles_i, ib = t0 - j * tiles_i;
-        const int64_t step_j = 2 * (int64_t)gridDim.x / tiles_i, step_i = 2 * (int64_t)gridDim.x - step_j * tiles_i;
+        const int64_t t0 = (int64_t)blockIdx.x + (int64_t)set * G;
+        int j = (int)(t0 / tiles_i), ib = (int)(t0 - (int64_t)j * tiles_i);
+        const int step_j = (2 * G) / tiles_i, step_i = 2 * G - step_j * tiles_i;
         const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
-        for (int64_t t = t0; t < total; t += 2 * (int64_t)gridDim.x) {
-            const int64_t i = ib * K5_TILE_I + q * 32 + lane;
-            const int64_t jcur = j;
+        const int il = q * 32 + lane;                        // row of this thread inside the tile (and il + 128)
+        int ib_loaded = -1, e0 = 0, e1 = 0;
+        int fnext = t0 < total ? __ldg(f + j) : 0;           // f_j of the tile about to be processed, loaded one tile ahead
+        for (int64_t t = t0; t < total; t += 2 * (int64_t)G) {
+            const int i = ib * K5_TILE_I + il;
+            const int jcur = j;
+            const bool ok_a = i < m, ok_b = i + 128 < m;
+            if (ib != ib_loaded) {                           // with gridDim.x a multiple of tiles_i this happens once
+                e0 = ok_a ? __ldg(e + i) : 0;
+                e1 = ok_b ? __ldg(e + i + 128) : 0;
+                ib_loaded = ib;
+            }
+            const int fj = fnext;
             ib += step_i; j += step_j;
             if (ib >= tiles_i) { ib -= tiles_i; j++; }
-            const int fj = __ldg(f + jcur);
-            const int e0 = i < m ? __ldg(e + i) : 0, e1 = i + 128 < m ? __ldg(e + i + 128) : 0;
+            if (t + 2 * (int64_t)G < total) fnext = __ldg(f + j);
             mbar_wait_a(tfull + 8 * b, bph);
             tc_fence_after();
             uint32_t S[BUF_COLS];
@@ -402,7 +493,11 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int64_t m, int64_t n,
             if (lane == 0) mbar_arrive_a(tempty + 8 * b);
             b += 2;
             if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
-            if (i < m) k5_finish2<NW, WANT_CPP, TO>(S, S + NS, T, i, jcur, m, e0 + fj, e1 + fj, alpha, beta, C, ldc, Cpp);
+            if (ok_a) {
+                TO *dst = C + i + (int64_t)jcur * ldc;
+                uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)jcur * m + i) * 4 : nullptr;
+                k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, T, N, ok_a, ok_b, e0 + fj, e1 + fj, alpha, beta, dst, cpp);
+            }
         }
     }
     __syncthreads();
@@ -425,12 +520,17 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
-    const int64_t tiles = ((m + K5_TILE_I - 1) / K5_TILE_I) * n;
+    const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I, tiles = tiles_i * n;
     const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads
     int64_t grid = (int64_t)sms * per_sm;
     if (grid > tiles) grid = tiles;
-    if (Cpp) k5_crt_tc<NW, true, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, Cpp);
-    else k5_crt_tc<NW, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, m, n, e, f, alpha, beta, C, ldc, nullptr);
+    // a grid that is a multiple of the tiles per column keeps every CTA on one row block (its exponents e_i stay in
+    // registers); worth it while it costs less than an eighth of the resident slots
+    if (tiles_i <= grid && grid - grid % tiles_i >= grid - grid / 8) grid -= grid % tiles_i;
+    const int mi = (int)m, ni = (int)n;
+    if (Cpp) k5_crt_tc<NW, true, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldc, Cpp);
+    else if (beta == (TO)0) k5_crt_tc<NW, false, true, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldc, nullptr);
+    else k5_crt_tc<NW, false, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldc, nullptr);
     oz2_count_launches(1);
     return (int)cudaGetLastError();
 }
