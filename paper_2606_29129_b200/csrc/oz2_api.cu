@@ -6,6 +6,7 @@
 
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <atomic>
 #include <mutex>
 #include <string.h>
@@ -231,6 +232,19 @@ Layout make_layout(int64_t m, int64_t n, int64_t k, int N, int mode)
     return L;
 }
 
+// GEMM variant of the path: CTA pairs on 256 x 256 tiles (cta_group::2; measured 4 - 5 % faster than one CTA per
+// 128 x 256 tile at 8192^3 under the board's power cap: a third less shared-memory fill per MMA), falling back to the
+// single-CTA kernel for m <= 128 and K-blocked products.  OZAKI2_GEMM=single in the environment when the library is
+// first used forces the single-CTA kernel (a tuning knob; results are identical).
+int path_gemm_variant()
+{
+    static const int v = [] {
+        const char *e = getenv("OZAKI2_GEMM");
+        return (e && strcmp(e, "single") == 0) ? OZ2_GEMM_PATH : OZ2_GEMM_PAIR;
+    }();
+    return v;
+}
+
 // widths: fast / prop  <= floor(P'_prop) + 1 bits, accurate <= floor(P'_accu) + 7 bits; the narrow conversion format
 // holds a' as a signed 64-bit integer, |a'| < 2^63
 bool needs_wide_words(int N, int mode)
@@ -331,7 +345,7 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
         OZ2_CUDA_TRY(cudaMemsetAsync(colmax, 0, sizeof(int32_t) * (size_t)n, st));
         if ((rc = oz2_launch_scale_accu_side(f32, strided_a, m, k, A, lda, amax, EA, Abar, L.kp, st))) return rc;
         if ((rc = oz2_launch_scale_accu_side(f32, strided_b, n, k, B, ldb, amax, EB, Bbar, L.kp, st))) return rc;
-        if ((rc = oz2_launch_gemm_tc(OZ2_GEMM_PATH, 1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
+        if ((rc = oz2_launch_gemm_tc(path_gemm_variant(), 1, 0, m, n, k, Abar, Bbar, L.kp, nullptr, L.mp, rowmax, colmax, st))) return rc;
         if ((rc = oz2_launch_scale_accu_finish(N, m, n, EA, EB, rowmax, colmax, e, f, st))) return rc;
     } else {
         if (strided_a) rc = oz2_launch_scale_rows(mode, N, f32, m, k, A, lda, amax, ssq, e, st);
@@ -350,7 +364,7 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[2], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[2], st));
     // ---- S3 residue GEMMs
-    if ((rc = oz2_launch_gemm_tc(OZ2_GEMM_PATH, N, 0, m, n, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
+    if ((rc = oz2_launch_gemm_tc(path_gemm_variant(), N, 0, m, n, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
     if (timing) OZ2_CUDA_TRY(cudaEventRecord(ev[3], st));
     if (uev) OZ2_CUDA_TRY(cudaEventRecord(uev[3], st));
     // ---- S4 + S5
@@ -449,7 +463,7 @@ static int host_pipelined_enqueue(int f32, int64_t m, int64_t n, int64_t k, doub
         OZ2_CUDA_TRY(cudaStreamWaitEvent(st, dev->evB[p], 0));
         if ((rc = oz2_launch_scale_cols(mode, N, f32, nc, k, dB + esz * (size_t)(j0 * k), k, f, st))) return rc;
         if ((rc = oz2_launch_convert(1, N, wide, f32, nc, k, dB + esz * (size_t)(j0 * k), k, f, RB, L.kp, st))) return rc;
-        if ((rc = oz2_launch_gemm_tc(OZ2_GEMM_PATH, N, 0, m, nc, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
+        if ((rc = oz2_launch_gemm_tc(path_gemm_variant(), N, 0, m, nc, k, RA, RB, L.kp, U, L.mp, nullptr, nullptr, st))) return rc;
         if ((rc = oz2_launch_crt(N, f32, m, nc, U, L.mp, e, f, alpha, beta, dC + esz * (size_t)(j0 * m), m, nullptr, st))) return rc;
         OZ2_CUDA_TRY(cudaEventRecord(dev->evC[p], st));
         OZ2_CUDA_TRY(cudaStreamWaitEvent(sd, dev->evC[p], 0));

@@ -11,7 +11,9 @@
 //   * epilogue: 16 warps (four per TMEM lane quarter, 64 accumulator columns each) read the accumulator with
 //     tcgen05.ld, reduce mod p_l and write one byte per element, overlapping the MMAs of the next tile,
 //   * persistent grid (one CTA per SM), static tile order: modulus-major, then groups of 32 M-tiles so that the
-//     148 tiles in flight share A / B panels in L2.
+//     148 tiles in flight share A / B panels in L2,
+//   * the path runs the CTA-pair form of this kernel (k3_residue_gemm_pair, cta_group::2, 256 x 256 tiles: each
+//     CTA loads its 128 rows of A and HALF of the B tile), the single-CTA form serves m <= 128 and K-blocked products.
 // INT32 accumulation wraps (never saturates): with reading R6 that keeps k <= 2^17 exact for p = 256.
 #include "oz2_common.cuh"
 #include "oz2_tc.cuh"
@@ -100,6 +102,103 @@ __device__ __forceinline__ TileCoord decode_tile(int64_t t, int tiles_m, int til
 // EPI = EPI_MODP: U[plane][j][mp] = acc mod p_(mod_base + plane);  EPI_MAX: rowmax / colmax of the accumulators;
 // EPI_NONE: the accumulator is handed back unread (the measured INT8 ceiling of this very loop, bench.py)
 enum { EPI_MODP = 0, EPI_MAX = 1, EPI_NONE = 2 };
+// Epilogue of one 128 x 256 accumulator: this warp's 32 TMEM lanes (rows m0 + 32 q + lane) x its 64-column slice.
+// EPI_MODP: reduce mod p_l, pack, store (or, for the later blocks of a K-blocked product, add to the stored residues);
+// EPI_MAX: row / column maxima (accurate mode); EPI_NONE: nothing.  taddr0 = TMEM address of lane 0 of the
+// accumulator buffer.
+template <int EPI>
+__device__ __forceinline__ void k3_epilogue(uint32_t tmem_buf, int plane, int m0, int n0, int q, int half, int lane, int mod_base,
+                                            int m, int n, int accum, uint8_t *__restrict__ U, int64_t mp,
+                                            int32_t *__restrict__ rowmax, int32_t *__restrict__ colmax)
+{
+    const int i = m0 + q * 32 + lane;                // output row of this thread
+    const uint32_t taddr = tmem_buf + ((uint32_t)(q * 32) << 16);
+    if (EPI == EPI_NONE) {
+        // nothing: MMA-only ceiling run
+    } else if (EPI == EPI_MODP) {
+        const int l = mod_base + plane;
+        const Oz2ModTab tb = c_mod[l];
+        if (!accum) {
+            // Packed path.  A thread holds 32 columns of ITS row; the bytes are packed four columns to a word and
+            // 4 x 4 byte blocks are transposed inside each lane quad (two shuffles + two byte permutes per word),
+            // after which lane 4g + t holds rows 4g .. 4g+3 of the columns = t (mod 4): 4-byte stores, a quarter
+            // of the store instructions and no per-element address arithmetic.
+            const int t4 = lane & 3, row4 = m0 + q * 32 + (lane & ~3);
+            const uint32_t selA = (t4 & 1) ? 0x3715u : 0x6240u, selB = (t4 & 2) ? 0x3276u : 0x5410u;
+#pragma unroll 1
+            for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
+                uint32_t v[32];
+                tc_ld32(taddr + (uint32_t)(cc * 32), v);
+                uint32_t W[8];
+                if (l == 0) {
+#pragma unroll
+                    for (int w = 0; w < 8; w++)
+                        W[w] = __byte_perm(__byte_perm(v[4 * w], v[4 * w + 1], 0x0040), __byte_perm(v[4 * w + 2], v[4 * w + 3], 0x0040), 0x5410);
+                } else {
+#pragma unroll
+                    for (int w = 0; w < 8; w++) {
+                        const uint32_t r0 = mod_p_i32((int32_t)v[4 * w], tb), r1 = mod_p_i32((int32_t)v[4 * w + 1], tb);
+                        const uint32_t r2 = mod_p_i32((int32_t)v[4 * w + 2], tb), r3 = mod_p_i32((int32_t)v[4 * w + 3], tb);
+                        W[w] = __byte_perm(__byte_perm(r0, r1, 0x0040), __byte_perm(r2, r3, 0x0040), 0x5410);
+                    }
+                }
+#pragma unroll
+                for (int w = 0; w < 8; w++) {
+                    uint32_t y = __shfl_xor_sync(0xffffffffu, W[w], 1);
+                    W[w] = __byte_perm(W[w], y, selA);
+                    y = __shfl_xor_sync(0xffffffffu, W[w], 2);
+                    W[w] = __byte_perm(W[w], y, selB);
+                }
+                const int col0 = n0 + cc * 32 + t4;
+                if (row4 < mp) {                       // rows m .. mp-1 are pitch padding: written, never read back
+                    uint8_t *o = U + ((int64_t)plane * n + col0) * mp + row4;
+#pragma unroll
+                    for (int w = 0; w < 8; w++) {
+                        if (col0 + 4 * w < n) *reinterpret_cast<uint32_t *>(o) = W[w];
+                        o += 4 * mp;
+                    }
+                }
+            }
+        } else {
+            // k blocked at 2^17: add the residues of the earlier blocks mod p, element by element
+            uint8_t *out = U + ((int64_t)plane * n + n0) * mp + i;
+#pragma unroll 1
+            for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
+                uint32_t v[32];
+                tc_ld32(taddr + (uint32_t)(cc * 32), v);
+                if (i < m) {
+#pragma unroll
+                    for (int u = 0; u < 32; u++) {
+                        const int j = n0 + cc * 32 + u;
+                        uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
+                        if (j < n) {
+                            uint8_t *o = out + (int64_t)(cc * 32 + u) * mp;
+                            r += *o;
+                            *o = (uint8_t)(l == 0 ? (r & 0xFFu) : (r >= tb.p ? r - tb.p : r));
+                        }
+                    }
+                }
+            }
+        }
+    } else {
+        int rmax = 0;
+#pragma unroll 1
+        for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
+            uint32_t v[32];
+            tc_ld32(taddr + (uint32_t)(cc * 32), v);
+#pragma unroll
+            for (int u = 0; u < 32; u++) {
+                const int j = n0 + cc * 32 + u;
+                int val = (i < m && j < n) ? (int)v[u] : 0;
+                rmax = max(rmax, val);
+                int cm = __reduce_max_sync(0xffffffffu, val);
+                if (lane == 0 && j < n && cm > 0) atomicMax(colmax + j, cm);
+            }
+        }
+        if (i < m && rmax > 0) atomicMax(rowmax + i, rmax);
+    }
+}
+
 template <int EPI>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, int nplanes,
@@ -186,92 +285,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
             const TileCoord c = decode_tile(t, tiles_m, tiles_n);
             mbar_wait_idle(smem_u32(tfull + as), aphase);
             tc_fence_after();
-            const int i = c.m0 + q * 32 + lane;                // output row of this thread
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TILE_N);
-            if (EPI == EPI_NONE) {
-                // nothing: MMA-only ceiling run
-            } else if (EPI == EPI_MODP) {
-                const int l = mod_base + c.plane;
-                const Oz2ModTab tb = c_mod[l];
-                if (!accum) {
-                    // Packed path.  A thread holds 32 columns of ITS row; the bytes are packed four columns to a word and
-                    // 4 x 4 byte blocks are transposed inside each lane quad (two shuffles + two byte permutes per word),
-                    // after which lane 4g + t holds rows 4g .. 4g+3 of the columns = t (mod 4): 4-byte stores, a quarter
-                    // of the store instructions and no per-element address arithmetic.
-                    const int t4 = lane & 3, row4 = c.m0 + q * 32 + (lane & ~3);
-                    const uint32_t selA = (t4 & 1) ? 0x3715u : 0x6240u, selB = (t4 & 2) ? 0x3276u : 0x5410u;
-#pragma unroll 1
-                    for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
-                        uint32_t v[32];
-                        tc_ld32(taddr + (uint32_t)(cc * 32), v);
-                        uint32_t W[8];
-                        if (l == 0) {
-#pragma unroll
-                            for (int w = 0; w < 8; w++)
-                                W[w] = __byte_perm(__byte_perm(v[4 * w], v[4 * w + 1], 0x0040), __byte_perm(v[4 * w + 2], v[4 * w + 3], 0x0040), 0x5410);
-                        } else {
-#pragma unroll
-                            for (int w = 0; w < 8; w++) {
-                                const uint32_t r0 = mod_p_i32((int32_t)v[4 * w], tb), r1 = mod_p_i32((int32_t)v[4 * w + 1], tb);
-                                const uint32_t r2 = mod_p_i32((int32_t)v[4 * w + 2], tb), r3 = mod_p_i32((int32_t)v[4 * w + 3], tb);
-                                W[w] = __byte_perm(__byte_perm(r0, r1, 0x0040), __byte_perm(r2, r3, 0x0040), 0x5410);
-                            }
-                        }
-#pragma unroll
-                        for (int w = 0; w < 8; w++) {
-                            uint32_t y = __shfl_xor_sync(0xffffffffu, W[w], 1);
-                            W[w] = __byte_perm(W[w], y, selA);
-                            y = __shfl_xor_sync(0xffffffffu, W[w], 2);
-                            W[w] = __byte_perm(W[w], y, selB);
-                        }
-                        const int col0 = c.n0 + cc * 32 + t4;
-                        if (row4 < mp) {                       // rows m .. mp-1 are pitch padding: written, never read back
-                            uint8_t *o = U + ((int64_t)c.plane * n + col0) * mp + row4;
-#pragma unroll
-                            for (int w = 0; w < 8; w++) {
-                                if (col0 + 4 * w < n) *reinterpret_cast<uint32_t *>(o) = W[w];
-                                o += 4 * mp;
-                            }
-                        }
-                    }
-                } else {
-                    // k blocked at 2^17: add the residues of the earlier blocks mod p, element by element
-                    uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
-#pragma unroll 1
-                    for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
-                        uint32_t v[32];
-                        tc_ld32(taddr + (uint32_t)(cc * 32), v);
-                        if (i < m) {
-#pragma unroll
-                            for (int u = 0; u < 32; u++) {
-                                const int j = c.n0 + cc * 32 + u;
-                                uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
-                                if (j < n) {
-                                    uint8_t *o = out + (int64_t)(cc * 32 + u) * mp;
-                                    r += *o;
-                                    *o = (uint8_t)(l == 0 ? (r & 0xFFu) : (r >= tb.p ? r - tb.p : r));
-                                }
-                            }
-                        }
-                    }
-                }
-            } else {
-                int rmax = 0;
-#pragma unroll 1
-                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
-                    uint32_t v[32];
-                    tc_ld32(taddr + (uint32_t)(cc * 32), v);
-#pragma unroll
-                    for (int u = 0; u < 32; u++) {
-                        const int j = c.n0 + cc * 32 + u;
-                        int val = (i < m && j < n) ? (int)v[u] : 0;
-                        rmax = max(rmax, val);
-                        int cm = __reduce_max_sync(0xffffffffu, val);
-                        if (lane == 0 && j < n && cm > 0) atomicMax(colmax + j, cm);
-                    }
-                }
-                if (i < m && rmax > 0) atomicMax(rowmax + i, rmax);
-            }
+            k3_epilogue<EPI>(tmem_base + (uint32_t)(as * TILE_N), c.plane, c.m0, c.n0, q, half, lane, mod_base, m, n, accum, U, mp, rowmax, colmax);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty + as);
@@ -444,43 +458,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
             const TileCoord c = decode_tile_pair(t, tiles_m, tiles_n);
             mbar_wait_a(tfull + 8 * as, aphase);
             tc_fence_after();
-            const int i = c.m0 + (int)rank * 128 + q * 32 + lane;
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * TILE_N);
-            if (EPI == EPI_NONE) {
-            } else if (EPI == EPI_MODP) {
-                const int l = mod_base + c.plane;
-                const Oz2ModTab tb = c_mod[l];
-                uint8_t *out = U + ((int64_t)c.plane * n + c.n0) * mp + i;
-#pragma unroll 1
-                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
-                    uint32_t v[32];
-                    tc_ld32(taddr + (uint32_t)(cc * 32), v);
-                    if (i < m) {
-#pragma unroll
-                        for (int u = 0; u < 32; u++) {
-                            const int j = c.n0 + cc * 32 + u;
-                            uint32_t r = l == 0 ? (v[u] & 0xFFu) : mod_p_i32((int32_t)v[u], tb);
-                            if (j < n) out[(int64_t)(cc * 32 + u) * mp] = (uint8_t)r;
-                        }
-                    }
-                }
-            } else {
-                int rmax = 0;
-#pragma unroll 1
-                for (int cc = half * (TILE_N / 32 / EPI_SPLIT); cc < (half + 1) * (TILE_N / 32 / EPI_SPLIT); cc++) {
-                    uint32_t v[32];
-                    tc_ld32(taddr + (uint32_t)(cc * 32), v);
-#pragma unroll
-                    for (int u = 0; u < 32; u++) {
-                        const int j = c.n0 + cc * 32 + u;
-                        int val = (i < m && j < n) ? (int)v[u] : 0;
-                        rmax = max(rmax, val);
-                        int cm = __reduce_max_sync(0xffffffffu, val);
-                        if (lane == 0 && j < n && cm > 0) atomicMax(colmax + j, cm);
-                    }
-                }
-                if (i < m && rmax > 0) atomicMax(rowmax + i, rmax);
-            }
+            k3_epilogue<EPI>(tmem_base + (uint32_t)(as * TILE_N), c.plane, c.m0 + (int)rank * 128, c.n0, q, half, lane, mod_base, m, n, 0, U, mp, rowmax, colmax);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(leader_tempty + 8 * as);
@@ -552,10 +530,11 @@ int oz2_gemm_upload_tables(const Oz2HostTables &t)
     return 0;
 }
 
-// variant OZ2_GEMM_PATH: one CTA per 128 x 256 tile -- what ozaki2_dgemm runs.  OZ2_GEMM_PAIR: CTA pairs on 256 x 256
-// tiles (cta_group::2); measured at 8192^3, N = 16 on random residues, 20 calls back to back: 5.98 / 6.06 ms single vs
-// 6.29 / 6.15 ms pairs, so it stays a tested alternative behind ozaki2_debug_residue_gemm.  OZ2_GEMM_MMA_ONLY: the
-// path kernel with the epilogue reduced to handing the accumulator back (INT8 ceiling of this loop; U untouched).
+// variant OZ2_GEMM_PAIR: CTA pairs on 256 x 256 tiles (cta_group::2) -- what ozaki2_dgemm runs for m > 128 and
+// k <= 2^17.  OZ2_GEMM_PATH: one CTA per 128 x 256 tile (small m, K-blocked products, OZAKI2_GEMM=single).  Measured at
+// 8192^3, N = 16, inside the step (profiles/r02_gemm_variants.md): pairs 5.54 - 5.66 ms, single 5.84 - 5.95 ms.
+// OZ2_GEMM_MMA_ONLY / OZ2_GEMM_PAIR_MMA_ONLY: the same kernels with the epilogue reduced to handing the accumulator
+// back (INT8 ceiling of the loop; U untouched).
 int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA,
                        const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
 {
