@@ -61,6 +61,7 @@ def parse_args():
     ap.add_argument("--moduli", type=int, default=0, help="number of moduli N (default: 16 / 20 / 16 for config 2 / 3 / 4)")
     ap.add_argument("--mode", type=int, default=2, help="0 accurate, 1 original fast, 2 revised fast (headline)")
     ap.add_argument("--size", type=int, default=0, help="m = n = k override (keeps the config's distribution)")
+    ap.add_argument("--phi", type=float, default=None, help="spread parameter of eq. (15) override (paper: 0 .. 4)")
     ap.add_argument("--protocol", default="fixed", choices=["fixed", "paper"],
                     help="paper: P:387-392 iteration caps (warm-up 3 s / 100, timed 12 s / 100) instead of --steps / --warmup")
     ap.add_argument("--sgemm", action="store_true", help="SURVEY 8(f) #1: the FP32 in / FP32 out variant (paper: N = 3..12)")
@@ -78,9 +79,10 @@ def parse_args():
 def workload_shape(args):
     import workloads as W
     c = W.CONFIGS[args.config]
+    phi = c["phi"] if args.phi is None else args.phi
     if args.size:
-        return args.size, args.size, args.size, c["phi"]
-    return c["m"], c["n"], c["k"], c["phi"]
+        return args.size, args.size, args.size, phi
+    return c["m"], c["n"], c["k"], phi
 
 
 def workload_name(args, m, n, k, phi, N, mode, f32=False):
@@ -197,7 +199,7 @@ def run_reference(args):
     N, mode = args.moduli, args.mode
     ms, ns, _ = cpu_slab_shape(m, n, k)
     # the slab keeps the workload's distribution: same generator, same phi, shape (ms, ns, k)
-    A, B = W.config_matrices(args.config, 0, shape=(ms, ns, k))
+    A, B = W.eq15_matrices(ms, ns, k, phi, W.seed_for(args.config, 0))
     steps, warm = max(1, min(args.steps, 3)), max(0, min(args.warmup, 1))
     threads = 0
     for _ in range(warm):
@@ -287,7 +289,7 @@ def main():
     flops = 2.0 * m * n * k
 
     # ---- inputs: eq. (15), seeded, one variant per rank (replicas)
-    A, B = W.config_matrices(args.config, rank, shape=(m, n, k))
+    A, B = W.eq15_matrices(m, n, k, phi, W.seed_for(args.config, rank))
     f32 = bool(args.sgemm)
     npdt, tdt, esz = (np.float32, torch.float32, 4) if f32 else (np.float64, torch.float64, 8)
     if f32:

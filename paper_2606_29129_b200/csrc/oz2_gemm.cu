@@ -17,6 +17,7 @@
 // INT32 accumulation wraps (never saturates): with reading R6 that keeps k <= 2^17 exact for p = 256.
 #include "oz2_common.cuh"
 #include "oz2_tc.cuh"
+#include <stdlib.h>
 
 namespace {
 
@@ -512,6 +513,8 @@ int num_sms()
         int dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const char *e = getenv("OZAKI2_GEMM_SMS");        // experiment knob: SMs the persistent GEMM grid may use
+        if (e && atoi(e) > 1 && atoi(e) < sms) sms = atoi(e);
     }
     return sms;
 }
