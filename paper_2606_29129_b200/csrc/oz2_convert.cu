@@ -6,11 +6,13 @@
 //     a'' = sum_i d_i 256^i      =>      a'' mod p_l  =  ( sum_i d_i (256^i mod p_l) ) mod p_l ,
 // i.e. (elements x digits) x (digits x moduli).  One tcgen05.mma kind::i8 (unsigned x unsigned, M = 128, K = 32,
 // N = up to 64) handles 128 "quads" = 512 elements: a K row of 32 bytes carries the 8-byte digit strings of the 4
-// consecutive elements of a quad side by side (two 16-byte strings when |a'| needs more than 63 bits), and the B
-// operand is a constant block-diagonal image of the byte weights 256^i mod p_l, so that accumulator column
-// (l, slot) holds  Y = sum_i d_i(slot) (256^i mod p_l) < 2^20.  A second MMA with a constant all-ones operand adds a
-// per-modulus bias.  What is left for the CUDA cores is 2 multiplies per element and modulus and a packed store:
-//     a''  = a' + 2^63 (two's complement of a' with the top bit flipped: non-negative, sign handled for free),
+// consecutive elements of a quad side by side, and the B operand is a constant block-diagonal image of the byte
+// weights 256^i mod p_l, so that accumulator column (l, slot) holds  Y = sum_i d_i(slot) (256^i mod p_l) < 2^20.
+// When |a'| needs more than 63 bits (N >= 17, accurate mode from N = 15) a second K row carries digits 8 .. 11 and a
+// second MMA with the weights 256^(8+i) mod p_l accumulates onto the same columns.  One more MMA with a constant
+// all-ones operand adds a per-modulus bias.  What is left for the CUDA cores is 2 multiplies per element and modulus and a packed store:
+//     a''  = a' + 2^63 (two's complement of a' with the top bit flipped: non-negative, sign handled for free;
+//            2^95 in the wide format),
 //     bias = (p-1)/2 - 2^63 mod p,  Y ~ a' + (p-1)/2 (mod p),  u = Y mod p = Y - umulhi(Y, magic) p  in [0, p),
 //     r    = u - (p-1)/2  in [-(p-1)/2, (p-1)/2]  is the symmetric residue (reading R5 for p = 256, where the
 //     byte is simply the low byte of a'); four u bytes are packed, the per-byte offset 128 - (p-1)/2 is added to the
@@ -44,8 +46,10 @@ constexpr int CV_ONES_BYTES = 256;                 // all-ones A operand of the 
 constexpr int CV_TMEM_COLS = 64;
 constexpr int CV_CHUNK_H = 4 * CV_THREADS;         // contiguous side: h per round
 
-// operand images: [wide][0: byte weights, 1: bias][2048], canonical no-swizzle K-major layout (see tile_off)
-__device__ uint8_t g_conv_img[2][2][CV_IMG_BYTES];
+// operand images in the canonical no-swizzle K-major layout (see tile_off), 64 accumulator columns (= 16 moduli x 4
+// slots) each.  [g][t]: column group g (moduli 16 g .. 16 g + 15), t = 0: weights of digits 0 .. 7, 1: weights of
+// digits 8 .. 11 (wide format), 2: bias of the narrow format, 3: bias of the wide format.
+__device__ uint8_t g_conv_img[2][4][CV_IMG_BYTES];
 
 // byte offset of (row r, K byte kb) in a K-major, no-swizzle operand: 8 x 16-byte core matrices,
 // K-direction core-matrix stride (LBO) 128 B, 8-row group stride (SBO) 256 B
@@ -136,24 +140,26 @@ __device__ __forceinline__ void digits_wide(double a, int ex, uint32_t (&w)[3])
 // ---------------------------------------------------------------------------------------------
 // per-round tensor-core step and epilogue
 // ---------------------------------------------------------------------------------------------
+template <int WIDE>
 struct ConvSmem {                                   // dynamic shared memory, 128-byte aligned base
-    uint8_t tile[CV_TILE_BYTES];
+    uint8_t tile[WIDE ? 2 : 1][CV_TILE_BYTES];      // K rows of digits 0 .. 7 (and 8 .. 11)
     uint8_t ones[CV_ONES_BYTES];
-    uint8_t imgw[CV_IMG_BYTES];
-    uint8_t imgb[CV_IMG_BYTES];
+    uint8_t img[WIDE ? 6 : 2][CV_IMG_BYTES];        // narrow: weights, bias; wide: + high-digit weights, and all three for moduli 16 ..
     uint64_t mbar;
-    uint32_t tmem_slot;
-    uint32_t pad;
+    uint32_t tmem_slot[2];
 };
 
 struct ConvCtx {
     uint32_t tile_row;          // shared address of this thread's 32-byte K row (first 16 bytes; +128 for the rest)
     uint32_t mbar;              // shared address of the MMA-done barrier
     uint32_t phase;
-    uint32_t tmem;              // TMEM address of this thread's lane, column 0
+    uint32_t tmem;              // TMEM address of this thread's lane, column 0 (moduli 0 .. 15)
     uint32_t tmem_base;
+    uint32_t tmem2, tmem2_base; // wide format: the 32-column accumulator of moduli 16 .. 19
     uint64_t adesc, bdesc, odesc, biasdesc;
-    uint32_t idesc;
+    uint64_t ahdesc, bhdesc;    // wide format: K rows / weights of digits 8 .. 11
+    uint64_t b2desc, bh2desc, bias2desc;
+    uint32_t idesc, idesc2;     // idesc2 == 0: no second column group
 };
 
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
@@ -161,7 +167,8 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, ui
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
 
-// all 128 K rows are in place: run the two MMAs (digits x weights, ones x bias) and wait for the accumulator
+// all 128 K rows are in place: run the MMAs (digits x weights, ones x bias) and wait for the accumulator
+template <int WIDE>
 __device__ __forceinline__ void conv_mma(ConvCtx &cx)
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy stores -> tensor-core reads
@@ -170,7 +177,13 @@ __device__ __forceinline__ void conv_mma(ConvCtx &cx)
     if (threadIdx.x == 0) {
         tc_fence_after();
         tc_mma_i8(cx.tmem_base, cx.adesc, cx.bdesc, cx.idesc, 0u);
+        if (WIDE) tc_mma_i8(cx.tmem_base, cx.ahdesc, cx.bhdesc, cx.idesc, 1u);
         tc_mma_i8(cx.tmem_base, cx.odesc, cx.biasdesc, cx.idesc, 1u);
+        if (WIDE && cx.idesc2) {
+            tc_mma_i8(cx.tmem2_base, cx.adesc, cx.b2desc, cx.idesc2, 0u);
+            tc_mma_i8(cx.tmem2_base, cx.ahdesc, cx.bh2desc, cx.idesc2, 1u);
+            tc_mma_i8(cx.tmem2_base, cx.odesc, cx.bias2desc, cx.idesc2, 1u);
+        }
         tc_commit_a(cx.mbar);
     }
 }
@@ -221,7 +234,8 @@ __device__ __forceinline__ void store_group4(const uint32_t *v, int N, int8_t *d
     }
 }
 
-__device__ __forceinline__ void epilogue_narrow(const ConvCtx &cx, int N, int8_t *dst, int64_t plane_stride, bool ok)
+template <int WIDE>
+__device__ __forceinline__ void conv_epilogue(const ConvCtx &cx, int N, int8_t *dst, int64_t plane_stride, bool ok)
 {
     uint32_t v[32];
     tc_ld32(cx.tmem, v);
@@ -236,57 +250,13 @@ __device__ __forceinline__ void epilogue_narrow(const ConvCtx &cx, int N, int8_t
             if (N > 12) store_group4<12>(v + 16, N, dst, plane_stride);
         }
     }
-}
-
-// wide epilogue: accumulator column = 2 l + slot; a round has two MMA passes (elements 0, 1 and 2, 3 of the quad).
-// Pass 0 keeps u0 | u1 << 8 per modulus in H[], pass 1 completes the words.
-template <int L>
-__device__ __forceinline__ uint32_t half_word(uint32_t y0, uint32_t y1)
-{
-    if constexpr (L == 0) return __byte_perm(y0, y1, 0x0040) & 0xFFFFu;
-    else return __byte_perm(umod<L>(y0), umod<L>(y1), 0x0040) & 0xFFFFu;
-}
-template <int L>
-__device__ __forceinline__ uint32_t finish_word(uint32_t h)
-{
-    if constexpr (L == 0) return h;
-    else {
-        constexpr uint32_t half = (modulus_of(L) - 1) / 2, c = (128u - half) * 0x01010101u;
-        return (h + c) ^ 0x80808080u;
-    }
-}
-template <int L0, int PASS>
-__device__ __forceinline__ void wide_group4(const uint32_t *v, int N, uint32_t *H, int8_t *dst, int64_t plane_stride, bool ok)
-{
-    // v: 8 accumulator values (4 moduli x 2 slots) of moduli L0 .. L0 + 3
-    if (L0 >= N) return;
-    uint32_t h0 = half_word<L0 + 0>(v[0], v[1]), h1 = half_word<L0 + 1 < OZ2_MAX_MODULI ? L0 + 1 : 0>(v[2], v[3]);
-    uint32_t h2 = half_word<L0 + 2 < OZ2_MAX_MODULI ? L0 + 2 : 0>(v[4], v[5]), h3 = half_word<L0 + 3 < OZ2_MAX_MODULI ? L0 + 3 : 0>(v[6], v[7]);
-    if (PASS == 0) {
-        H[L0 + 0] = h0; H[L0 + 1] = h1; H[L0 + 2] = h2; H[L0 + 3] = h3;
-    } else if (ok) {
-        *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 0) * plane_stride) = finish_word<L0 + 0>(H[L0 + 0] | (h0 << 16));
-        if (L0 + 1 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 1) * plane_stride) = finish_word<L0 + 1 < OZ2_MAX_MODULI ? L0 + 1 : 0>(H[L0 + 1] | (h1 << 16));
-        if (L0 + 2 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 2) * plane_stride) = finish_word<L0 + 2 < OZ2_MAX_MODULI ? L0 + 2 : 0>(H[L0 + 2] | (h2 << 16));
-        if (L0 + 3 < N) *reinterpret_cast<uint32_t *>(dst + (int64_t)(L0 + 3) * plane_stride) = finish_word<L0 + 3 < OZ2_MAX_MODULI ? L0 + 3 : 0>(H[L0 + 3] | (h3 << 16));
-    }
-}
-template <int PASS>
-__device__ __forceinline__ void epilogue_wide(const ConvCtx &cx, int N, uint32_t *H, int8_t *dst, int64_t plane_stride, bool ok)
-{
-    uint32_t v[32];
-    tc_ld32(cx.tmem, v);                                              // moduli 0 .. 15
-    wide_group4<0, PASS>(v, N, H, dst, plane_stride, ok);
-    wide_group4<4, PASS>(v + 8, N, H, dst, plane_stride, ok);
-    wide_group4<8, PASS>(v + 16, N, H, dst, plane_stride, ok);
-    wide_group4<12, PASS>(v + 24, N, H, dst, plane_stride, ok);
-    if (N > 16) {                                                     // uniform; moduli 16 .. 19 (columns 32 .. 39)
-        tc_ld32(cx.tmem + 32u, v);
-        wide_group4<16, PASS>(v, N, H, dst, plane_stride, ok);
+    if (WIDE && N > 16) {                                             // uniform; second accumulator: moduli 16 .. 19
+        tc_ld32(cx.tmem2, v);
+        if (ok) store_group4<16>(v, N, dst, plane_stride);
     }
 }
 
-// one quad: digits -> K row -> MMA -> residues of all N moduli -> 4-byte stores.  `overlap()` runs between the MMA
+// one quad: digits -> K row(s) -> MMA -> residues of all N moduli -> 4-byte stores.  `overlap()` runs between the MMA
 // issue and the wait for its result (the callers put the loads of their next work item there).
 template <int WIDE, typename F>
 __device__ __forceinline__ void convert_quad(ConvCtx &cx, const double (&a)[4], int ex, int N, int8_t *dst,
@@ -297,39 +267,41 @@ __device__ __forceinline__ void convert_quad(ConvCtx &cx, const double (&a)[4], 
         const unsigned long long d2 = digits_narrow(a[2], ex), d3 = digits_narrow(a[3], ex);
         sts128(cx.tile_row, (uint32_t)d0, (uint32_t)(d0 >> 32), (uint32_t)d1, (uint32_t)(d1 >> 32));
         sts128(cx.tile_row + 128u, (uint32_t)d2, (uint32_t)(d2 >> 32), (uint32_t)d3, (uint32_t)(d3 >> 32));
-        conv_mma(cx);
-        overlap();
-        conv_wait(cx);
-        epilogue_narrow(cx, N, dst, plane_stride, ok);
     } else {
-        uint32_t H[OZ2_MAX_MODULI + 4];
-        uint32_t w[3];
-        digits_wide(a[0], ex, w);
-        sts128(cx.tile_row, w[0], w[1], w[2], 0u);
-        digits_wide(a[1], ex, w);
-        sts128(cx.tile_row + 128u, w[0], w[1], w[2], 0u);
-        conv_mma(cx);
-        overlap();
-        conv_wait(cx);
-        epilogue_wide<0>(cx, N, H, dst, plane_stride, ok);
-        digits_wide(a[2], ex, w);
-        sts128(cx.tile_row, w[0], w[1], w[2], 0u);
-        digits_wide(a[3], ex, w);
-        sts128(cx.tile_row + 128u, w[0], w[1], w[2], 0u);
-        conv_mma(cx);
-        conv_wait(cx);
-        epilogue_wide<1>(cx, N, H, dst, plane_stride, ok);
+        uint32_t w0[3], w1[3], w2[3], w3[3];
+        digits_wide(a[0], ex, w0);
+        digits_wide(a[1], ex, w1);
+        digits_wide(a[2], ex, w2);
+        digits_wide(a[3], ex, w3);
+        sts128(cx.tile_row, w0[0], w0[1], w1[0], w1[1]);
+        sts128(cx.tile_row + 128u, w2[0], w2[1], w3[0], w3[1]);
+        sts128(cx.tile_row + CV_TILE_BYTES, w0[2], 0u, w1[2], 0u);             // digits 8 .. 11 (12 .. 15 are zero)
+        sts128(cx.tile_row + CV_TILE_BYTES + 128u, w2[2], 0u, w3[2], 0u);
     }
+    conv_mma<WIDE>(cx);
+    overlap();
+    conv_wait(cx);
+    conv_epilogue<WIDE>(cx, N, dst, plane_stride, ok);
 }
 
 // CTA prologue: operand images, barrier, tensor memory
 template <int WIDE>
-__device__ __forceinline__ void conv_setup(ConvSmem *S, ConvCtx &cx, int N)
+__device__ __forceinline__ void conv_setup(ConvSmem<WIDE> *S, ConvCtx &cx, int N)
 {
     const int tid = threadIdx.x;
+    // images: narrow {weights, bias}; wide {weights lo, weights hi, bias} for moduli 0 .. 15 and the same for 16 .. 19
     for (int t = tid; t < CV_IMG_BYTES / 16; t += CV_THREADS) {
-        reinterpret_cast<uint4 *>(S->imgw)[t] = reinterpret_cast<const uint4 *>(g_conv_img[WIDE][0])[t];
-        reinterpret_cast<uint4 *>(S->imgb)[t] = reinterpret_cast<const uint4 *>(g_conv_img[WIDE][1])[t];
+        if (!WIDE) {
+            reinterpret_cast<uint4 *>(S->img[0])[t] = reinterpret_cast<const uint4 *>(g_conv_img[0][0])[t];
+            reinterpret_cast<uint4 *>(S->img[1])[t] = reinterpret_cast<const uint4 *>(g_conv_img[0][2])[t];
+        } else {
+#pragma unroll
+            for (int g = 0; g < 2; g++) {
+                reinterpret_cast<uint4 *>(S->img[3 * g + 0])[t] = reinterpret_cast<const uint4 *>(g_conv_img[g][0])[t];
+                reinterpret_cast<uint4 *>(S->img[3 * g + 1])[t] = reinterpret_cast<const uint4 *>(g_conv_img[g][1])[t];
+                reinterpret_cast<uint4 *>(S->img[3 * g + 2])[t] = reinterpret_cast<const uint4 *>(g_conv_img[g][3])[t];
+            }
+        }
     }
     if (tid < CV_ONES_BYTES / 16)                                     // K byte 0 of every row = 1: first byte of the 8 core rows of K chunk 0
         reinterpret_cast<uint4 *>(S->ones)[tid] = make_uint4(tid < 8 ? 1u : 0u, 0u, 0u, 0u);
@@ -338,40 +310,60 @@ __device__ __forceinline__ void conv_setup(ConvSmem *S, ConvCtx &cx, int N)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    const bool second = WIDE && N > 16;
     if (tid < 32) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&S->tmem_slot)), "n"(CV_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&S->tmem_slot[0])), "n"(CV_TMEM_COLS) : "memory");
+        if (second)
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" ::"r"(smem_u32(&S->tmem_slot[1])) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    cx.tmem_base = S->tmem_slot;
-    cx.tmem = cx.tmem_base + ((uint32_t)(tid & ~31) << 16);          // lane quarter of this warp
-    cx.tile_row = smem_u32(S->tile) + (uint32_t)tile_off(tid, 0);
+    const uint32_t lane_off = (uint32_t)(tid & ~31) << 16;            // lane quarter of this warp
+    cx.tmem_base = S->tmem_slot[0];
+    cx.tmem = cx.tmem_base + lane_off;
+    cx.tmem2_base = second ? S->tmem_slot[1] : 0u;
+    cx.tmem2 = cx.tmem2_base + lane_off;
+    cx.tile_row = smem_u32(S->tile[0]) + (uint32_t)tile_off(tid, 0);
     cx.mbar = smem_u32(&S->mbar);
     cx.phase = 0;
-    cx.adesc = kmajor_desc(smem_u32(S->tile), 256u);
+    cx.adesc = kmajor_desc(smem_u32(S->tile[0]), 256u);
     cx.odesc = kmajor_desc(smem_u32(S->ones), 0u);                    // every 8-row group reads the same 256 bytes
-    cx.bdesc = kmajor_desc(smem_u32(S->imgw), 256u);
-    cx.biasdesc = kmajor_desc(smem_u32(S->imgb), 256u);
-    // accumulator columns in use: 4 per modulus (narrow) / 2 per modulus (wide), rounded up to the MMA's N granule of 16
-    const int cols = WIDE ? 2 * N : 4 * N;
-    const uint32_t nmma = (uint32_t)((cols + 15) & ~15);
+    cx.bdesc = kmajor_desc(smem_u32(S->img[0]), 256u);
+    if (!WIDE) {
+        cx.biasdesc = kmajor_desc(smem_u32(S->img[1]), 256u);
+        cx.ahdesc = cx.bhdesc = cx.b2desc = cx.bh2desc = cx.bias2desc = 0;
+    } else {
+        cx.ahdesc = kmajor_desc(smem_u32(S->tile[WIDE ? 1 : 0]), 256u);
+        cx.bhdesc = kmajor_desc(smem_u32(S->img[1]), 256u);
+        cx.biasdesc = kmajor_desc(smem_u32(S->img[2]), 256u);
+        cx.b2desc = kmajor_desc(smem_u32(S->img[WIDE ? 3 : 0]), 256u);
+        cx.bh2desc = kmajor_desc(smem_u32(S->img[WIDE ? 4 : 0]), 256u);
+        cx.bias2desc = kmajor_desc(smem_u32(S->img[WIDE ? 5 : 0]), 256u);
+    }
+    // accumulator columns in use: 4 per modulus, rounded up to the MMA's N granule of 16; moduli 16 .. 19 in the second group
+    const int n1 = N < 16 ? N : 16;
+    const uint32_t nmma = (uint32_t)((4 * n1 + 15) & ~15);
     // kind::i8: D = S32, A = B = unsigned 8 bit, both K-major, M = 128
     cx.idesc = (2u << 4) | ((nmma >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+    cx.idesc2 = second ? ((2u << 4) | ((16u >> 3) << 17) | ((uint32_t)(128 >> 4) << 24)) : 0u;
 }
 
 __device__ __forceinline__ void conv_teardown(const ConvCtx &cx)
 {
     tc_fence_before();
     __syncthreads();
-    if (threadIdx.x < 32)
+    if (threadIdx.x < 32) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(cx.tmem_base), "n"(CV_TMEM_COLS) : "memory");
+        if (cx.idesc2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 32;" ::"r"(cx.tmem2_base) : "memory");
+    }
 }
 
-__device__ __forceinline__ ConvSmem *conv_smem(uint8_t *raw)
+template <int WIDE>
+__device__ __forceinline__ ConvSmem<WIDE> *conv_smem(uint8_t *raw)
 {
-    return reinterpret_cast<ConvSmem *>((reinterpret_cast<uintptr_t>(raw) + 127) & ~(uintptr_t)127);   // no swizzle: 16 B would do
+    return reinterpret_cast<ConvSmem<WIDE> *>((reinterpret_cast<uintptr_t>(raw) + 127) & ~(uintptr_t)127);   // no swizzle: 16 B would do
 }
 
 // four consecutive elements of a contiguous vector as doubles: two 16-byte loads (FP64) or one (FP32)
@@ -399,12 +391,12 @@ __device__ __forceinline__ void load_quad(const T *vec, int64_t h, int64_t k, bo
 // contiguous vectors: vector j is X[h + j ldx].  Work item = (vector, chunk of 512 h), persistent CTAs.
 // ---------------------------------------------------------------------------------------------
 template <int WIDE, typename T>
-__global__ void __launch_bounds__(CV_THREADS, WIDE ? 6 : 8)
+__global__ void __launch_bounds__(CV_THREADS, WIDE ? 5 : 8)
 k2_tc_cols(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx, const int32_t *__restrict__ ex,
            int8_t *__restrict__ planes, int64_t kp)
 {
     extern __shared__ uint8_t smem_raw[];
-    ConvSmem *S = conv_smem(smem_raw);
+    ConvSmem<WIDE> *S = conv_smem<WIDE>(smem_raw);
     ConvCtx cx;
     conv_setup<WIDE>(S, cx, N);
     const int tid = threadIdx.x;
@@ -463,12 +455,12 @@ __device__ __forceinline__ void cp_async_zfill(uint32_t dst, const void *src, bo
 }
 
 template <int WIDE, typename T>
-__global__ void __launch_bounds__(CV_THREADS, WIDE ? 6 : 8)
+__global__ void __launch_bounds__(CV_THREADS, WIDE ? 5 : 8)
 k2_tc_rows(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx, const int32_t *__restrict__ ex,
            int8_t *__restrict__ planes, int64_t kp)
 {
     extern __shared__ uint8_t smem_raw[];
-    ConvSmem *S = conv_smem(smem_raw);
+    ConvSmem<WIDE> *S = conv_smem<WIDE>(smem_raw);
     constexpr int PITCH = StageRow<T>::PITCH;
     T *stage = reinterpret_cast<T *>(S + 1);
     ConvCtx cx;
@@ -620,9 +612,10 @@ int num_sms()
     return sms;
 }
 
-template <typename T>
-constexpr size_t rows_smem() { return sizeof(ConvSmem) + 128 + (size_t)ST_ROWS * StageRow<T>::PITCH * sizeof(T); }
-constexpr size_t cols_smem() { return sizeof(ConvSmem) + 128; }
+template <int WIDE, typename T>
+constexpr size_t rows_smem() { return sizeof(ConvSmem<WIDE>) + 128 + (size_t)ST_ROWS * StageRow<T>::PITCH * sizeof(T); }
+template <int WIDE>
+constexpr size_t cols_smem() { return sizeof(ConvSmem<WIDE>) + 128; }
 
 template <typename T>
 int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *X, int64_t ldx, const int32_t *ex,
@@ -637,19 +630,19 @@ int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *
             k2_bar_cols<T><<<(unsigned)((total + BAR_THREADS - 1) / BAR_THREADS), BAR_THREADS, 0, st>>>(rows, k, X, ldx, ex, planes, kp);
         }
     } else {
-        const int per_sm = wide ? 6 : 8;              // tensor memory: 64 columns per CTA
+        const int per_sm = wide ? 5 : 8;              // tensor memory: 64 (+ 32) columns per CTA
         if (op == 0) {
             const int64_t items = ((rows + ST_ROWS - 1) / ST_ROWS) * (kp / ST_H);
             int64_t grid = (int64_t)num_sms() * per_sm;
             if (grid > items) grid = items;
-            if (wide) k2_tc_rows<1, T><<<(unsigned)grid, CV_THREADS, rows_smem<T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
-            else k2_tc_rows<0, T><<<(unsigned)grid, CV_THREADS, rows_smem<T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            if (wide) k2_tc_rows<1, T><<<(unsigned)grid, CV_THREADS, rows_smem<1, T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            else k2_tc_rows<0, T><<<(unsigned)grid, CV_THREADS, rows_smem<0, T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
         } else {
             const int64_t items = rows * ((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);
             int64_t grid = (int64_t)num_sms() * per_sm;
             if (grid > items) grid = items;
-            if (wide) k2_tc_cols<1, T><<<(unsigned)grid, CV_THREADS, cols_smem(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
-            else k2_tc_cols<0, T><<<(unsigned)grid, CV_THREADS, cols_smem(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            if (wide) k2_tc_cols<1, T><<<(unsigned)grid, CV_THREADS, cols_smem<1>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            else k2_tc_cols<0, T><<<(unsigned)grid, CV_THREADS, cols_smem<0>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
         }
     }
     oz2_count_launches(1);
@@ -661,32 +654,34 @@ int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *
 
 int oz2_convert_upload_tables(const Oz2HostTables &t)
 {
-    static uint8_t img[2][2][CV_IMG_BYTES];
+    static uint8_t img[2][4][CV_IMG_BYTES];
     memset(img, 0, sizeof(img));
-    for (int wide = 0; wide < 2; wide++) {
-        const int slots = wide ? 2 : 4, digits = wide ? 12 : 8, kstride = wide ? 16 : 8, topbit = wide ? 95 : 63;
-        for (int l = 0; l < OZ2_MAX_MODULI; l++) {
-            const uint32_t p = t.mod[l].p;
-            uint32_t two = 1 % p;                                    // 2^topbit mod p
-            for (int b = 0; b < topbit; b++) two = (two * 2u) % p;
-            const uint32_t half = (p - 1) / 2;
-            const uint32_t bias = l == 0 ? 0u : (half + p - two) % p;      // Y ~ a' + half (mod p); p = 256 keeps the low byte
-            for (int s = 0; s < slots; s++) {
-                const int col = l * slots + s;
-                if (col >= 64) continue;
-                for (int i = 0; i < digits; i++) {
-                    const uint32_t w = (t.mod[l].wb[i / 4] >> (8 * (i % 4))) & 0xFFu;   // 256^i mod p
-                    img[wide][0][tile_off(col, kstride * s + i)] = (uint8_t)w;
-                }
-                img[wide][1][tile_off(col, 0)] = (uint8_t)bias;
+    for (int l = 0; l < OZ2_MAX_MODULI; l++) {
+        const uint32_t p = t.mod[l].p, half = (p - 1) / 2;
+        const int g = l / 16;
+        uint32_t two = 1 % p, bias[2] = { 0u, 0u };                  // 2^b mod p; bias = half - 2^topbit mod p: Y ~ a' + half (mod p)
+        for (int b = 0; b <= 95; b++) {
+            if (b == 63) bias[0] = (half + p - two) % p;
+            if (b == 95) bias[1] = (half + p - two) % p;
+            two = (two * 2u) % p;
+        }
+        if (l == 0) bias[0] = bias[1] = 0u;                           // p = 256 keeps the low byte of a'
+        for (int s = 0; s < 4; s++) {
+            const int col = (l % 16) * 4 + s;
+            for (int i = 0; i < 12; i++) {
+                const uint32_t w = (t.mod[l].wb[i / 4] >> (8 * (i % 4))) & 0xFFu;          // 256^i mod p
+                if (i < 8) img[g][0][tile_off(col, 8 * s + i)] = (uint8_t)w;
+                else img[g][1][tile_off(col, 8 * s + i - 8)] = (uint8_t)w;
             }
+            img[g][2][tile_off(col, 0)] = (uint8_t)bias[0];
+            img[g][3][tile_off(col, 0)] = (uint8_t)bias[1];
         }
     }
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(g_conv_img, img, sizeof(img)));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<0, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<double>()));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<1, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<double>()));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<float>()));
-    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<1, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<float>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<0, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<0, double>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<1, double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<1, double>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<0, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<0, float>()));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k2_tc_rows<1, float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rows_smem<1, float>()));
     return 0;
 }
 
