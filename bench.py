@@ -440,17 +440,18 @@ def main():
         if mode != 0:       # e_i, f_j of modes 1, 2 depend on their own row / column only: the slab of C is comparable
             Cg = Cd[:ns_, :ms_].cpu().numpy().T
             cpu["gpu_slab_bit_exact_vs_oracle"] = bool(np.array_equal(Cg, Cs))
-    if rank == 0 and world == 1 and args.accuracy and not f32:
+    if rank == 0 and world == 1 and args.accuracy:
         # max elementwise relative error against a double-double reference, on a sampled slab of the GPU's C
+        # (SGEMM: the reference is the double-double product of the promoted FP32 inputs)
         from oracle import ozaki2_oracle as O
         ra, ca = min(m, 256), min(n, 512)
-        hi, lo = O.dd_reference(np.asfortranarray(A[:ra, :]), np.asfortranarray(B[:, :ca]))
-        Cg = Cd[:ca, :ra].cpu().numpy().T
+        hi, lo = O.dd_reference(np.asfortranarray(A[:ra, :].astype(np.float64)), np.asfortranarray(B[:, :ca].astype(np.float64)))
+        Cg = Cd[:ca, :ra].cpu().numpy().T.astype(np.float64)
         nz = hi != 0
         accuracy = dict(max_rel_err=float(np.max(np.abs((Cg[nz] - hi[nz]) - lo[nz]) / np.abs(hi[nz]))),
                         sample=f"rows 0..{ra - 1} x columns 0..{ca - 1} of C vs oracle double-double AB",
                         zero_reference_entries=int(np.sum(~nz)))
-        if mode != 0:
+        if mode != 0 and not f32:
             g = pkg.dgemm_stages(Ad, Bd, N, mode, C_dev=Cd, want=("e", "f"))
             torch.cuda.synchronize()
             e, f = g["e"].cpu().numpy(), g["f"].cpu().numpy()

@@ -2,8 +2,9 @@
 scaling modes, plus the scale-invariance variant c in {2^-500, 1e-100, 1, 1e100, 2^500}.
 
 For every (N, mode) the CUDA result is compared bit for bit with the oracle's and its max elementwise relative error
-against the double-double reference is recorded; the table is written to
-gpurun_out/accuracy_report.md (copied to profiles/ by hand).  Assertions are the paper's claims as trends."""
+against the double-double reference is recorded.  The two table builders return their markdown lines to
+the caller: the tests assert the paper's claims as trends on the numbers, and running this file as a script prints the
+tables on stdout (that is how profiles/r02_accuracy.md is made: `python tests/test_gpu_report.py > ...`)."""
 import os
 
 import numpy as np
@@ -56,7 +57,8 @@ def slab_violations(A, Bm, e, f, N, rows=48, cols=48):
     return cnt["violations"], cnt["wrong"]
 
 
-def test_config1_error_vs_moduli_and_modes(B):
+def config1_error_table(B):
+    """(markdown lines, {(N, mode): max rel err}) for config 1; full-size bit-exact parity asserted on the way."""
     c = W.CONFIGS[1]
     A, Bm = W.config_matrices(1)
     hi, lo = O.dd_reference(A, Bm)
@@ -75,18 +77,22 @@ def test_config1_error_vs_moduli_and_modes(B):
             errs[(N, mode)] = max_rel_err(Cg, hi, lo)
             row.append(f"{errs[(N, mode)]:.3e}")
         lines.append(f"| {N} | " + " | ".join(row) + " |")
+    return lines, errs
+
+
+def test_config1_error_vs_moduli_and_modes(B):
+    c = W.CONFIGS[1]
+    _, errs = config1_error_table(B)
     # P:377 errors fall as N grows until the FP64 floor; P:383 prop ~ accu, fast worse at phi >= 1
     assert errs[(8, 2)] > 1e3 * errs[(12, 2)] > 1e6 * errs[(16, 2)]
     for N in c["moduli"]:
         assert errs[(N, 2)] <= 32 * errs[(N, 0)], N
     assert errs[(20, 2)] < 1e-15 and errs[(20, 0)] < 1e-15
     assert errs[(14, 1)] > 4 * errs[(14, 2)]
-    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
-    with open(os.path.join(ROOT, "gpurun_out", "accuracy_report.md"), "w") as fh:
-        fh.write("\n".join(lines) + "\n")
 
 
-def test_config1_scale_invariance_variant(B):
+def scale_invariance_table(B):
+    """(markdown lines, {(c name, mode): (C, e, f, widths of A, err, violations)}) for the scale-invariance variant."""
     A0, B0 = W.config_matrices(1)
     N = 16
     lines = ["", f"# Scale-invariance variant (A, B both times c), N = {N}: effective bit width of the rows of A (min/median/max),",
@@ -103,8 +109,14 @@ def test_config1_scale_invariance_variant(B):
             err = max_rel_err(Cg, hi, lo)
             lines.append(f"| {cname} | {MODES[mode]} | {wa[0]}/{wa[1]:.0f}/{wa[2]} | {wb[0]}/{wb[1]:.0f}/{wb[2]} | {viol} | {wrong} | {err:.3e} |")
             ref[(cname, mode)] = (Cg, e, f, wa, err, viol)
-            if mode != 1:
-                assert viol == 0, (cname, mode)
+    return lines, ref
+
+
+def test_config1_scale_invariance_variant(B):
+    _, ref = scale_invariance_table(B)
+    for (cname, mode), v in ref.items():
+        if mode != 1:
+            assert v[5] == 0, (cname, mode)
     # power-of-two scalings: revised mode is bit-invariant (exponents shift by -s, C scales by c^2 exactly)
     C1, e1, f1, w1, err1, _ = ref[("1", 2)]
     for cname, s in (("2^-500", -500), ("2^500", 500)):
@@ -117,5 +129,12 @@ def test_config1_scale_invariance_variant(B):
         assert abs(ref[(cname, 2)][3][1] - w1[1]) <= 1
     assert ref[("2^500", 1)][3][1] < w1[1] - 8                    # fast mode: width collapses for large inputs
     assert ref[("2^-500", 1)][5] > 0                               # and violates condition (1) for small ones
-    with open(os.path.join(ROOT, "gpurun_out", "accuracy_report.md"), "a") as fh:
-        fh.write("\n".join(lines) + "\n")
+
+
+if __name__ == "__main__":
+    import sys
+    sys.path.insert(0, ROOT)
+    import paper_2606_29129_b200 as pkg
+    pkg.lib()
+    print("\n".join(config1_error_table(pkg)[0]))
+    print("\n".join(scale_invariance_table(pkg)[0]))
