@@ -110,6 +110,21 @@ int ozaki2_sgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, 
                       int64_t lda, const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli,
                       int scaling_mode, void *stream);
 
+/*
+ * Complex variant (named as future work at P:58, P:444 without formulas -- reading in DESIGN.md 8b #4):
+ * C := alpha A B + beta C for interleaved complex FP64 matrices (re, im pairs; column-major; lda, ldb, ldc in complex
+ * elements; 16-byte aligned device pointers), computed as ozaki2_dgemm on the real embedding
+ * [C_r; C_i] = [[A_r, -A_i], [A_i, A_r]] [B_r; B_i]  (a (2m x 2k)(2k x n) product: one scaling exponent per complex row
+ * of A / column of B, condition (1) holds for both parts), then out = alpha c + beta C in plain complex arithmetic with
+ * every product and sum rounded on its own (alpha == 1 and beta == 0 are not multiplied; beta == 0 overwrites).  The
+ * embedded operands are materialised in the workspace: register ozaki2_zgemm_workspace_bytes(...) bytes with
+ * ozaki2_set_workspace.  2k <= OZAKI2_MAX_K (OZAKI2_MAX_K_ACCURATE in accurate mode).  Errors: -i for argument i.
+ */
+int ozaki2_zgemm(int64_t m, int64_t n, int64_t k, double alpha_re, double alpha_im, const double *A, int64_t lda,
+                 const double *B, int64_t ldb, double beta_re, double beta_im, double *C, int64_t ldc,
+                 int num_moduli, int scaling_mode, void *stream);
+size_t ozaki2_zgemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
+
 /* Bytes of device workspace ozaki2_dgemm / ozaki2_sgemm needs for this problem (0 for an invalid one). */
 size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 

@@ -275,6 +275,42 @@ def sgemm(A, B, N: int, mode: int, alpha: float = 1.0, beta: float = 0.0, C_in=N
     return out
 
 
+def zgemm_embedding(A, B):
+    """Real embedding of a complex product (DESIGN.md 8b #4): [C_r; C_i] = [[A_r, -A_i], [A_i, A_r]] [B_r; B_i]."""
+    A = np.asarray(A, dtype=np.complex128)
+    B = np.asarray(B, dtype=np.complex128)
+    At = np.block([[A.real, -A.imag], [A.imag, A.real]])
+    Bt = np.vstack([B.real, B.imag])
+    return np.asfortranarray(At), np.asfortranarray(Bt)
+
+
+def zgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_in=None):
+    """Complex variant (named as future work at P:58; reading in DESIGN.md 8b #4): oz2o_dgemm on the real embedding,
+    then out = alpha c + beta C_in in plain complex arithmetic -- every product and every sum rounded on its own, in the
+    order written below; alpha == 1 and beta == 0 are not multiplied (BLAS rule: beta == 0 overwrites)."""
+    A = np.asarray(A, dtype=np.complex128)
+    B = np.asarray(B, dtype=np.complex128)
+    m = A.shape[0]
+    At, Bt = zgemm_embedding(A, B)
+    Ct = dgemm(At, Bt, N, mode)
+    cr, ci = Ct[:m], Ct[m:]
+    alpha, beta = complex(alpha), complex(beta)
+    if alpha != 1.0:
+        with np.errstate(all="ignore"):
+            tr = alpha.real * cr - alpha.imag * ci
+            ti = alpha.real * ci + alpha.imag * cr
+    else:
+        tr, ti = cr, ci
+    if beta != 0.0:
+        Cin = np.asarray(C_in, dtype=np.complex128)
+        with np.errstate(all="ignore"):
+            tr = tr + (beta.real * Cin.real - beta.imag * Cin.imag)
+            ti = ti + (beta.real * Cin.imag + beta.imag * Cin.real)
+    out = np.empty(cr.shape, np.complex128, order="F")
+    out.real, out.imag = tr, ti
+    return out
+
+
 def dd_reference(A, B):
     """AB in double-double: (hi, lo), each (m, n) column-major."""
     A, B = _f(A), _f(B)

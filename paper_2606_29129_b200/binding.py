@@ -65,6 +65,10 @@ def lib() -> C.CDLL:
         L.ozaki2_dgemm_blas.restype = ci
         L.ozaki2_sgemm_blas.argtypes = [ci, ci, ci] + sgemm_args
         L.ozaki2_sgemm_blas.restype = ci
+        L.ozaki2_zgemm.argtypes = [i64, i64, i64, dbl, dbl, vp, i64, vp, i64, dbl, dbl, vp, i64, ci, ci, vp]
+        L.ozaki2_zgemm.restype = ci
+        L.ozaki2_zgemm_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
+        L.ozaki2_zgemm_workspace_bytes.restype = C.c_size_t
         L.ozaki2_debug_crt.argtypes = [ci, i64, i64, vp, vp, vp, dbl, dbl, vp, i64, vp, ci, vp]
         L.ozaki2_debug_crt.restype = ci
         L.ozaki2_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
@@ -196,6 +200,33 @@ def ozaki2_sgemm_blas(layout, transa, transb, m, n, k, alpha, A, lda, B, ldb, be
                       stream=None) -> int:
     return int(lib().ozaki2_sgemm_blas(_flag(layout), _flag(transa), _flag(transb), m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb,
                                        beta, _ptr(Cm), ldc, num_moduli, scaling_mode, _stream(stream)))
+
+
+def ozaki2_zgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode) -> int:
+    return int(lib().ozaki2_zgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode))
+
+
+def ozaki2_zgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None) -> int:
+    """Complex variant: A, B, Cm are complex128 device tensors (column-major) or addresses; alpha, beta complex."""
+    alpha, beta = complex(alpha), complex(beta)
+    return int(lib().ozaki2_zgemm(m, n, k, alpha.real, alpha.imag, _ptr(A), lda, _ptr(B), ldb, beta.real, beta.imag, _ptr(Cm), ldc,
+                                  num_moduli, scaling_mode, _stream(stream)))
+
+
+def ensure_zgemm_workspace(m, n, k, num_moduli, scaling_mode):
+    """Allocate (grow-only) and register a workspace large enough for ozaki2_zgemm on the current device."""
+    import torch
+    need = ozaki2_zgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode)
+    dev = torch.cuda.current_device()
+    cur = _ws_tensor.get(dev)
+    if cur is None or cur.numel() < need:
+        _ws_tensor[dev] = None
+        cur = torch.empty(max(need, 256), dtype=torch.uint8, device=f"cuda:{dev}")
+        _ws_tensor[dev] = cur
+    rc = ozaki2_set_workspace(cur, cur.numel())
+    if rc:
+        raise Ozaki2Error(rc, "ozaki2_set_workspace")
+    return cur
 
 
 def ozaki2_debug_crt(num_moduli, m, n, U, e, f, alpha, beta, Cm, ldc, Cpp=None, is_f32=False, stream=None) -> int:

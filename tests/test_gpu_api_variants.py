@@ -166,3 +166,59 @@ def test_sgemm_host_buffer_entry_point(B, n, mode):
     assert np.array_equal(Ch[m:], Cin[m:])
     assert B.ozaki2_sgemm_host(m, n, k, 0.5, Ah, lda, Bh, ldb, 1.5, Ch, ldc, N, mode, scratch, 16) == -14
     assert "14" in B.ozaki2_status_string(-14)
+
+
+def _complex_inputs(m, n, k, phi, seed):
+    Ar, Br = W.eq15_matrices(m, n, k, phi, seed)
+    Ai, Bi = W.eq15_matrices(m, n, k, phi, seed + 1)
+    return np.asfortranarray(Ar + 1j * Ai), np.asfortranarray(Br + 1j * Bi)
+
+
+@pytest.mark.parametrize("m,n,k,N,mode,alpha,beta", [
+    (70, 50, 90, 14, 2, 1.0, 0.0), (129, 33, 257, 17, 2, 0.5 - 2.0j, -1.25 + 0.75j), (64, 64, 64, 10, 1, 1.0, 1.0),
+    (40, 130, 300, 16, 0, -1.0j, 0.0), (1, 1, 1, 2, 2, 1.0, 0.0), (200, 20, 1000, 20, 2, 2.0, 0.5j),
+])
+def test_zgemm_against_the_oracle_on_the_real_embedding(B, m, n, k, N, mode, alpha, beta):
+    # SURVEY 8(f) #4 (reading DESIGN.md 8b #4): bit-exact against oz2o_dgemm on the embedding + the stated tail
+    import torch
+    A, Bm = _complex_inputs(m, n, k, 1.0, 700 + m + n + k)
+    lda, ldb, ldc = m + 3, k + 1, m + 2
+    Ap = np.zeros((lda, k), np.complex128, order="F"); Ap[:m] = A
+    Bp = np.zeros((ldb, n), np.complex128, order="F"); Bp[:k] = Bm
+    rng = np.random.Generator(np.random.PCG64(9))
+    Cin = np.asfortranarray(rng.standard_normal((ldc, n)) + 1j * rng.standard_normal((ldc, n)))
+    Ad = torch.from_numpy(np.ascontiguousarray(Ap.T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray(Bp.T)).cuda()
+    Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+    B.ensure_zgemm_workspace(m, n, k, N, mode)
+    assert B.ozaki2_zgemm(m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == 0
+    torch.cuda.synchronize()
+    got = np.asfortranarray(Cd.cpu().numpy().T)
+    want = O.zgemm(A, Bm, N, mode, alpha=alpha, beta=beta, C_in=Cin[:m])
+    assert np.array_equal(got[:m], want)
+    assert np.array_equal(got[m:], Cin[m:])
+    if mode != 1:
+        ref = A @ Bm
+        assert np.max(np.abs(O.zgemm(A, Bm, N, mode) - ref) / np.abs(ref)) < {10: 1e-2, 14: 1e-6, 16: 1e-8, 17: 1e-9, 20: 1e-13}.get(N, 1.0)
+
+
+def test_zgemm_quick_returns_and_errors(B):
+    import torch
+    m, n, k, N = 32, 16, 24, 12
+    A, Bm = _complex_inputs(m, n, k, 0.5, 3)
+    Ad = torch.from_numpy(np.ascontiguousarray(A.T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray(Bm.T)).cuda()
+    Cin = np.asfortranarray(np.arange(m * n).reshape(m, n) * (1.0 + 0.5j))
+    Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+    B.ensure_zgemm_workspace(m, n, k, N, 2)
+    assert B.ozaki2_zgemm(m, n, k, 0.0, Ad, m, Bd, k, 2.0j, Cd, m, N, 2) == 0        # alpha == 0: C := beta C
+    torch.cuda.synchronize()
+    assert np.array_equal(np.asfortranarray(Cd.cpu().numpy().T), 2.0j * Cin)
+    assert B.ozaki2_zgemm(m, n, 0, 1.0, Ad, m, Bd, 1, 0.0, Cd, m, N, 2) == 0          # k == 0, beta == 0: zeros
+    torch.cuda.synchronize()
+    assert not np.any(Cd.cpu().numpy())
+    assert B.ozaki2_zgemm(-1, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == -1
+    assert B.ozaki2_zgemm(m, n, k, 1.0, Ad, m - 1, Bd, k, 0.0, Cd, m, N, 2) == -7
+    assert B.ozaki2_zgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, 21, 2) == -14
+    assert B.ozaki2_set_workspace(None, 0) == 0
+    assert B.ozaki2_zgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == B.OZAKI2_ERR_WORKSPACE

@@ -1,0 +1,78 @@
+"""Pins for the oracle's complex variant (the paper names ZGEMM as future work without formulas, P:58, P:444;
+reading in DESIGN.md 8b #4: the product of the real embeddings).  What fixes it: the textbook identity between a complex
+product and its real embedding, exact integer cases, the real special case, and the paper's invariants carried over."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import ozaki2_oracle as O
+
+ACCU, FAST, PROP = 0, 1, 2
+
+
+def complex_inputs(m, n, k, phi, seed):
+    Ar, Br = W.eq15_matrices(m, n, k, phi, seed)
+    Ai, Bi = W.eq15_matrices(m, n, k, phi, seed + 1)
+    return Ar + 1j * Ai, Br + 1j * Bi
+
+
+def test_embedding_is_the_complex_product_exactly_on_gaussian_integers():
+    rng = np.random.Generator(np.random.PCG64(3))
+    A = rng.integers(-9, 10, (7, 11)) + 1j * rng.integers(-9, 10, (7, 11))
+    B = rng.integers(-9, 10, (11, 5)) + 1j * rng.integers(-9, 10, (11, 5))
+    At, Bt = O.zgemm_embedding(A, B)
+    Ct = At @ Bt
+    want = A @ B                                           # small integers: exact in FP64
+    assert np.array_equal(Ct[:7], want.real) and np.array_equal(Ct[7:], want.imag)
+    # rows i and m + i of the embedded A carry the complex row's 2-norm and max-norm: one exponent per complex row
+    assert np.array_equal(np.sum(At[:7] ** 2, axis=1), np.sum(At[7:] ** 2, axis=1))
+    assert np.array_equal(np.sum(At[:7] ** 2, axis=1), np.sum(np.abs(A) ** 2, axis=1))
+
+
+@pytest.mark.parametrize("mode", [ACCU, FAST, PROP])
+def test_gaussian_integer_matrices_exact(mode):
+    rng = np.random.Generator(np.random.PCG64(5))
+    A = rng.integers(-8, 9, (12, 30)) + 1j * rng.integers(-8, 9, (12, 30))
+    B = rng.integers(-8, 9, (30, 9)) + 1j * rng.integers(-8, 9, (30, 9))
+    assert np.array_equal(O.zgemm(A, B, 10, mode), A @ B)
+
+
+@pytest.mark.parametrize("mode", [FAST, PROP])
+def test_real_inputs_reduce_to_dgemm_bit_for_bit(mode):
+    # imaginary parts zero: the embedded rows (a, 0) and (0, a) have the statistics of the real row (zeros add nothing to
+    # the max or to the rounded-up sum of squares), so the real part is oz2o_dgemm's result and the imaginary part is 0
+    A, B = W.eq15_matrices(20, 14, 60, 1.0, 8)
+    C = O.zgemm(A.astype(np.complex128), B.astype(np.complex128), 14, mode)
+    assert np.array_equal(C.real, O.dgemm(A, B, 14, mode)) and not np.any(C.imag)
+
+
+def test_both_rows_of_a_complex_row_get_the_same_exponent_and_condition_1_holds():
+    A, B = complex_inputs(16, 12, 64, 1.0, 20)
+    At, Bt = O.zgemm_embedding(A, B)
+    for mode in (ACCU, PROP):
+        e, f = O.exponents(mode, 15, At, Bt)
+        if mode == PROP:
+            assert np.array_equal(e[:16], e[16:])           # one scaling per complex row (P:303-311 on complex moduli)
+        Ap, Bp = O.truncate(0, At, e), O.truncate(1, Bt, f)
+        _, _, cnt = O.exact_product(15, Ap, Bp, want_words=False)
+        assert cnt["violations"] == 0                       # P:358 / P:161-163 carried over to the embedding
+
+
+def test_error_against_numpy_complex_product_and_alpha_beta():
+    A, B = complex_inputs(24, 18, 128, 0.5, 30)
+    ref = A @ B
+    C = O.zgemm(A, B, 18, PROP)
+    assert np.max(np.abs(C - ref) / np.abs(ref)) < 1e-12
+    # power-of-two scale invariance of the revised mode, complex scalars of modulus 2^s included
+    C2 = O.zgemm(A * 2.0 ** 40, B * (2.0 ** -70 * 1j), 18, PROP)
+    assert np.array_equal(C2, C * (2.0 ** -30 * 1j))
+    alpha, beta = 0.5 - 2.0j, -1.25 + 0.75j
+    rng = np.random.Generator(np.random.PCG64(2))
+    Cin = rng.standard_normal((24, 18)) + 1j * rng.standard_normal((24, 18))
+    out = O.zgemm(A, B, 18, PROP, alpha=alpha, beta=beta, C_in=Cin)
+    want = alpha * C + beta * Cin
+    assert np.max(np.abs(out - want)) <= 4 * np.finfo(float).eps * np.max(np.abs(want))
+    # the stated operation order, element by element
+    tr = alpha.real * C.real - alpha.imag * C.imag + (beta.real * Cin.real - beta.imag * Cin.imag)
+    ti = alpha.real * C.imag + alpha.imag * C.real + (beta.real * Cin.imag + beta.imag * Cin.real)
+    assert np.array_equal(out.real, tr) and np.array_equal(out.imag, ti)
