@@ -68,6 +68,7 @@ def parse_args():
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: leave out the oracle leg")
     ap.add_argument("--skip-ceiling", action="store_true", help="profiling runs only: leave out the MMA-only ceiling runs")
+    ap.add_argument("--ceiling-reps", type=int, default=20, help="launches per MMA-only ceiling run (200: sustained, under the power cap)")
     ap.add_argument("--accuracy", action="store_true", help="add max relative error vs the double-double reference "
                     "(P:268) on a sampled slab, and max |R_l| on it (INT32 headroom, P:113)")
     a = ap.parse_args()
@@ -224,16 +225,17 @@ def run_reference(args):
     return 0
 
 
-def measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=10):
-    """The path's GEMM kernel with the epilogue reduced to handing the accumulator back (ozaki2_debug_residue_gemm,
-    variant 3), on uniform random symmetric residues and on all-zero planes: what this MMA / TMA loop can deliver on
-    this board at the clocks it gets, next to which the mod-p epilogue and the real data are judged."""
+def measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=20):
+    """The GEMM kernels with the epilogue reduced to handing the accumulator back (ozaki2_debug_residue_gemm, variants
+    4 = CTA pairs, the path's form, and 3 = one CTA per tile), on uniform random symmetric residues and on all-zero
+    planes: what this MMA / TMA loop can deliver on this board at the clocks it gets, next to which the mod-p epilogue
+    and the real data are judged.  Board power and SM clock are sampled during each run (nvidia-smi, 10 ms)."""
     if k % 128 or m % 16 or k > (1 << 17):
         return None
     out = {}
     RA = torch.empty((N, m, k), dtype=torch.int8, device="cuda")
     RB = torch.empty((N, n, k), dtype=torch.int8, device="cuda")
-    U = torch.empty((16,), dtype=torch.uint8, device="cuda")          # untouched by variant 3
+    U = torch.empty((16,), dtype=torch.uint8, device="cuda")          # untouched by variants 3, 4
     for name in ("random", "zero"):
         if name == "random":
             g = torch.Generator(device="cuda")
@@ -243,18 +245,31 @@ def measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=10):
                     t[l].copy_(torch.randint(-86, 87, t[l].shape, dtype=torch.int8, device="cuda", generator=g))
         else:
             RA.zero_(); RB.zero_()
-        for _ in range(3):
-            rc = pkg.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, U, 3, stream)
-            if rc:
-                raise pkg.Ozaki2Error(rc, "ozaki2_debug_residue_gemm(3)")
-        evs = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
-        evs[0].record(stream)
-        for r in range(reps):
-            pkg.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, U, 3, stream)
-            evs[r + 1].record(stream)
-        torch.cuda.synchronize()
-        ms = statistics.median(evs[r].elapsed_time(evs[r + 1]) for r in range(reps))
-        out[name] = dict(tops=N * 2.0 * m * n * k / (ms * 1e-3) / 1e12, ms=ms)
+        for form, variant in (("pair", 4), ("single", 3)):
+            for _ in range(3):
+                rc = pkg.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, U, variant, stream)
+                if rc:
+                    raise pkg.Ozaki2Error(rc, "ozaki2_debug_residue_gemm")
+            torch.cuda.synchronize()
+            sampler = ClockSampler(torch.cuda.current_device())
+            sampler.start()
+            sampler.wait_first_sample()
+            evs = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+            sampler.window[0] = time.time()
+            evs[0].record(stream)
+            for r in range(reps):
+                pkg.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, U, variant, stream)
+                evs[r + 1].record(stream)
+            torch.cuda.synchronize()
+            sampler.window[1] = time.time()
+            clk = sampler.stop()
+            ms = statistics.median(evs[r].elapsed_time(evs[r + 1]) for r in range(reps))
+            entry = dict(tops=N * 2.0 * m * n * k / (ms * 1e-3) / 1e12, ms=ms, reps=reps, sm_mhz=clk.get("sm_mhz"),
+                         power_w_max=clk.get("power_w_max"), reasons=clk.get("reasons"))
+            if form == "pair":
+                out[name] = entry                                     # the path's kernel: roofline.int8_ceiling_tops.{random, zero}
+            else:
+                out[name + "_single_cta"] = entry
     del RA, RB
     torch.cuda.empty_cache()
     return out
@@ -361,7 +376,7 @@ def main():
     achieved = N * flops / (s3_ms * 1e-3) / 1e12
     ceiling = None
     if not args.skip_ceiling and not f32:
-        ceiling = measure_int8_ceiling(pkg, torch, m, n, k, N, stream)
+        ceiling = measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=args.ceiling_reps)
     roofline = dict(bound="tensor", kernel="k3_residue_gemm<EPI_MODP> (tcgen05.mma kind::i8, batched over N moduli)",
                     achieved=achieved, peak=int8_peak, unit="TFLOP/s", frac=achieved / int8_peak,
                     peak_source=f"2 x bf16_tflops burst ({peaks['source']}): another dtype's measured peak x the nominal "
