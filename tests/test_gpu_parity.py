@@ -296,6 +296,20 @@ def test_residue_gemm_tensor_core_vs_oracle_and_check_kernel(B, m, n, k, N):
         assert np.array_equal(Ud.cpu().numpy(), want), f"tensor_cores={tc}"
 
 
+def test_mma_only_variants_leave_U_untouched(B):
+    # variants 3 / 4 of ozaki2_debug_residue_gemm (the INT8 ceiling runs of bench.py) hand the accumulator back unread
+    import torch
+    N, m, n, k = 2, 256, 512, 256
+    RA = torch.randint(-100, 100, (N, m, k), dtype=torch.int8, device="cuda")
+    RB = torch.randint(-100, 100, (N, n, k), dtype=torch.int8, device="cuda")
+    Ud = torch.full((N, n, m), 7, dtype=torch.uint8, device="cuda")
+    for variant in (3, 4):
+        assert B.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, Ud, variant) == 0
+        torch.cuda.synchronize()
+        assert bool((Ud == 7).all())
+    assert B.ozaki2_debug_residue_gemm(N, m, n, k, RA, RB, Ud, 5) == -8
+
+
 def test_k_blocked_residue_gemm_beyond_2pow17(B):
     # k > 2^17 is computed in blocks of 2^17 whose residues are added mod p_l in the epilogue; worst-case
     # operands (-128 x -128 for p = 256, 127 x 127 for 255) over 2 1/2 blocks

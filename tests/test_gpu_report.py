@@ -6,15 +6,19 @@ against the double-double reference is recorded.  The two table b
 the caller: the tests assert the paper's claims as trends on the numbers, and running this file as a script prints the
 tables on stdout (that is how profiles/r02_accuracy.md is made: `python tests/test_gpu_report.py > ...`)."""
 import os
+import sys
 
 import numpy as np
 import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:                      # script mode (pytest gets the path from conftest.py)
+    sys.path.insert(0, ROOT)
 
 import workloads as W
 from oracle import ozaki2_oracle as O
 
 pytestmark = pytest.mark.gpu
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 MODES = {0: "accu", 1: "fast", 2: "prop"}
 
 
@@ -132,8 +136,6 @@ def test_config1_scale_invariance_variant(B):
 
 
 if __name__ == "__main__":
-    import sys
-    sys.path.insert(0, ROOT)
     import paper_2606_29129_b200 as pkg
     pkg.lib()
     print("\n".join(config1_error_table(pkg)[0]))
