@@ -106,9 +106,11 @@ __device__ __forceinline__ unsigned long long digits_narrow(double a, int ex)
     return (unsigned long long)t ^ 0x8000000000000000ull;
 }
 
-// wide format: |a'| < 2^95 as three 32-bit words of a' + 2^95 (two's complement, top bit flipped)
-__device__ __forceinline__ void digits_wide(double a, int ex, uint32_t (&w)[3])
+// wide format: |a'| < 2^95 as three 32-bit words of a' + 2^95 (two's complement, top bit flipped).
+// Integer route (any input; used for zero / subnormal inputs): shifts of the 53-bit mantissa.
+__device__ __noinline__ uint3 digits_wide_int(double a, int ex)
 {
+    uint32_t w[3];
     const unsigned long long b = (unsigned long long)__double_as_longlong(a);
     const uint32_t hi = (uint32_t)(b >> 32), lo = (uint32_t)b;
     const uint32_t negm = (uint32_t)((int32_t)hi >> 31);
@@ -135,6 +137,36 @@ __device__ __forceinline__ void digits_wide(double a, int ex, uint32_t (&w)[3])
     asm("add.cc.u32 %0, %0, %3;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.u32 %2, %2, 0;"
         : "+r"(w[0]), "+r"(w[1]), "+r"(w[2]) : "r"(negm & 1u));
     w[2] ^= 0x80000000u;
+    return make_uint3(w[0], w[1], w[2]);                          // by value: the caller's words stay in registers
+}
+
+// FP64 route (normal inputs): a' = th 2^32 + tl with th = trunc(a 2^(ex-32)) and tl = a 2^ex - th 2^32, both exact:
+// th < 2^52 (|a'| < 2^84), and the remainder is a multiple of ulp(a 2^ex) below 2^32, so the FMA forms it without
+// rounding.  th and tl carry the sign of a; their 96-bit two's-complement sum is assembled with one 64-bit add.
+__device__ __forceinline__ void digits_wide(double a, int ex, uint32_t (&w)[3])
+{
+    const long long bits = __double_as_longlong(a);
+    const int hi = (int)(bits >> 32);
+    const int be = (hi >> 20) & 0x7FF;
+    if (be == 0) {
+        uint3 r = make_uint3(0u, 0u, 0x80000000u);
+        if ((bits << 1) != 0) r = digits_wide_int(a, ex);
+        w[0] = r.x; w[1] = r.y; w[2] = r.z;
+        return;
+    }
+    const int ne = be + ex;                                       // biased exponent of a 2^ex
+    const double x = __hiloint2double(hi + ex * 1048576, (int)bits);
+    const double xh = __hiloint2double(hi + (ex - 32) * 1048576, (int)bits);
+    const double hd = trunc(xh);                                  // |a 2^ex| >= 1 keeps a 2^(ex-32) a normal number
+    const double rem = fma(hd, -4294967296.0, x);                 // exact
+    long long th = __double2ll_rz(hd), tl = __double2ll_rz(rem);
+    if (ne < 1023) { th = 0; tl = 0; }                            // |a 2^ex| < 1 truncates to 0
+    const unsigned long long top = (unsigned long long)th << 32;
+    const unsigned long long lo64 = top + (unsigned long long)tl;
+    const int carry = lo64 < top ? 1 : 0;
+    w[0] = (uint32_t)lo64;
+    w[1] = (uint32_t)(lo64 >> 32);
+    w[2] = ((uint32_t)((int)(th >> 32) + (int)(tl >> 63) + carry)) ^ 0x80000000u;
 }
 
 // ---------------------------------------------------------------------------------------------
