@@ -449,7 +449,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
             }
         }
     } else {
-        // ===================== epilogue: warps 2..9 of both CTAs, rows m0 + 128 rank + 32 q + lane =====================
+        // ===================== epilogue: warps 2..17 of both CTAs, rows m0 + 128 rank + 32 q + lane =====================
         const int q = warp & 3;                                // TMEM lane quarter
         const int half = (warp - 2) >> 2;                      // column slice of the tile
         int as = 0;

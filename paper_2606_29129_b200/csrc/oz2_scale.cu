@@ -299,8 +299,14 @@ int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const 
     const double *A = static_cast<const double *>(Av);
     const float *Af = static_cast<const float *>(Av);
     if (m <= 0) return 0;
-    OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
-    OZ2_CUDA_TRY(cudaMemsetAsync(ssqA, 0, sizeof(unsigned long long) * (size_t)m, st));
+    // the two statistics arrays are neighbours in the workspace: one memset node instead of two when they are
+    const char *lo = reinterpret_cast<const char *>(amaxA), *hi = reinterpret_cast<const char *>(ssqA + m);
+    if (ssqA > amaxA && (size_t)(hi - lo) <= 16 * (size_t)m + 1024) {
+        OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, (size_t)(hi - lo), st));
+    } else {
+        OZ2_CUDA_TRY(cudaMemsetAsync(amaxA, 0, sizeof(unsigned long long) * (size_t)m, st));
+        OZ2_CUDA_TRY(cudaMemsetAsync(ssqA, 0, sizeof(unsigned long long) * (size_t)m, st));
+    }
     int64_t kchunk;
     int gy = rows_grid_y(m, k, &kchunk);
     dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
