@@ -198,77 +198,139 @@ __device__ __forceinline__ void mp_inc(uint32_t (&x)[W], uint32_t one)
             : "+r"(x[0]), "+r"(x[1]), "+r"(x[2]), "+r"(x[3]), "+r"(x[4]) : "r"(one));
 }
 
-// per-thread copy of the per-N constants the common case needs (kept in registers across the tile loop)
-template <int NW>
-struct CrtRegs {
-    uint32_t P[NW];
-    double invP;
+// per-N constants of the common case (constant bank; the compiler keeps them in uniform registers)
+struct K5Consts {
+    uint32_t Pn[OZ2_MAX_WORDS];     // 2^(32 NW) - P: C' + Q Pn = C' - Q P  (mod 2^(32 NW))
+    uint32_t nterms;                // (unused padding)
+    double K0, K1;                  // 2^(32 (NW-1)) / P and 2^(32 (NW-2)) / P: weights of the two top 32-bit columns
 };
+__constant__ K5Consts c_k5[OZ2_MAX_MODULI + 1];
 
-// The common case of crt_exact without a branch: the quotient estimate is away from a half-integer and the result
-// is a normal number.  `rare` is set when that does not hold (the caller then takes crt_exact).
+// The common case without a branch, straight from the byte slices S[0 .. 4 NW) of one element:
+//   Z_k  = sum_b S[4k+b] 256^b (< 2^46): the 32-bit columns of C' before carries, C' = sum_k Z_k 2^(32 k)
+//   Q    = round(C' / P) from the two top columns in FP64 (dropped columns < 2^-22.9, arithmetic < 2^-38: any Q within
+//          2^-20 of a half-integer is handed to the exact routine)
+//   R    = C' + Q (2^(32 NW) - P) mod 2^(32 NW) = C'' in two's complement: W_k = Z_k + Q Pn_k (< 2^47) per column, then
+//          ONE carry chain over the NW columns -- fold and subtraction together cost 5 instructions per word
+//   |R|  -> the 64 bits from the leading one (top three words after at most NW - 3 whole-word shifts; a value below
+//          2^64 passes exactly through the clamped funnel shifts) + sticky bit -> one rounding (I2F) -> exponent field
+// `rare` is set when the result needs crt_exact (near-half quotient, subnormal or overflowing result).
 template <int NW, typename TO>
-__device__ __forceinline__ TO crt_fast(const uint32_t (&c)[NW + 1], const CrtRegs<NW> &T, int esum, bool &rare)
+__device__ __forceinline__ TO crt_fast(const uint32_t *S, const K5Consts &T, int esum, bool &rare)
 {
-    // ---- Q = round(C' / P) from the top words (error of the estimate < 2^-30)
-    double top = (double)(long long)(((unsigned long long)c[NW] << 32) | c[NW - 1]);
-    if constexpr (NW >= 2) top = fma((double)c[NW - 2], 2.3283064365386963e-10, top);
-    const double qd = top * T.invP;
-    const double qr = rint(qd);
-    const uint32_t Q = (uint32_t)__double2int_rn(qd);
-    rare = fabs(qd - qr) > 0.5 - 9.5367431640625e-07;                 // within 2^-20 of a half-integer: exact compare needed
-    // ---- R = C' - Q P in two's complement: C' - lo(Q P_t) 2^(32 t) - hi(Q P_t) 2^(32 (t + 1))
-    uint32_t lo[NW + 1], hi[NW + 1], r[NW + 1];
-    hi[0] = 0u;
+    unsigned long long Z[NW];
 #pragma unroll
-    for (int t = 0; t < NW; t++) {
-        const unsigned long long pr = (unsigned long long)Q * T.P[t];
-        lo[t] = (uint32_t)pr;
-        hi[t + 1] = (uint32_t)(pr >> 32);
+    for (int k = 0; k < NW; k++) {
+        const uint32_t a = S[4 * k] + (S[4 * k + 1] << 8), b = S[4 * k + 2] + (S[4 * k + 3] << 8);   // < 2^30
+        Z[k] = (unsigned long long)b * 65536ull + (unsigned long long)a;
     }
-    lo[NW] = 0u;
-    mp_sub<NW + 1>(r, c, lo);
-    mp_sub<NW + 1>(r, r, hi);
-    // ---- |R| (NW words: |C''| <= P/2 < 2^(32 NW - 1)), branch-free negate
-    const uint32_t negm = (uint32_t)((int32_t)r[NW] >> 31);
+    // ---- Q (Z < 2^46: the conversions are exact)
+    double qd = (double)(long long)Z[NW - 1] * T.K0;
+    if constexpr (NW >= 2) qd = fma((double)(long long)Z[NW - 2], T.K1, qd);
+    const double MAGIC = 6755399441055744.0;                          // 1.5 2^52: RN to an integer in the low word
+    const double tq = qd + MAGIC;
+    const uint32_t Q = (uint32_t)__double2loint(tq);
+    rare = fabs(qd - (tq - MAGIC)) > 0.5 - 9.5367431640625e-07;       // within 2^-20 of a half-integer: exact compare needed
+    // ---- R = C' - Q P (mod 2^(32 NW))
+    uint32_t r[NW];
+    {
+        unsigned long long W[NW];
+#pragma unroll
+        for (int k = 0; k < NW; k++) W[k] = (unsigned long long)Q * T.Pn[k] + Z[k];
+        uint32_t lo[NW], hi[NW];
+#pragma unroll
+        for (int k = 0; k < NW; k++) { lo[k] = (uint32_t)W[k]; hi[k] = (uint32_t)(W[k] >> 32); }
+        r[0] = lo[0];
+        if constexpr (NW == 2) r[1] = lo[1] + hi[0];
+        if constexpr (NW == 3)
+            asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, %5;" : "=r"(r[1]), "=r"(r[2]) : "r"(lo[1]), "r"(hi[0]), "r"(lo[2]), "r"(hi[1]));
+        if constexpr (NW == 4)
+            asm("add.cc.u32 %0, %3, %4;\n\taddc.cc.u32 %1, %5, %6;\n\taddc.u32 %2, %7, %8;"
+                : "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(lo[1]), "r"(hi[0]), "r"(lo[2]), "r"(hi[1]), "r"(lo[3]), "r"(hi[2]));
+        if constexpr (NW == 5)
+            asm("add.cc.u32 %0, %4, %5;\n\taddc.cc.u32 %1, %6, %7;\n\taddc.cc.u32 %2, %8, %9;\n\taddc.u32 %3, %10, %11;"
+                : "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4])
+                : "r"(lo[1]), "r"(hi[0]), "r"(lo[2]), "r"(hi[1]), "r"(lo[3]), "r"(hi[2]), "r"(lo[4]), "r"(hi[3]));
+    }
+    // ---- |R| (|C''| <= P/2 < 2^(32 NW - 1)), branch-free negate
+    const uint32_t negm = (uint32_t)((int32_t)r[NW - 1] >> 31);
     uint32_t x[NW];
 #pragma unroll
     for (int t = 0; t < NW; t++) x[t] = r[t] ^ negm;
     mp_inc<NW>(x, negm & 1u);
-    // ---- top 64 bits from the leading one, sticky bit
-    auto X = [&](int t) -> uint32_t { return t < NW ? x[t < NW ? t : 0] : 0u; };
-    const unsigned long long X0 = ((unsigned long long)X(1) << 32) | X(0);
-    const unsigned long long X1 = ((unsigned long long)X(3) << 32) | X(2);
-    const unsigned long long X2 = (unsigned long long)X(4);
-    const bool use2 = NW >= 5 && X2 != 0ull, use1 = !use2 && NW >= 3 && X1 != 0ull;
-    const unsigned long long ptop = use2 ? X2 : (use1 ? X1 : X0), pmid = use2 ? X1 : (use1 ? X0 : 0ull), plow = use2 ? X0 : 0ull;
-    const int base = use2 ? 128 : (use1 ? 64 : 0);
-    const bool zero = ptop == 0ull;
-    const int lz = __clzll((long long)(ptop | (unsigned long long)zero));
-    const unsigned long long mant = (ptop << lz) | ((pmid >> 1) >> (63 - lz));
-    const uint32_t sticky = (((pmid << lz) | plow) != 0ull) ? 1u : 0u;
-    const int pos = base + 63 - lz, sc = pos - 63 - esum, Ex = pos - esum;
+    // ---- 64-bit mantissa from the leading one + sticky bit; value = mant 2^sc
+    unsigned long long mant;
+    int sc = -esum;
+    if constexpr (NW == 1) mant = x[0];
+    else if constexpr (NW == 2) mant = ((unsigned long long)x[1] << 32) | x[0];
+    else {
+        sc += 32 * (NW - 2);
+#pragma unroll
+        for (int s = 0; s < NW - 3; s++) {                            // whole-word shifts while the top word is empty
+            const bool z = x[NW - 1] == 0u;
+#pragma unroll
+            for (int t = NW - 1; t >= 1; t--) x[t] = z ? x[t - 1] : x[t];
+            x[0] = z ? 0u : x[0];
+            sc -= z ? 32 : 0;
+        }
+        const int lz = __clz((int)x[NW - 1]);                         // 32 for an empty top word: the shifts below clamp
+        const uint32_t mh = __funnelshift_lc(x[NW - 2], x[NW - 1], lz), ml = __funnelshift_lc(x[NW - 3], x[NW - 2], lz);
+        uint32_t rest = __funnelshift_lc(0u, x[NW - 3], lz);
+#pragma unroll
+        for (int t = 0; t < NW - 3; t++) rest |= x[t];
+        mant = ((unsigned long long)mh << 32) | (ml | (rest != 0u ? 1u : 0u));
+        sc -= lz;
+    }
     if constexpr (sizeof(TO) == 8) {
-        rare |= !zero && (Ex < -1020 || Ex > 1021);
-        const double d = __ull2double_rn(mant | sticky);              // the one rounding, ties to even
-        const int hw = (__double2hiint(d) + (sc << 20)) | (int)(negm & 0x80000000u);
-        return zero ? 0.0 : __hiloint2double(hw, __double2loint(d));
+        const double d = NW == 1 ? (double)(uint32_t)mant : __ull2double_rn(mant);   // the one rounding, ties to even
+        const int hd = __double2hiint(d);
+        const bool zero = hd == 0;
+        const int be = (hd >> 20) + sc;                               // biased exponent of the result
+        rare |= !zero && (uint32_t)(be - 2) > 2043u;                  // subnormal or overflowing result: exact routine
+        const int hw = (hd + (sc << 20)) | (int)(negm & 0x80000000u);
+        return __hiloint2double(zero ? 0 : hw, __double2loint(d));
     } else {
-        rare |= !zero && (Ex < -124 || Ex > 125);
-        const float d = __ull2float_rn(mant | sticky);
-        const int bits = (__float_as_int(d) + sc * 8388608) | (int)(negm & 0x80000000u);
+        const float d = NW == 1 ? __uint2float_rn((uint32_t)mant) : __ull2float_rn(mant);
+        const int hd = __float_as_int(d);
+        const bool zero = hd == 0;
+        const int be = (hd >> 23) + sc;
+        rare |= !zero && (uint32_t)(be - 2) > 251u;
+        const int bits = (hd + (sc << 23)) | (int)(negm & 0x80000000u);
         return __int_as_float(zero ? 0 : bits);
     }
 }
 
-// by-value gate to crt_exact: the words travel in a struct so that the hot path keeps them in registers (an array
-// passed by reference to a non-inlined function would live in local memory for the whole loop)
+// by-value gate to crt_exact for the parity surface (every element, C'' words wanted): the words travel in a struct
+// so that the caller keeps them in registers
 template <int NW>
 struct CWords { uint32_t w[NW + 1]; };
 template <int NW, typename TO>
 __device__ __noinline__ TO crt_exact_v(CWords<NW> cw, int N, int esum, uint64_t *cpp_out)
 {
     return crt_exact<NW, TO>(cw.w, c_crt[N], esum, cpp_out);
+}
+
+// The rare path of the production kernel, decoupled from the registers of the common case: C' = sum_l w_l U_l is
+// recomputed in plain integer arithmetic from the element's N residue bytes in global memory (planes `plane` bytes
+// apart), then crt_exact.
+template <int NW, typename TO>
+__device__ __noinline__ TO crt_exact_global(const uint8_t *__restrict__ Uel, size_t plane, int N, int esum)
+{
+    uint32_t c[NW + 1];
+#pragma unroll
+    for (int t = 0; t <= NW; t++) c[t] = 0u;
+    for (int l = 0; l < N; l++) {
+        const uint32_t u = Uel[(size_t)l * plane];
+        unsigned long long carry = 0;
+#pragma unroll
+        for (int t = 0; t < NW; t++) {
+            const unsigned long long v = (unsigned long long)u * c_crt[N].w[l][t] + c[t] + carry;
+            c[t] = (uint32_t)v;
+            carry = v >> 32;
+        }
+        c[NW] += (uint32_t)carry;
+    }
+    return crt_exact<NW, TO>(c, c_crt[N], esum, nullptr);
 }
 
 // =============================================================================================
@@ -330,32 +392,26 @@ __device__ __forceinline__ void k5_store(TO cij, TO alpha, TO beta, TO *dst)
 }
 
 // the two elements (i, j) and (i + 128, j) of one thread: C'' -> C -> alpha / beta -> store.  Both go through the
-// branch-free crt_fast side by side (two independent dependency chains per thread); crt_exact is the rare path.
+// branch-free crt_fast side by side (two independent dependency chains per thread); the exact routine is the rare path.
 template <int NW, bool WANT_CPP, bool BETA0, typename TO>
-__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, const CrtRegs<NW> &T, int N, bool ok_a, bool ok_b,
+__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, int N, bool ok_a, bool ok_b,
                                            int esum_a, int esum_b, TO alpha, TO beta, TO *__restrict__ dst,
-                                           uint64_t *__restrict__ cpp)
+                                           uint64_t *__restrict__ cpp, const uint8_t *__restrict__ Uel, size_t plane)
 {
-    uint32_t ca[NW + 1], cb[NW + 1];
-    k5_fold<NW>(Sa, ca);
-    k5_fold<NW>(Sb, cb);
     TO va, vb;
     if constexpr (WANT_CPP) {
         CWords<NW> wa, wb;
-#pragma unroll
-        for (int t = 0; t <= NW; t++) { wa.w[t] = ca[t]; wb.w[t] = cb[t]; }
+        k5_fold<NW>(Sa, wa.w);
+        k5_fold<NW>(Sb, wb.w);
         va = ok_a ? crt_exact_v<NW, TO>(wa, N, esum_a, cpp) : (TO)0;
         vb = ok_b ? crt_exact_v<NW, TO>(wb, N, esum_b, cpp + 128 * 4) : (TO)0;
     } else {
         bool rare_a, rare_b;
-        va = crt_fast<NW, TO>(ca, T, esum_a, rare_a);
-        vb = crt_fast<NW, TO>(cb, T, esum_b, rare_b);
+        va = crt_fast<NW, TO>(Sa, c_k5[N], esum_a, rare_a);
+        vb = crt_fast<NW, TO>(Sb, c_k5[N], esum_b, rare_b);
         if ((rare_a && ok_a) || (rare_b && ok_b)) {                   // rare: near-half quotient, subnormal or overflowing result
-            CWords<NW> wa, wb;
-#pragma unroll
-            for (int t = 0; t <= NW; t++) { wa.w[t] = ca[t]; wb.w[t] = cb[t]; }
-            if (rare_a && ok_a) va = crt_exact_v<NW, TO>(wa, N, esum_a, nullptr);
-            if (rare_b && ok_b) vb = crt_exact_v<NW, TO>(wb, N, esum_b, nullptr);
+            if (rare_a && ok_a) va = crt_exact_global<NW, TO>(Uel, plane, N, esum_a);
+            if (rare_b && ok_b) vb = crt_exact_global<NW, TO>(Uel + 128, plane, N, esum_b);
         }
     }
     if (ok_a) k5_store<BETA0, TO>(va, alpha, beta, dst);
@@ -365,8 +421,8 @@ __device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *S
 template <int NW, bool WANT_CPP, bool BETA0, typename TO>
 __global__ void __launch_bounds__(K5_THREADS, NW <= 4 ? 3 : 2)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const int32_t *__restrict__ e,
-          const int32_t *__restrict__ f, TO alpha, TO beta, TO *__restrict__ C, int64_t ldc,
-          uint64_t *__restrict__ Cpp)
+          const int32_t *__restrict__ f, TO alpha, TO beta, TO *__restrict__ C, int ldc,
+          uint64_t *__restrict__ Cpp, const uint8_t *__restrict__ U, int mp)
 {
     constexpr int NS = NW <= 4 ? 16 : 32;                    // byte slices = MMA N
     constexpr int BUF_COLS = 2 * NS;                         // two 128-element MMAs per accumulator buffer
@@ -382,8 +438,8 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // tile t = j * tiles_i + ib (ib fastest), walked with stride gridDim.x; (j, ib) advance without a division
     const int tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
-    const int64_t total = (int64_t)tiles_i * n;
-    const int G = (int)gridDim.x;
+    const uint32_t total = (uint32_t)tiles_i * (uint32_t)n;          // < 2^31 - 2 gridDim.x (checked by the launcher)
+    const uint32_t G = gridDim.x;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < K5_STAGES; s++) {
@@ -413,10 +469,10 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
 
     if (warp == 0) {
         if (lane == 0) {
-            const int step_j = G / tiles_i, step_i = G - step_j * tiles_i;
+            const int step_j = (int)G / tiles_i, step_i = (int)G - step_j * tiles_i;
             int j = (int)blockIdx.x / tiles_i, ib = (int)blockIdx.x - j * tiles_i;
             int s = 0; uint32_t ph = 0;
-            for (int64_t t = blockIdx.x; t < total; t += G) {
+            for (uint32_t t = blockIdx.x; t < total; t += G) {
                 mbar_wait_idle(empty + 8 * s, ph ^ 1u);          // the epilogue paces this kernel: poll lazily
                 mbar_expect_tx_a(full + 8 * s, K5_STAGE_BYTES);
                 const uint32_t dst = smem0 + s * K5_STAGE_BYTES;
@@ -435,7 +491,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
                                    ((uint64_t)(256u >> 4) << 32) | (1ull << 46);
             // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
             const uint64_t adesc0 = ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
-            for (int64_t t = blockIdx.x; t < total; t += G) {
+            for (uint32_t t = blockIdx.x; t < total; t += G) {
                 mbar_wait_idle(tempty + 8 * b, bph ^ 1u);
                 mbar_wait_idle(full + 8 * s, ph);
                 tc_fence_after();
@@ -452,20 +508,16 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     } else {
         const int q = warp & 3;                              // TMEM lane quarter of this warp
         const int set = (warp - 2) >> 2;                     // epilogue set 0 / 1 takes every second tile of the CTA
-        CrtRegs<NW> T;
-#pragma unroll
-        for (int t = 0; t < NW; t++) T.P[t] = c_crt[N].P[t];
-        T.invP = c_crt[N].invP;
         int b = set; uint32_t bph = 0;
         // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
-        const int64_t t0 = (int64_t)blockIdx.x + (int64_t)set * G;
-        int j = (int)(t0 / tiles_i), ib = (int)(t0 - (int64_t)j * tiles_i);
-        const int step_j = (2 * G) / tiles_i, step_i = 2 * G - step_j * tiles_i;
+        const uint32_t t0 = blockIdx.x + (uint32_t)set * G, stride = 2u * G;
+        int j = (int)(t0 / (uint32_t)tiles_i), ib = (int)(t0 - (uint32_t)j * (uint32_t)tiles_i);
+        const int step_j = (int)(stride / (uint32_t)tiles_i), step_i = (int)stride - step_j * tiles_i;
         const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
         const int il = q * 32 + lane;                        // row of this thread inside the tile (and il + 128)
         int ib_loaded = -1, e0 = 0, e1 = 0;
         int fnext = t0 < total ? __ldg(f + j) : 0;           // f_j of the tile about to be processed, loaded one tile ahead
-        for (int64_t t = t0; t < total; t += 2 * (int64_t)G) {
+        for (uint32_t t = t0; t < total; t += stride) {
             const int i = ib * K5_TILE_I + il;
             const int jcur = j;
             const bool ok_a = i < m, ok_b = i + 128 < m;
@@ -477,7 +529,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
             const int fj = fnext;
             ib += step_i; j += step_j;
             if (ib >= tiles_i) { ib -= tiles_i; j++; }
-            if (t + 2 * (int64_t)G < total) fnext = __ldg(f + j);
+            if (t + stride < total) fnext = __ldg(f + j);
             mbar_wait_a(tfull + 8 * b, bph);
             tc_fence_after();
             uint32_t S[BUF_COLS];
@@ -494,9 +546,11 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
             b += 2;
             if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
             if (ok_a) {
-                TO *dst = C + i + (int64_t)jcur * ldc;
+                const int64_t off = (int64_t)jcur * ldc + i;
                 uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)jcur * m + i) * 4 : nullptr;
-                k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, T, N, ok_a, ok_b, e0 + fj, e1 + fj, alpha, beta, dst, cpp);
+                const uint8_t *Uel = U + ((size_t)jcur * (size_t)mp + (size_t)i);
+                k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, N, ok_a, ok_b, e0 + fj, e1 + fj, alpha, beta, C + off, cpp, Uel,
+                                                    (size_t)n * (size_t)mp);
             }
         }
     }
@@ -527,10 +581,11 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
     // a grid that is a multiple of the tiles per column keeps every CTA on one row block (its exponents e_i stay in
     // registers); worth it while it costs less than an eighth of the resident slots
     if (tiles_i <= grid && grid - grid % tiles_i >= grid - grid / 8) grid -= grid % tiles_i;
-    const int mi = (int)m, ni = (int)n;
-    if (Cpp) k5_crt_tc<NW, true, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldc, Cpp);
-    else if (beta == (TO)0) k5_crt_tc<NW, false, true, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldc, nullptr);
-    else k5_crt_tc<NW, false, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldc, nullptr);
+    if (tiles + 2 * grid >= (int64_t)1 << 31 || ldc >= (int64_t)1 << 31 || mp >= (int64_t)1 << 31) return (int)cudaErrorInvalidValue;
+    const int mi = (int)m, ni = (int)n, ldi = (int)ldc, mpi = (int)mp;
+    if (Cpp) k5_crt_tc<NW, true, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, Cpp, U, mpi);
+    else if (beta == (TO)0) k5_crt_tc<NW, false, true, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, nullptr, U, mpi);
+    else k5_crt_tc<NW, false, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, nullptr, U, mpi);
     oz2_count_launches(1);
     return (int)cudaGetLastError();
 }
@@ -550,6 +605,21 @@ int oz2_crt_upload_tables(const Oz2HostTables &t)
                 img[N][(sl / 8) * 256 + (l / 16) * 128 + (sl % 8) * 16 + (l % 16)] = byte;
             }
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(g_wb_image, img, sizeof(img)));
+    // constants of the common case: Pn = 2^(32 NW) - P, K0 = 2^(32 (NW - 1)) / P, K1 = K0 2^-32
+    static K5Consts k5[OZ2_MAX_MODULI + 1];
+    memset(k5, 0, sizeof(k5));
+    for (int N = 2; N <= OZ2_MAX_MODULI; N++) {
+        const int nw = words_of_P(N);
+        unsigned long long borrow = 0;
+        for (int w = 0; w < nw; w++) {                       // 0 - P over nw words
+            const unsigned long long d = 0ull - (unsigned long long)t.crt[N].P[w] - borrow;
+            k5[N].Pn[w] = (uint32_t)d;
+            borrow = (d >> 32) & 1ull;
+        }
+        k5[N].K0 = t.crt[N].invP;
+        k5[N].K1 = t.crt[N].invP * 2.3283064365386963e-10;
+    }
+    OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_k5, k5, sizeof(k5)));
     return 0;
 }
 
