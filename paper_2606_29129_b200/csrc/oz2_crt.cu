@@ -343,9 +343,9 @@ __device__ __noinline__ TO crt_exact_global(const uint8_t *__restrict__ Uel, siz
 // multiply-adds per element on the integer pipe; the epilogue threads (one element each) only fold the slices
 // into words and run crt_from_words.
 // =============================================================================================
-constexpr int K5_STAGES = 4, K5_NBUF = 4, K5_THREADS = 320;     // warps: TMA, MMA, 2 sets of 4 epilogue warps
-constexpr int K5_TILE_I = 256, K5_KPAD = 32;                    // one pipeline step = 2 MMAs of 128 elements
-constexpr int K5_STAGE_BYTES = K5_TILE_I * K5_KPAD;             // 8 KB
+constexpr int K5_STAGES = 3, K5_NBUF = 2, K5_THREADS = 320;     // warps: TMA, MMA, 2 sets of 4 epilogue warps
+constexpr int K5_TILE_I = 512, K5_KPAD = 32;                    // one pipeline step = 4 MMAs of 128 elements
+constexpr int K5_STAGE_BYTES = K5_TILE_I * K5_KPAD;             // 16 KB
 constexpr int K5_SMEM = K5_STAGES * K5_STAGE_BYTES + 1024 /*B image*/ + 1024 /*alignment*/ + 512 /*barriers*/;
 
 __device__ uint8_t g_wb_image[OZ2_MAX_MODULI + 1][1024];        // per N: B operand image (see upload)
@@ -394,30 +394,39 @@ __device__ __forceinline__ void k5_store(TO cij, TO alpha, TO beta, TO *dst)
 // the two elements (i, j) and (i + 128, j) of one thread: C'' -> C -> alpha / beta -> store.  Both go through the
 // branch-free crt_fast side by side (two independent dependency chains per thread); the exact routine is the rare path.
 template <int NW, bool WANT_CPP, bool BETA0, typename TO>
-__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, int N, bool ok_a, bool ok_b,
-                                           int esum_a, int esum_b, TO alpha, TO beta, TO *__restrict__ dst,
-                                           uint64_t *__restrict__ cpp, const uint8_t *__restrict__ Uel, size_t plane)
+__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, int N, bool ok_b, int esum_a, int esum_b, TO alpha,
+                                           TO beta, TO *__restrict__ C, int ldc, uint64_t *__restrict__ Cpp, int m,
+                                           const uint8_t *__restrict__ U, int mp, size_t plane, int i, int j)
 {
     TO va, vb;
     if constexpr (WANT_CPP) {
+        uint64_t *cpp = Cpp + ((size_t)j * m + i) * 4;
         CWords<NW> wa, wb;
         k5_fold<NW>(Sa, wa.w);
         k5_fold<NW>(Sb, wb.w);
-        va = ok_a ? crt_exact_v<NW, TO>(wa, N, esum_a, cpp) : (TO)0;
+        va = crt_exact_v<NW, TO>(wa, N, esum_a, cpp);
         vb = ok_b ? crt_exact_v<NW, TO>(wb, N, esum_b, cpp + 128 * 4) : (TO)0;
     } else {
         bool rare_a, rare_b;
         va = crt_fast<NW, TO>(Sa, c_k5[N], esum_a, rare_a);
         vb = crt_fast<NW, TO>(Sb, c_k5[N], esum_b, rare_b);
-        if ((rare_a && ok_a) || (rare_b && ok_b)) {                   // rare: near-half quotient, subnormal or overflowing result
-            if (rare_a && ok_a) va = crt_exact_global<NW, TO>(Uel, plane, N, esum_a);
+        if (rare_a || (rare_b && ok_b)) {                             // rare: near-half quotient, subnormal or overflowing result
+            const uint8_t *Uel = U + ((size_t)j * (size_t)mp + (size_t)i);
+            if (rare_a) va = crt_exact_global<NW, TO>(Uel, plane, N, esum_a);
             if (rare_b && ok_b) vb = crt_exact_global<NW, TO>(Uel + 128, plane, N, esum_b);
         }
     }
-    if (ok_a) k5_store<BETA0, TO>(va, alpha, beta, dst);
+    TO *dst = C + ((int64_t)j * ldc + i);
+    k5_store<BETA0, TO>(va, alpha, beta, dst);
     if (ok_b) k5_store<BETA0, TO>(vb, alpha, beta, dst + 128);
 }
 
+// One pipeline step = a tile of 512 consecutive elements of one column of C: four TMA boxes (128 elements x 32 planes)
+// in one 16 KB stage, four MMAs into one accumulator buffer of 4 NS columns.  The two epilogue sets take every second
+// tile of the CTA; a thread owns the four elements il + 128 h of its tile and works through them as two pairs, so that
+// the barrier wait, the tile walk, f_j and the address arithmetic are paid once per four elements.  Each set has ONE
+// accumulator buffer: it is handed back as soon as the second pair has been read out of tensor memory, i.e. half a
+// tile of epilogue work before the set needs the next one.
 template <int NW, bool WANT_CPP, bool BETA0, typename TO>
 __global__ void __launch_bounds__(K5_THREADS, NW <= 4 ? 3 : 2)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const int32_t *__restrict__ e,
@@ -425,7 +434,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
           uint64_t *__restrict__ Cpp, const uint8_t *__restrict__ U, int mp)
 {
     constexpr int NS = NW <= 4 ? 16 : 32;                    // byte slices = MMA N
-    constexpr int BUF_COLS = 2 * NS;                         // two 128-element MMAs per accumulator buffer
+    constexpr int BUF_COLS = 4 * NS;                         // four 128-element MMAs per accumulator buffer
     // kind::i8 instruction descriptor: D = S32, A = B = unsigned 8 bit, A MN-major, B K-major, N = NS, M = 128
     constexpr uint32_t IDESC = (2u << 4) | (1u << 15) | ((uint32_t)(NS >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
     extern __shared__ uint8_t smem_raw[];
@@ -476,8 +485,9 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
                 mbar_wait_idle(empty + 8 * s, ph ^ 1u);          // the epilogue paces this kernel: poll lazily
                 mbar_expect_tx_a(full + 8 * s, K5_STAGE_BYTES);
                 const uint32_t dst = smem0 + s * K5_STAGE_BYTES;
-                tma_load_3d_a(&mapU, full + 8 * s, dst, ib * K5_TILE_I, j, 0);
-                tma_load_3d_a(&mapU, full + 8 * s, dst + K5_STAGE_BYTES / 2, ib * K5_TILE_I + 128, j, 0);
+#pragma unroll
+                for (int h = 0; h < 4; h++)                      // boxes past the end of the column are zero filled
+                    tma_load_3d_a(&mapU, full + 8 * s, dst + h * (K5_STAGE_BYTES / 4), ib * K5_TILE_I + 128 * h, j, 0);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
                 ib += step_i; j += step_j;
                 if (ib >= tiles_i) { ib -= tiles_i; j++; }
@@ -492,13 +502,14 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
             // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
             const uint64_t adesc0 = ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
             for (uint32_t t = blockIdx.x; t < total; t += G) {
-                mbar_wait_idle(tempty + 8 * b, bph ^ 1u);
+                mbar_wait_a(tempty + 8 * b, bph ^ 1u);
                 mbar_wait_idle(full + 8 * s, ph);
                 tc_fence_after();
                 const uint32_t sa = smem0 + s * K5_STAGE_BYTES;
-                tc_mma_i8(tmem_base + (uint32_t)(b * BUF_COLS), adesc0 | (uint64_t)((sa & 0x3FFFFu) >> 4), bdesc, IDESC, 0u);
-                tc_mma_i8(tmem_base + (uint32_t)(b * BUF_COLS + NS), adesc0 | (uint64_t)(((sa + K5_STAGE_BYTES / 2) & 0x3FFFFu) >> 4),
-                          bdesc, IDESC, 0u);
+#pragma unroll
+                for (int h = 0; h < 4; h++)
+                    tc_mma_i8(tmem_base + (uint32_t)(b * BUF_COLS + h * NS),
+                              adesc0 | (uint64_t)(((sa + h * (K5_STAGE_BYTES / 4)) & 0x3FFFFu) >> 4), bdesc, IDESC, 0u);
                 tc_commit_a(empty + 8 * s);
                 tc_commit_a(tfull + 8 * b);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
@@ -508,49 +519,47 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     } else {
         const int q = warp & 3;                              // TMEM lane quarter of this warp
         const int set = (warp - 2) >> 2;                     // epilogue set 0 / 1 takes every second tile of the CTA
-        int b = set; uint32_t bph = 0;
+        uint32_t bph = 0;
+        const uint32_t bar_full = tfull + 8 * set, bar_empty = tempty + 8 * set;
         // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
         const uint32_t t0 = blockIdx.x + (uint32_t)set * G, stride = 2u * G;
         int j = (int)(t0 / (uint32_t)tiles_i), ib = (int)(t0 - (uint32_t)j * (uint32_t)tiles_i);
         const int step_j = (int)(stride / (uint32_t)tiles_i), step_i = (int)stride - step_j * tiles_i;
-        const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
-        const int il = q * 32 + lane;                        // row of this thread inside the tile (and il + 128)
-        int ib_loaded = -1, e0 = 0, e1 = 0;
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(set * BUF_COLS);
+        const int il = q * 32 + lane;                        // row of this thread inside the tile (and il + 128 h)
+        const size_t plane = (size_t)n * (size_t)mp;
+        int ib_loaded = -1, ev[4] = { 0, 0, 0, 0 };
         int fnext = t0 < total ? __ldg(f + j) : 0;           // f_j of the tile about to be processed, loaded one tile ahead
         for (uint32_t t = t0; t < total; t += stride) {
             const int i = ib * K5_TILE_I + il;
             const int jcur = j;
-            const bool ok_a = i < m, ok_b = i + 128 < m;
             if (ib != ib_loaded) {                           // with gridDim.x a multiple of tiles_i this happens once
-                e0 = ok_a ? __ldg(e + i) : 0;
-                e1 = ok_b ? __ldg(e + i + 128) : 0;
+#pragma unroll
+                for (int h = 0; h < 4; h++) ev[h] = i + 128 * h < m ? __ldg(e + i + 128 * h) : 0;
                 ib_loaded = ib;
             }
             const int fj = fnext;
             ib += step_i; j += step_j;
             if (ib >= tiles_i) { ib -= tiles_i; j++; }
             if (t + stride < total) fnext = __ldg(f + j);
-            mbar_wait_a(tfull + 8 * b, bph);
+            mbar_wait_a(bar_full, bph);
+            bph ^= 1u;
             tc_fence_after();
-            uint32_t S[BUF_COLS];
-            if constexpr (NS == 16) {
-                tc_ld32(lane_base + (uint32_t)(b * BUF_COLS), *reinterpret_cast<uint32_t(*)[32]>(S));
-            } else {
-                tc_ld32(lane_base + (uint32_t)(b * BUF_COLS), *reinterpret_cast<uint32_t(*)[32]>(S));
-                tc_ld32(lane_base + (uint32_t)(b * BUF_COLS + 32), *reinterpret_cast<uint32_t(*)[32]>(S + 32));
-            }
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_a(tempty + 8 * b);
-            b += 2;
-            if (b >= K5_NBUF) { b -= K5_NBUF; bph ^= 1u; }
-            if (ok_a) {
-                const int64_t off = (int64_t)jcur * ldc + i;
-                uint64_t *cpp = WANT_CPP ? Cpp + ((size_t)jcur * m + i) * 4 : nullptr;
-                const uint8_t *Uel = U + ((size_t)jcur * (size_t)mp + (size_t)i);
-                k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, N, ok_a, ok_b, e0 + fj, e1 + fj, alpha, beta, C + off, cpp, Uel,
-                                                    (size_t)n * (size_t)mp);
+#pragma unroll
+            for (int pr = 0; pr < 2; pr++) {                 // elements (i + 256 pr, i + 256 pr + 128)
+                uint32_t S[2 * NS];
+                tc_ld32(taddr + (uint32_t)(pr * 2 * NS), *reinterpret_cast<uint32_t(*)[32]>(S));
+                if constexpr (NS == 32) tc_ld32(taddr + (uint32_t)(pr * 2 * NS + 32), *reinterpret_cast<uint32_t(*)[32]>(S + 32));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (pr == 1) {                               // both pairs are out of tensor memory: hand the buffer back
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_a(bar_empty);
+                }
+                const int ia = i + 256 * pr;
+                if (ia < m)
+                    k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, N, ia + 128 < m, ev[2 * pr] + fj, ev[2 * pr + 1] + fj, alpha, beta, C, ldc,
+                                                        Cpp, m, U, mp, plane, ia, jcur);
             }
         }
     }
@@ -575,7 +584,7 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
     const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I, tiles = tiles_i * n;
-    const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads
+    const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads; 3 x 51 KB shared
     int64_t grid = (int64_t)sms * per_sm;
     if (grid > tiles) grid = tiles;
     // a grid that is a multiple of the tiles per column keeps every CTA on one row block (its exponents e_i stay in
@@ -583,9 +592,20 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
     if (tiles_i <= grid && grid - grid % tiles_i >= grid - grid / 8) grid -= grid % tiles_i;
     if (tiles + 2 * grid >= (int64_t)1 << 31 || ldc >= (int64_t)1 << 31 || mp >= (int64_t)1 << 31) return (int)cudaErrorInvalidValue;
     const int mi = (int)m, ni = (int)n, ldi = (int)ldc, mpi = (int)mp;
-    if (Cpp) k5_crt_tc<NW, true, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, Cpp, U, mpi);
-    else if (beta == (TO)0) k5_crt_tc<NW, false, true, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, nullptr, U, mpi);
-    else k5_crt_tc<NW, false, false, TO><<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, nullptr, U, mpi);
+    static bool attr_set[3] = { false, false, false };     // per kernel variant of this (NW, TO) instantiation
+    auto launch = [&](auto kern, int variant, uint64_t *cpp) -> int {
+        if (!attr_set[variant]) {
+            OZ2_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K5_SMEM));
+            attr_set[variant] = true;
+        }
+        kern<<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, cpp, U, mpi);
+        return 0;
+    };
+    int lrc;
+    if (Cpp) lrc = launch(k5_crt_tc<NW, true, false, TO>, 0, Cpp);
+    else if (beta == (TO)0) lrc = launch(k5_crt_tc<NW, false, true, TO>, 1, nullptr);
+    else lrc = launch(k5_crt_tc<NW, false, false, TO>, 2, nullptr);
+    if (lrc) return lrc;
     oz2_count_launches(1);
     return (int)cudaGetLastError();
 }
