@@ -198,13 +198,14 @@ __device__ __forceinline__ void mp_inc(uint32_t (&x)[W], uint32_t one)
             : "+r"(x[0]), "+r"(x[1]), "+r"(x[2]), "+r"(x[3]), "+r"(x[4]) : "r"(one));
 }
 
-// per-N constants of the common case (constant bank; the compiler keeps them in uniform registers)
+// per-N constants of the common case; passed to the kernel by value (__grid_constant__), so that they are constant-bank
+// operands of the instructions that use them and are never loaded
 struct K5Consts {
     uint32_t Pn[OZ2_MAX_WORDS];     // 2^(32 NW) - P: C' + Q Pn = C' - Q P  (mod 2^(32 NW))
     uint32_t nterms;                // (unused padding)
     double K0, K1;                  // 2^(32 (NW-1)) / P and 2^(32 (NW-2)) / P: weights of the two top 32-bit columns
 };
-__constant__ K5Consts c_k5[OZ2_MAX_MODULI + 1];
+K5Consts h_k5[OZ2_MAX_MODULI + 1];                 // host copy, filled by oz2_crt_upload_tables
 
 // The common case without a branch, straight from the byte slices S[0 .. 4 NW) of one element:
 //   Z_k  = sum_b S[4k+b] 256^b (< 2^46): the 32-bit columns of C' before carries, C' = sum_k Z_k 2^(32 k)
@@ -394,7 +395,7 @@ __device__ __forceinline__ void k5_store(TO cij, TO alpha, TO beta, TO *dst)
 // the two elements (i, j) and (i + 128, j) of one thread: C'' -> C -> alpha / beta -> store.  Both go through the
 // branch-free crt_fast side by side (two independent dependency chains per thread); the exact routine is the rare path.
 template <int NW, bool WANT_CPP, bool BETA0, typename TO>
-__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, int N, bool ok_b, int esum_a, int esum_b, TO alpha,
+__device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *Sb, const K5Consts &T, int N, bool ok_b, int esum_a, int esum_b, TO alpha,
                                            TO beta, TO *__restrict__ C, int ldc, uint64_t *__restrict__ Cpp, int m,
                                            const uint8_t *__restrict__ U, int mp, size_t plane, int i, int j)
 {
@@ -408,8 +409,8 @@ __device__ __forceinline__ void k5_finish2(const uint32_t *Sa, const uint32_t *S
         vb = ok_b ? crt_exact_v<NW, TO>(wb, N, esum_b, cpp + 128 * 4) : (TO)0;
     } else {
         bool rare_a, rare_b;
-        va = crt_fast<NW, TO>(Sa, c_k5[N], esum_a, rare_a);
-        vb = crt_fast<NW, TO>(Sb, c_k5[N], esum_b, rare_b);
+        va = crt_fast<NW, TO>(Sa, T, esum_a, rare_a);
+        vb = crt_fast<NW, TO>(Sb, T, esum_b, rare_b);
         if (rare_a || (rare_b && ok_b)) {                             // rare: near-half quotient, subnormal or overflowing result
             const uint8_t *Uel = U + ((size_t)j * (size_t)mp + (size_t)i);
             if (rare_a) va = crt_exact_global<NW, TO>(Uel, plane, N, esum_a);
@@ -431,7 +432,7 @@ template <int NW, bool WANT_CPP, bool BETA0, typename TO>
 __global__ void __launch_bounds__(K5_THREADS, NW <= 4 ? 3 : 2)
 k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const int32_t *__restrict__ e,
           const int32_t *__restrict__ f, TO alpha, TO beta, TO *__restrict__ C, int ldc,
-          uint64_t *__restrict__ Cpp, const uint8_t *__restrict__ U, int mp)
+          uint64_t *__restrict__ Cpp, const uint8_t *__restrict__ U, int mp, const __grid_constant__ K5Consts T, int ib0, int nib)
 {
     constexpr int NS = NW <= 4 ? 16 : 32;                    // byte slices = MMA N
     constexpr int BUF_COLS = 4 * NS;                         // four 128-element MMAs per accumulator buffer
@@ -445,10 +446,10 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     uint8_t *gen0 = smem_raw + (smem0 - smem_u32(smem_raw));                // generic pointer to the aligned base
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // tile t = j * tiles_i + ib (ib fastest), walked with stride gridDim.x; (j, ib) advance without a division
-    const int tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
-    const uint32_t total = (uint32_t)tiles_i * (uint32_t)n;          // < 2^31 - 2 gridDim.x (checked by the launcher)
-    const uint32_t G = gridDim.x;
+    // The grid is nib x gj CTAs: CTA b owns row block ib = ib0 + b % nib (512 rows: its exponents e_i stay in registers) and
+    // walks the columns j = b / nib, + gj, + 2 gj, ...
+    const int gj = (int)gridDim.x / nib;
+    const int j0 = (int)blockIdx.x / nib, ib = ib0 + ((int)blockIdx.x - j0 * nib);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < K5_STAGES; s++) {
@@ -478,10 +479,8 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
 
     if (warp == 0) {
         if (lane == 0) {
-            const int step_j = (int)G / tiles_i, step_i = (int)G - step_j * tiles_i;
-            int j = (int)blockIdx.x / tiles_i, ib = (int)blockIdx.x - j * tiles_i;
             int s = 0; uint32_t ph = 0;
-            for (uint32_t t = blockIdx.x; t < total; t += G) {
+            for (int j = j0; j < n; j += gj) {
                 mbar_wait_idle(empty + 8 * s, ph ^ 1u);          // the epilogue paces this kernel: poll lazily
                 mbar_expect_tx_a(full + 8 * s, K5_STAGE_BYTES);
                 const uint32_t dst = smem0 + s * K5_STAGE_BYTES;
@@ -489,8 +488,6 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
                 for (int h = 0; h < 4; h++)                      // boxes past the end of the column are zero filled
                     tma_load_3d_a(&mapU, full + 8 * s, dst + h * (K5_STAGE_BYTES / 4), ib * K5_TILE_I + 128 * h, j, 0);
                 if (++s == K5_STAGES) { s = 0; ph ^= 1u; }
-                ib += step_i; j += step_j;
-                if (ib >= tiles_i) { ib -= tiles_i; j++; }
             }
         }
     } else if (warp == 1) {
@@ -501,7 +498,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
                                    ((uint64_t)(256u >> 4) << 32) | (1ull << 46);
             // A: MN-major, SWIZZLE_128B: one 128-byte MN block per K row, 8-row K groups 1024 B apart (SBO)
             const uint64_t adesc0 = ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
-            for (uint32_t t = blockIdx.x; t < total; t += G) {
+            for (int j = j0; j < n; j += gj) {
                 mbar_wait_a(tempty + 8 * b, bph ^ 1u);
                 mbar_wait_idle(full + 8 * s, ph);
                 tc_fence_after();
@@ -521,27 +518,20 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
         const int set = (warp - 2) >> 2;                     // epilogue set 0 / 1 takes every second tile of the CTA
         uint32_t bph = 0;
         const uint32_t bar_full = tfull + 8 * set, bar_empty = tempty + 8 * set;
-        // this set starts at tile blockIdx.x + set * gridDim.x and strides by 2 * gridDim.x
-        const uint32_t t0 = blockIdx.x + (uint32_t)set * G, stride = 2u * G;
-        int j = (int)(t0 / (uint32_t)tiles_i), ib = (int)(t0 - (uint32_t)j * (uint32_t)tiles_i);
-        const int step_j = (int)(stride / (uint32_t)tiles_i), step_i = (int)stride - step_j * tiles_i;
+        // this set takes the columns j0 + set gj, + 2 gj, ...
+        const int stride = 2 * gj;
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(set * BUF_COLS);
-        const int il = q * 32 + lane;                        // row of this thread inside the tile (and il + 128 h)
+        const int i = ib * K5_TILE_I + q * 32 + lane;        // first of the four rows i + 128 h of this thread
         const size_t plane = (size_t)n * (size_t)mp;
-        int ib_loaded = -1, ev[4] = { 0, 0, 0, 0 };
-        int fnext = t0 < total ? __ldg(f + j) : 0;           // f_j of the tile about to be processed, loaded one tile ahead
-        for (uint32_t t = t0; t < total; t += stride) {
-            const int i = ib * K5_TILE_I + il;
-            const int jcur = j;
-            if (ib != ib_loaded) {                           // with gridDim.x a multiple of tiles_i this happens once
+        int ev[4];
 #pragma unroll
-                for (int h = 0; h < 4; h++) ev[h] = i + 128 * h < m ? __ldg(e + i + 128 * h) : 0;
-                ib_loaded = ib;
-            }
+        for (int h = 0; h < 4; h++) ev[h] = i + 128 * h < m ? __ldg(e + i + 128 * h) : 0;
+        int j = j0 + set * gj;
+        int fnext = j < n ? __ldg(f + j) : 0;                // f_j of the tile about to be processed, loaded one tile ahead
+        for (; j < n; j += stride) {
+            const int jcur = j;
             const int fj = fnext;
-            ib += step_i; j += step_j;
-            if (ib >= tiles_i) { ib -= tiles_i; j++; }
-            if (t + stride < total) fnext = __ldg(f + j);
+            if (j + stride < n) fnext = __ldg(f + j + stride);
             mbar_wait_a(bar_full, bph);
             bph ^= 1u;
             tc_fence_after();
@@ -558,7 +548,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
                 }
                 const int ia = i + 256 * pr;
                 if (ia < m)
-                    k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, N, ia + 128 < m, ev[2 * pr] + fj, ev[2 * pr + 1] + fj, alpha, beta, C, ldc,
+                    k5_finish2<NW, WANT_CPP, BETA0, TO>(S, S + NS, T, N, ia + 128 < m, ev[2 * pr] + fj, ev[2 * pr + 1] + fj, alpha, beta, C, ldc,
                                                         Cpp, m, U, mp, plane, ia, jcur);
             }
         }
@@ -583,14 +573,10 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
-    const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I, tiles = tiles_i * n;
+    const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
     const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads; 3 x 51 KB shared
-    int64_t grid = (int64_t)sms * per_sm;
-    if (grid > tiles) grid = tiles;
-    // a grid that is a multiple of the tiles per column keeps every CTA on one row block (its exponents e_i stay in
-    // registers); worth it while it costs less than an eighth of the resident slots
-    if (tiles_i <= grid && grid - grid % tiles_i >= grid - grid / 8) grid -= grid % tiles_i;
-    if (tiles + 2 * grid >= (int64_t)1 << 31 || ldc >= (int64_t)1 << 31 || mp >= (int64_t)1 << 31) return (int)cudaErrorInvalidValue;
+    const int64_t gmax = (int64_t)sms * per_sm;
+    if (ldc >= (int64_t)1 << 31 || mp >= (int64_t)1 << 31) return (int)cudaErrorInvalidValue;
     const int mi = (int)m, ni = (int)n, ldi = (int)ldc, mpi = (int)mp;
     static bool attr_set[3] = { false, false, false };     // per kernel variant of this (NW, TO) instantiation
     auto launch = [&](auto kern, int variant, uint64_t *cpp) -> int {
@@ -598,7 +584,15 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
             OZ2_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K5_SMEM));
             attr_set[variant] = true;
         }
-        kern<<<(unsigned)grid, K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, cpp, U, mpi);
+        // grid = (row blocks of the launch) x (columns in flight); more row blocks than resident CTAs: several launches
+        for (int64_t ib0 = 0; ib0 < tiles_i; ib0 += gmax) {
+            const int64_t nib = tiles_i - ib0 < gmax ? tiles_i - ib0 : gmax;
+            int64_t gj = gmax / nib;
+            if (gj > n) gj = n;
+            kern<<<(unsigned)(nib * gj), K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, cpp, U, mpi, h_k5[N], (int)ib0,
+                                                                  (int)nib);
+            oz2_count_launches(1);
+        }
         return 0;
     };
     int lrc;
@@ -606,7 +600,6 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
     else if (beta == (TO)0) lrc = launch(k5_crt_tc<NW, false, true, TO>, 1, nullptr);
     else lrc = launch(k5_crt_tc<NW, false, false, TO>, 2, nullptr);
     if (lrc) return lrc;
-    oz2_count_launches(1);
     return (int)cudaGetLastError();
 }
 
@@ -626,8 +619,8 @@ int oz2_crt_upload_tables(const Oz2HostTables &t)
             }
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(g_wb_image, img, sizeof(img)));
     // constants of the common case: Pn = 2^(32 NW) - P, K0 = 2^(32 (NW - 1)) / P, K1 = K0 2^-32
-    static K5Consts k5[OZ2_MAX_MODULI + 1];
-    memset(k5, 0, sizeof(k5));
+    K5Consts *k5 = h_k5;
+    memset(h_k5, 0, sizeof(h_k5));
     for (int N = 2; N <= OZ2_MAX_MODULI; N++) {
         const int nw = words_of_P(N);
         unsigned long long borrow = 0;
@@ -639,7 +632,6 @@ int oz2_crt_upload_tables(const Oz2HostTables &t)
         k5[N].K0 = t.crt[N].invP;
         k5[N].K1 = t.crt[N].invP * 2.3283064365386963e-10;
     }
-    OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_k5, k5, sizeof(k5)));
     return 0;
 }
 
