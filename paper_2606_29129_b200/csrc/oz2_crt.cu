@@ -208,7 +208,7 @@ struct K5Consts {
 K5Consts h_k5[OZ2_MAX_MODULI + 1];                 // host copy, filled by oz2_crt_upload_tables
 
 // The common case without a branch, straight from the byte slices S[0 .. 4 NW) of one element:
-//   Z_k  = sum_b S[4k+b] 256^b (< 2^46): the 32-bit columns of C' before carries, C' = sum_k Z_k 2^(32 k)
+//   Z_k  : the 32-bit columns of C' before carries, sum_b S[4k+b] 256^b (< 2^46) up to the pairing below; C' = sum_k Z_k 2^(32 k)
 //   Q    = round(C' / P) from the two top columns in FP64 (dropped columns < 2^-22.9, arithmetic < 2^-38: any Q within
 //          2^-20 of a half-integer is handed to the exact routine)
 //   R    = C' + Q (2^(32 NW) - P) mod 2^(32 NW) = C'' in two's complement: W_k = Z_k + Q Pn_k (< 2^47) per column, then
@@ -219,13 +219,22 @@ K5Consts h_k5[OZ2_MAX_MODULI + 1];                 // host copy, filled by oz2_c
 template <int NW, typename TO>
 __device__ __forceinline__ TO crt_fast(const uint32_t *S, const K5Consts &T, int esum, bool &rare)
 {
-    unsigned long long Z[NW];
+    // (the low halves a_k travel in pairs: Z_k carries a_k + 2^32 a_(k+1) as the 64-bit addend of its multiply-add and
+    // Z_(k+1) = 2^16 b_(k+1) none, so that no addend needs a zeroed high word; sum_k Z_k 2^(32 k) is unchanged)
+    uint32_t a[NW], b[NW];
 #pragma unroll
     for (int k = 0; k < NW; k++) {
-        const uint32_t a = S[4 * k] + (S[4 * k + 1] << 8), b = S[4 * k + 2] + (S[4 * k + 3] << 8);   // < 2^30
-        Z[k] = (unsigned long long)b * 65536ull + (unsigned long long)a;
+        a[k] = S[4 * k] + (S[4 * k + 1] << 8);                        // < 2^30
+        b[k] = S[4 * k + 2] + (S[4 * k + 3] << 8);
     }
-    // ---- Q (Z < 2^46: the conversions are exact)
+    unsigned long long Z[NW];
+#pragma unroll
+    for (int k = NW - 2; k >= 0; k -= 2) {
+        Z[k] = (unsigned long long)b[k] * 65536ull + (((unsigned long long)a[k + 1] << 32) | a[k]);
+        Z[k + 1] = (unsigned long long)b[k + 1] * 65536ull;
+    }
+    if constexpr (NW & 1) Z[0] = (unsigned long long)b[0] * 65536ull + (unsigned long long)a[0];
+    // ---- Q (Z < 2^63; the conversion of the second column may round: relative 2^-53, far below the guard)
     double qd = (double)(long long)Z[NW - 1] * T.K0;
     if constexpr (NW >= 2) qd = fma((double)(long long)Z[NW - 2], T.K1, qd);
     const double MAGIC = 6755399441055744.0;                          // 1.5 2^52: RN to an integer in the low word

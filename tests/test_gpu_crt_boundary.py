@@ -34,6 +34,21 @@ def boundary_integers(N, count_random, seed):
         for sgn in (1, -1):
             for d in (t * step, -t * step, t, -t):
                 zs.append(sgn * h + d)
+    # every magnitude class (leading bit 0 .. log2 P - 2: all word positions of the normalisation) and the rounding
+    # patterns of RN_64 / RN_32 at each of them: exact ties (round to even both ways), ties broken by a sticky bit far
+    # below, all-ones carries into the next binade
+    L = P.bit_length() - 2
+    for bpos in range(0, L + 1):
+        for v in ((1 << bpos), (1 << bpos) - 1, (1 << bpos) + 1):
+            if 0 < v < h:
+                zs.extend((v, -v))
+    for prec in (53, 24):
+        for sh in list(range(1, max(2, L - prec), 5)) + [max(1, L - prec - 1)]:
+            for mant in ((1 << prec) | 1, (1 << prec) | 3, (1 << (prec + 1)) - 1, (1 << prec) + 2):
+                base = (mant << sh) >> 1                      # prec + 1 significant bits: the last one is the round bit
+                for v in (base, base + 1, base - 1, base + (1 << (sh // 2)), base - (1 << (sh // 2))):
+                    if 0 < v < h:
+                        zs.extend((v, -v))
     rng = random.Random(seed)
     win = max(2, P >> 20)
     for _ in range(count_random):                     # within P 2^-20 of +-P/2: the near-half quotient window
@@ -57,7 +72,7 @@ def planes_from_integers(N, zs, m, n):
 @pytest.mark.parametrize("N", range(2, 21))
 def test_crt_kernel_on_boundary_residues(B, N):
     import torch
-    m, n = 272, 72                                    # 19584 elements, m = 16 * 17: ragged against the 256-row tile
+    m, n = 272, 96                                    # 26112 elements, m = 16 * 17: ragged against the 512-row tile
     zs, P = boundary_integers(N, 10000, 100 + N)
     assert len(zs) <= m * n
     U = planes_from_integers(N, zs, m, n)
@@ -119,3 +134,20 @@ def test_crt_kernel_alpha_beta_and_arguments(B):
     assert B.ozaki2_debug_crt(1, m, n, Ud, ed, fd, 1.0, 0.0, Cd, ldc) == -1
     assert B.ozaki2_debug_crt(N, m + 1, n, Ud, ed, fd, 1.0, 0.0, Cd, ldc) == -2
     assert B.ozaki2_debug_crt(N, m, n, Ud, ed, fd, 1.0, 0.0, Cd, m - 1) == -10
+
+
+def test_crt_kernel_more_row_blocks_than_resident_ctas(B):
+    """m beyond (resident CTAs) x 512 rows: the launcher covers the row blocks in several launches."""
+    import torch
+    N, m, n = 5, 148 * 3 * 512 + 704, 3              # m % 16 == 0: the debug entry uses the planes in place
+    rng = np.random.Generator(np.random.PCG64(77))
+    U = np.stack([rng.integers(0, q, size=(n, m), dtype=np.int64).astype(np.uint8) for q in O.constants(N)["p"]])
+    Cpp_o = O.crt(N, U)
+    e = rng.integers(-30, 30, size=m).astype(np.int32)
+    f = rng.integers(-30, 30, size=n).astype(np.int32)
+    want = O.unscale(Cpp_o, e, f)
+    Ud, ed, fd = torch.from_numpy(U).cuda(), torch.from_numpy(e).cuda(), torch.from_numpy(f).cuda()
+    Cd = torch.full((n, m), float("nan"), dtype=torch.float64, device="cuda")
+    assert B.ozaki2_debug_crt(N, m, n, Ud, ed, fd, 1.0, 0.0, Cd, m) == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(B.device_to_colmajor(Cd), want)
