@@ -1,5 +1,6 @@
 """GPU accuracy / invariance report on BASELINE configs[1] (-m gpu): 1024^3, eq. (15) phi = 1.0, N = 8..20, the three
-scaling modes, plus the scale-invariance variant c in {2^-500, 1e-100, 1, 1e100, 2^500}.
+scaling modes, plus the scale-invariance variant c in {2^-500, 1e-100, 1, 1e100, 2^500} and the
+paper's all-ones worked example alpha = 2^s, s = -10..10, N = 20, k in {1024, 16384} (Fig. 1 / Fig. 3).
 
 For every (N, mode) the CUDA result is compared bit for bit with the oracle's and its max elementwise relative error
 against the double-double reference is recorded.  The two table builders return their markdown lines to
@@ -135,8 +136,57 @@ def test_config1_scale_invariance_variant(B):
     assert ref[("2^-500", 1)][5] > 0                               # and violates condition (1) for small ones
 
 
+def allones_sweep_table(B, m=96, n=80):
+    """Fig. 1 / Fig. 3 analogue on the GPU: A = alpha ones, B = alpha ones, alpha = 2^s, s = -10..10,
+    N = 20, k in {1024, 16384}.  Returns (markdown lines, {(k, s, mode): (log2 (A'B')_ij, violated, max rel err)}).
+    The exact product is k alpha^2 (a power of two), so the error is exact; every GPU result is also compared bit for bit
+    with the oracle's."""
+    N = 20
+    import math
+    log2_half_P = math.log2(O.constants(N)["P"]) - 1.0
+    lines = ["", f"# All-ones worked example (P:232-257, Fig. 1 / Fig. 3): A = B^T = alpha ones, alpha = 2^s, N = {N}, GPU result ({m} x {n} x k)",
+             f"log2 (A'B')_ij against log2(P/2) = {log2_half_P:.2f} (`>` = condition (1) violated), and the max relative error against the exact k alpha^2",
+             "", "| k | s | accu: log2 A'B' | err | fast: log2 A'B' | err | prop: log2 A'B' | err |", "|---|---|---|---|---|---|---|---|"]
+    res = {}
+    for k in (1024, 16384):
+        for s_ in range(-10, 11):
+            A, Bm = W.all_ones_scaled(m, n, k, 2.0 ** s_)
+            exact = k * 4.0 ** s_
+            row = []
+            for mode in (0, 1, 2):
+                Cg, e, f = gpu_run(B, A, Bm, N, mode)
+                Co = O.dgemm(A, Bm, N, mode)
+                assert np.array_equal(Cg, Co), (k, s_, mode)
+                assert np.all(e == e[0]) and np.all(f == f[0])
+                lg = np.log2(k) + (s_ + int(e[0])) + (s_ + int(f[0]))           # a' = 2^(s+e), b' = 2^(s+f) exactly
+                viol = lg > log2_half_P
+                err = float(np.max(np.abs(Cg - exact)) / exact)
+                res[(k, s_, mode)] = (lg, viol, err)
+                row.append(f"{lg:.0f}{' >' if viol else ''} | {err:.3g}")
+            lines.append(f"| {k} | {s_} | " + " | ".join(row) + " |")
+    return lines, res
+
+
+def test_allones_worked_example(B):
+    """the original fast mode violates condition (1) exactly for alpha <= 2^-2 (both k); its error is then about 1
+    while accurate mode stays exact; the revised mode never violates and is exact for every s."""
+    _, res = allones_sweep_table(B)
+    for (k, s_, mode), (lg, viol, err) in res.items():
+        if mode == 1:
+            assert viol == (s_ <= -2), (k, s_)
+            if viol:
+                assert err > 0.5, (k, s_, err)
+        else:
+            assert not viol and err == 0.0, (k, s_, mode, err)
+    # plateau of the fast mode for alpha <= k^(-1/2) (P:236-244): A'B' = k 2^(2 floor(P'_fast - 1)) independent of s
+    for k in (1024, 16384):
+        plateau = {res[(k, s_, 1)][0] for s_ in range(-10, 11) if 4.0 ** s_ * k <= 1.0}
+        assert len(plateau) == 1, (k, plateau)
+
+
 if __name__ == "__main__":
     import paper_2606_29129_b200 as pkg
     pkg.lib()
     print("\n".join(config1_error_table(pkg)[0]))
     print("\n".join(scale_invariance_table(pkg)[0]))
+    print("\n".join(allones_sweep_table(pkg)[0]))
