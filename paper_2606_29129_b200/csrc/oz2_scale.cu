@@ -80,6 +80,24 @@ __device__ __forceinline__ unsigned long long sq_term(unsigned long long b, int 
     return __double2ull_ru(__dmul_ru(x, x));
 }
 
+// The same term for a whole vector whose E is known: x = RU(|v| 2^hs) with the scale 2^hs, hs = SQ/2 - E, held as a double.
+// While x is a normal number the product is an exact exponent shift; when it underflows, rounding up keeps 0 < x < 1, so
+// that ceil(RU(x x)) = 1 = ceil(x^2) as it must; v = 0 gives 0.  Three FP64 instructions per element instead of the
+// exponent-field arithmetic of sq_term.  Needs 2^hs representable: sq_scale_ok(E, SQ).
+__device__ __forceinline__ bool sq_scale_ok(int E, int SQ) { const int hs = (SQ >> 1) - E; return hs >= -1022 && hs <= 1023; }
+__device__ __forceinline__ double sq_scale(int E, int SQ) { return __longlong_as_double((long long)((SQ >> 1) - E + 1023) << 52); }
+__device__ __forceinline__ unsigned long long sq_term_scaled(double v, double scale)
+{
+    const double x = __dmul_ru(fabs(v), scale);
+    return __double2ull_ru(__dmul_ru(x, x));
+}
+
+// max |v| over a vector is needed only through floor(log2 .) and "is it zero": for normal numbers the high word of the
+// bit pattern decides both, so the streaming loops keep a 32-bit maximum of the high words (sign bit cleared); only a
+// vector whose high-word maximum stays below 2^20 (nothing but subnormals and zeros) is re-read for the exact pattern.
+__device__ __forceinline__ uint32_t hi_abs(double v) { return (uint32_t)__double2hiint(v) & 0x7FFFFFFFu; }
+constexpr uint32_t HI_NORMAL = 0x00100000u;
+
 // LOG2F(x) = RN_32(log2 x) for float x in [1,2] (reading R3): FP64 log2 (<= 1 ulp), rounded once.
 __device__ __forceinline__ float log2f_rn(float x) { return __double2float_rn(log2((double)x)); }
 
@@ -135,32 +153,49 @@ k1_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, int64_t kchu
     int64_t h1 = h0 + kchunk < k ? h0 + kchunk : k;
     if (i >= m) return;
     const T *p = A + i;
-    unsigned long long acc = 0;
-    int E = 0;
-    if (PASS == 1) {
-        unsigned long long mx = amax[i];
-        if (mx == 0) return;
-        E = floor_log2_bits(mx);
-    }
-    int64_t h = h0 + threadIdx.y;
-    for (; h + 7 * KSLICES < h1; h += 8 * KSLICES) {
-        double v[8];
+    if (PASS == 0) {
+        uint32_t mh = 0;
+        int64_t h = h0 + threadIdx.y;
+        for (; h + 7 * KSLICES < h1; h += 8 * KSLICES) {
+            double v[8];
 #pragma unroll
-        for (int u = 0; u < 8; u++) v[u] = (double)__ldg(p + (h + u * KSLICES) * lda);
+            for (int u = 0; u < 8; u++) v[u] = (double)__ldg(p + (h + u * KSLICES) * lda);
 #pragma unroll
-        for (int u = 0; u < 8; u++) {
-            unsigned long long b = abs_bits(v[u]);
-            if (PASS == 0) acc = b > acc ? b : acc;
-            else acc += sq_term(b, E, SQ);
+            for (int u = 0; u < 8; u++) mh = max(mh, hi_abs(v[u]));
         }
+        for (; h < h1; h += KSLICES) mh = max(mh, hi_abs((double)__ldg(p + h * lda)));
+        if (mh >= HI_NORMAL) {
+            atomicMax(amax + i, (unsigned long long)mh << 32);    // same floor(log2 .) as the exact pattern
+        } else {
+            // nothing but subnormals and zeros in this slice (rare): exact 64-bit pattern
+            unsigned long long acc = 0;
+            for (int64_t hh = h0 + threadIdx.y; hh < h1; hh += KSLICES) {
+                const unsigned long long b = abs_bits((double)__ldg(p + hh * lda));
+                acc = b > acc ? b : acc;
+            }
+            if (acc) atomicMax(amax + i, acc);
+        }
+    } else {
+        const unsigned long long mx = amax[i];
+        if (mx == 0) return;
+        const int E = floor_log2_bits(mx);
+        unsigned long long acc = 0;
+        int64_t h = h0 + threadIdx.y;
+        if (sq_scale_ok(E, SQ)) {
+            const double scale = sq_scale(E, SQ);
+            for (; h + 7 * KSLICES < h1; h += 8 * KSLICES) {
+                double v[8];
+#pragma unroll
+                for (int u = 0; u < 8; u++) v[u] = (double)__ldg(p + (h + u * KSLICES) * lda);
+#pragma unroll
+                for (int u = 0; u < 8; u++) acc += sq_term_scaled(v[u], scale);
+            }
+            for (; h < h1; h += KSLICES) acc += sq_term_scaled((double)__ldg(p + h * lda), scale);
+        } else {
+            for (; h < h1; h += KSLICES) acc += sq_term(abs_bits((double)__ldg(p + h * lda)), E, SQ);
+        }
+        if (acc) atomicAdd(ssq + i, acc);
     }
-    for (; h < h1; h += KSLICES) {
-        unsigned long long b = abs_bits((double)__ldg(p + h * lda));
-        if (PASS == 0) acc = b > acc ? b : acc;
-        else acc += sq_term(b, E, SQ);
-    }
-    if (PASS == 0) { if (acc) atomicMax(amax + i, acc); }
-    else if (acc) atomicAdd(ssq + i, acc);
 }
 
 __global__ void k1_rows_finalize(int mode, int N, int64_t m, const unsigned long long *__restrict__ amax,
@@ -206,19 +241,23 @@ k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_
     __shared__ unsigned long long sm[COL_THREADS / 32];
     const T *col = B + (int64_t)blockIdx.x * ldb;
     bool vec = ((((uintptr_t)col) & (2 * sizeof(T) - 1)) == 0);
-    unsigned long long mx = 0;
     int64_t kv = vec ? (k & ~(int64_t)1) : 0;
+    uint32_t mh = 0;
     for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {
         double2 v = ld2(col + h);
-        unsigned long long b0 = abs_bits(v.x), b1 = abs_bits(v.y);
-        mx = b0 > mx ? b0 : mx;
-        mx = b1 > mx ? b1 : mx;
+        mh = max(mh, max(hi_abs(v.x), hi_abs(v.y)));
     }
-    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) {
-        unsigned long long b = abs_bits((double)__ldg(col + h));
-        mx = b > mx ? b : mx;
+    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) mh = max(mh, hi_abs((double)__ldg(col + h)));
+    unsigned long long mx = block_reduce((unsigned long long)mh << 32, true, sm);
+    if (mx < ((unsigned long long)HI_NORMAL << 32)) {
+        // nothing but subnormals and zeros in this column (rare; uniform for the block): exact 64-bit pattern
+        unsigned long long acc = 0;
+        for (int64_t h = threadIdx.x; h < k; h += COL_THREADS) {
+            const unsigned long long b = abs_bits((double)__ldg(col + h));
+            acc = b > acc ? b : acc;
+        }
+        mx = block_reduce(acc, true, sm);
     }
-    mx = block_reduce(mx, true, sm);
     if (ACCU) {
         if (threadIdx.x == 0) EB[blockIdx.x] = mx ? floor_log2_bits(mx) : OZ2_E_ZERO;
         return;
@@ -229,11 +268,16 @@ k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_
     }
     int E = floor_log2_bits(mx);
     unsigned long long acc = 0;
-    for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {      // second read: L2 hits
-        double2 v = ld2(col + h);
-        acc += sq_term(abs_bits(v.x), E, SQ) + sq_term(abs_bits(v.y), E, SQ);
+    if (sq_scale_ok(E, SQ)) {                                                           // uniform for the block
+        const double scale = sq_scale(E, SQ);
+        for (int64_t h = 2 * (int64_t)threadIdx.x; h < kv; h += 2 * COL_THREADS) {      // second read: L2 hits
+            double2 v = ld2(col + h);
+            acc += sq_term_scaled(v.x, scale) + sq_term_scaled(v.y, scale);
+        }
+        for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term_scaled((double)__ldg(col + h), scale);
+    } else {
+        for (int64_t h = threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits((double)__ldg(col + h)), E, SQ);
     }
-    for (int64_t h = kv + threadIdx.x; h < k; h += COL_THREADS) acc += sq_term(abs_bits((double)__ldg(col + h)), E, SQ);
     acc = block_reduce(acc, false, sm);
     if (threadIdx.x == 0) f[blockIdx.x] = exponent_fastprop(mode, c_crt[N], mx, acc, SQ);
 }
