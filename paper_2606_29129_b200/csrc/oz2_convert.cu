@@ -169,6 +169,38 @@ __device__ __forceinline__ void digits_wide(double a, int ex, uint32_t (&w)[3])
     w[2] = ((uint32_t)((int)(th >> 32) + (int)(tl >> 63) + carry)) ^ 0x80000000u;
 }
 
+// The common case of both formats: when 2^ex is a normal double (|ex| <= 1022), a 2^ex is ONE exact FP64 multiply by the
+// vector's scale -- also for subnormal a, and when the product falls below 1 (even into the subnormal range, where it may
+// round) the truncation gives 0 as it must -- so trunc(a 2^ex) is a multiply and a conversion, with no exponent-field
+// arithmetic.  Vectors whose exponent is outside that range (all entries below 2^-960 or so) take the routines above.
+__device__ __forceinline__ bool scale_ok(int ex) { return ex >= -1022 && ex <= 1022; }
+__device__ __forceinline__ double scale_of(int ex) { return __hiloint2double((ex + 1023) << 20, 0); }
+__device__ __forceinline__ unsigned long long digits_narrow_scaled(double a, double scale)
+{
+    return (unsigned long long)__double2ll_rz(a * scale) ^ 0x8000000000000000ull;
+}
+__device__ __forceinline__ void digits_wide_scaled(double a, double scale, uint32_t (&w)[3])
+{
+    const double x = a * scale;                                   // exact (or below 1)
+    const double hd = trunc(x * 2.3283064365386963e-10);          // th = trunc(a' / 2^32): exact, |.| < 2^52
+    const double rem = fma(hd, -4294967296.0, x);                 // exact: a multiple of ulp(x) below 2^32 in magnitude
+    const long long th = __double2ll_rz(hd), tl = __double2ll_rz(rem);
+    const unsigned long long top = (unsigned long long)th << 32;
+    const unsigned long long lo64 = top + (unsigned long long)tl;
+    const int carry = lo64 < top ? 1 : 0;
+    w[0] = (uint32_t)lo64;
+    w[1] = (uint32_t)(lo64 >> 32);
+    w[2] = ((uint32_t)((int)(th >> 32) + (int)(tl >> 63) + carry)) ^ 0x80000000u;
+}
+// the other vectors (rare, uniform for the warp): out of line
+__device__ __noinline__ unsigned long long digits_narrow_slow(double a, int ex) { return digits_narrow(a, ex); }
+__device__ __noinline__ uint3 digits_wide_slow(double a, int ex)
+{
+    uint32_t w[3];
+    digits_wide(a, ex, w);
+    return make_uint3(w[0], w[1], w[2]);
+}
+
 // ---------------------------------------------------------------------------------------------
 // per-round tensor-core step and epilogue
 // ---------------------------------------------------------------------------------------------
@@ -294,17 +326,31 @@ template <int WIDE, typename F>
 __device__ __forceinline__ void convert_quad(ConvCtx &cx, const double (&a)[4], int ex, int N, int8_t *dst,
                                              int64_t plane_stride, bool ok, F overlap)
 {
+    const double scale = scale_of(ex);
     if (!WIDE) {
-        const unsigned long long d0 = digits_narrow(a[0], ex), d1 = digits_narrow(a[1], ex);
-        const unsigned long long d2 = digits_narrow(a[2], ex), d3 = digits_narrow(a[3], ex);
-        sts128(cx.tile_row, (uint32_t)d0, (uint32_t)(d0 >> 32), (uint32_t)d1, (uint32_t)(d1 >> 32));
-        sts128(cx.tile_row + 128u, (uint32_t)d2, (uint32_t)(d2 >> 32), (uint32_t)d3, (uint32_t)(d3 >> 32));
+        unsigned long long d[4];
+        if (scale_ok(ex)) {                                                   // uniform for the warp
+#pragma unroll
+            for (int u = 0; u < 4; u++) d[u] = digits_narrow_scaled(a[u], scale);
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; u++) d[u] = digits_narrow_slow(a[u], ex);
+        }
+        sts128(cx.tile_row, (uint32_t)d[0], (uint32_t)(d[0] >> 32), (uint32_t)d[1], (uint32_t)(d[1] >> 32));
+        sts128(cx.tile_row + 128u, (uint32_t)d[2], (uint32_t)(d[2] >> 32), (uint32_t)d[3], (uint32_t)(d[3] >> 32));
     } else {
         uint32_t w0[3], w1[3], w2[3], w3[3];
-        digits_wide(a[0], ex, w0);
-        digits_wide(a[1], ex, w1);
-        digits_wide(a[2], ex, w2);
-        digits_wide(a[3], ex, w3);
+        if (scale_ok(ex)) {                                                   // uniform for the warp
+            digits_wide_scaled(a[0], scale, w0);
+            digits_wide_scaled(a[1], scale, w1);
+            digits_wide_scaled(a[2], scale, w2);
+            digits_wide_scaled(a[3], scale, w3);
+        } else {
+            uint3 r = digits_wide_slow(a[0], ex); w0[0] = r.x; w0[1] = r.y; w0[2] = r.z;
+            r = digits_wide_slow(a[1], ex); w1[0] = r.x; w1[1] = r.y; w1[2] = r.z;
+            r = digits_wide_slow(a[2], ex); w2[0] = r.x; w2[1] = r.y; w2[2] = r.z;
+            r = digits_wide_slow(a[3], ex); w3[0] = r.x; w3[1] = r.y; w3[2] = r.z;
+        }
         sts128(cx.tile_row, w0[0], w0[1], w1[0], w1[1]);
         sts128(cx.tile_row + 128u, w2[0], w2[1], w3[0], w3[1]);
         sts128(cx.tile_row + CV_TILE_BYTES, w0[2], 0u, w1[2], 0u);             // digits 8 .. 11 (12 .. 15 are zero)
