@@ -125,6 +125,16 @@ int ozaki2_zgemm(int64_t m, int64_t n, int64_t k, double alpha_re, double alpha_
                  int num_moduli, int scaling_mode, void *stream);
 size_t ozaki2_zgemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 
+/*
+ * The same for interleaved complex FP32 matrices (8-byte aligned device pointers): ozaki2_sgemm on the real embedding of the
+ * FP32 parts (one rounding RN_32 of the exact integer for each of c_r, c_i; P:375 for the moduli counts), then the tail
+ * out = alpha c + beta C with every product and sum rounded to FP32 on its own.  Workspace: ozaki2_cgemm_workspace_bytes.
+ */
+int ozaki2_cgemm(int64_t m, int64_t n, int64_t k, float alpha_re, float alpha_im, const float *A, int64_t lda,
+                 const float *B, int64_t ldb, float beta_re, float beta_im, float *C, int64_t ldc,
+                 int num_moduli, int scaling_mode, void *stream);
+size_t ozaki2_cgemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
+
 /* Bytes of device workspace ozaki2_dgemm / ozaki2_sgemm needs for this problem (0 for an invalid one). */
 size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 

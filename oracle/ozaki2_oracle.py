@@ -311,6 +311,37 @@ def zgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_
     return out
 
 
+def cgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_in=None):
+    """Single-precision complex variant (same reading as zgemm, DESIGN.md 8b #4): oz2o_sgemm on the real embedding of the FP32
+    parts, then out = alpha c + beta C_in in FP32 complex arithmetic -- every product and every sum rounded to FP32 on its own,
+    in the order written below; alpha == 1 and beta == 0 are not multiplied."""
+    A = np.asarray(A, dtype=np.complex64)
+    B = np.asarray(B, dtype=np.complex64)
+    m = A.shape[0]
+    At = np.asfortranarray(np.block([[A.real, -A.imag], [A.imag, A.real]]).astype(np.float32))
+    Bt = np.asfortranarray(np.vstack([B.real, B.imag]).astype(np.float32))
+    Ct = sgemm(At, Bt, N, mode)
+    cr, ci = Ct[:m], Ct[m:]
+    alpha, beta = complex(alpha), complex(beta)
+    f = np.float32
+    if alpha != 1.0:
+        ar, ai = f(alpha.real), f(alpha.imag)
+        with np.errstate(all="ignore"):
+            tr = (ar * cr).astype(f) - (ai * ci).astype(f)
+            ti = (ar * ci).astype(f) + (ai * cr).astype(f)
+    else:
+        tr, ti = cr, ci
+    if beta != 0.0:
+        Cin = np.asarray(C_in, dtype=np.complex64)
+        br, bi = f(beta.real), f(beta.imag)
+        with np.errstate(all="ignore"):
+            tr = tr + ((br * Cin.real).astype(f) - (bi * Cin.imag).astype(f))
+            ti = ti + ((br * Cin.imag).astype(f) + (bi * Cin.real).astype(f))
+    out = np.empty(cr.shape, np.complex64, order="F")
+    out.real, out.imag = tr, ti
+    return out
+
+
 def dd_reference(A, B):
     """AB in double-double: (hi, lo), each (m, n) column-major."""
     A, B = _f(A), _f(B)

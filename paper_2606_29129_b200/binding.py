@@ -69,6 +69,10 @@ def lib() -> C.CDLL:
         L.ozaki2_zgemm.restype = ci
         L.ozaki2_zgemm_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
         L.ozaki2_zgemm_workspace_bytes.restype = C.c_size_t
+        L.ozaki2_cgemm.argtypes = [i64, i64, i64, C.c_float, C.c_float, vp, i64, vp, i64, C.c_float, C.c_float, vp, i64, ci, ci, vp]
+        L.ozaki2_cgemm.restype = ci
+        L.ozaki2_cgemm_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
+        L.ozaki2_cgemm_workspace_bytes.restype = C.c_size_t
         L.ozaki2_debug_crt.argtypes = [ci, i64, i64, vp, vp, vp, dbl, dbl, vp, i64, vp, ci, vp]
         L.ozaki2_debug_crt.restype = ci
         L.ozaki2_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
@@ -213,8 +217,19 @@ def ozaki2_zgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scal
                                   num_moduli, scaling_mode, _stream(stream)))
 
 
+def ozaki2_cgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode) -> int:
+    return int(lib().ozaki2_cgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode))
+
+
+def ozaki2_cgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None) -> int:
+    """Single-precision complex variant: A, B, Cm are complex64 device tensors (column-major) or addresses."""
+    alpha, beta = complex(alpha), complex(beta)
+    return int(lib().ozaki2_cgemm(m, n, k, alpha.real, alpha.imag, _ptr(A), lda, _ptr(B), ldb, beta.real, beta.imag, _ptr(Cm), ldc,
+                                  num_moduli, scaling_mode, _stream(stream)))
+
+
 def ensure_zgemm_workspace(m, n, k, num_moduli, scaling_mode):
-    """Allocate (grow-only) and register a workspace large enough for ozaki2_zgemm on the current device."""
+    """Allocate (grow-only) and register a workspace large enough for ozaki2_zgemm (and ozaki2_cgemm) on the current device."""
     import torch
     need = ozaki2_zgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode)
     dev = torch.cuda.current_device()

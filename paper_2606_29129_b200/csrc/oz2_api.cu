@@ -285,13 +285,25 @@ __global__ void k_scale_c(int64_t m, int64_t n, T beta, T *C, int64_t ldc)
     }
 }
 
-// ---- complex variant (DESIGN.md 8b #4): real embedding and the complex alpha / beta tail -----------
+// ---- complex variants (DESIGN.md 8b #4): real embedding and the complex alpha / beta tail -----------
+// R = double (zgemm) or float (cgemm); R2 = the interleaved pair type
+template <typename R> struct Pair;
+template <> struct Pair<double> { typedef double2 type; };
+template <> struct Pair<float> { typedef float2 type; };
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+
 // Atilde (2m x 2k) = [[A_r, -A_i], [A_i, A_r]] from interleaved complex A (m x k, lda complex elements)
-__global__ void k_zembed_a(int64_t m, int64_t k, const double2 *__restrict__ A, int64_t lda, double *__restrict__ At)
+template <typename R>
+__global__ void k_zembed_a(int64_t m, int64_t k, const typename Pair<R>::type *__restrict__ A, int64_t lda, R *__restrict__ At)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, h = blockIdx.y;
     if (i >= m) return;
-    const double2 v = A[i + h * lda];
+    const typename Pair<R>::type v = A[i + h * lda];
     const int64_t ld = 2 * m;
     At[i + h * ld] = v.x;
     At[i + (k + h) * ld] = -v.y;
@@ -299,37 +311,41 @@ __global__ void k_zembed_a(int64_t m, int64_t k, const double2 *__restrict__ A, 
     At[m + i + (k + h) * ld] = v.x;
 }
 // Btilde (2k x n) = [B_r; B_i]
-__global__ void k_zembed_b(int64_t k, int64_t n, const double2 *__restrict__ B, int64_t ldb, double *__restrict__ Bt)
+template <typename R>
+__global__ void k_zembed_b(int64_t k, int64_t n, const typename Pair<R>::type *__restrict__ B, int64_t ldb, R *__restrict__ Bt)
 {
     const int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (h >= k) return;
-    const double2 v = B[h + j * ldb];
+    const typename Pair<R>::type v = B[h + j * ldb];
     Bt[h + j * 2 * k] = v.x;
     Bt[k + h + j * 2 * k] = v.y;
 }
 // C := alpha (c_r + i c_i) + beta C with [c_r; c_i] = Ct (2m x n); every product and sum rounded on its own, in the order
-// of the oracle (oracle/ozaki2_oracle.py zgemm); alpha == 1 and beta == 0 are not multiplied; have_c == 0: c = 0
-__global__ void k_zcombine(int64_t m, int64_t n, double ar, double ai, const double *__restrict__ Ct, int have_c, double br,
-                           double bi, double2 *__restrict__ C, int64_t ldc)
+// of the oracle (oracle/ozaki2_oracle.py zgemm / cgemm); alpha == 1 and beta == 0 are not multiplied; have_c == 0: c = 0
+template <typename R>
+__global__ void k_zcombine(int64_t m, int64_t n, R ar, R ai, const R *__restrict__ Ct, int have_c, R br, R bi,
+                           typename Pair<R>::type *__restrict__ C, int64_t ldc)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (i >= m) return;
-    double tr = 0.0, ti = 0.0;
+    R tr = 0, ti = 0;
     if (have_c) {
-        const double cr = Ct[i + j * 2 * m], ci = Ct[m + i + j * 2 * m];
-        if (ar == 1.0 && ai == 0.0) { tr = cr; ti = ci; }
+        const R cr = Ct[i + j * 2 * m], ci = Ct[m + i + j * 2 * m];
+        if (ar == (R)1 && ai == (R)0) { tr = cr; ti = ci; }
         else {
-            tr = __dsub_rn(__dmul_rn(ar, cr), __dmul_rn(ai, ci));
-            ti = __dadd_rn(__dmul_rn(ar, ci), __dmul_rn(ai, cr));
+            tr = sub_rn(mul_rn(ar, cr), mul_rn(ai, ci));
+            ti = add_rn(mul_rn(ar, ci), mul_rn(ai, cr));
         }
     }
-    double2 *dst = C + i + j * ldc;
-    if (br != 0.0 || bi != 0.0) {
-        const double2 c0 = *dst;
-        tr = __dadd_rn(tr, __dsub_rn(__dmul_rn(br, c0.x), __dmul_rn(bi, c0.y)));
-        ti = __dadd_rn(ti, __dadd_rn(__dmul_rn(br, c0.y), __dmul_rn(bi, c0.x)));
+    typename Pair<R>::type *dst = C + i + j * ldc;
+    if (br != (R)0 || bi != (R)0) {
+        const typename Pair<R>::type c0 = *dst;
+        tr = add_rn(tr, sub_rn(mul_rn(br, c0.x), mul_rn(bi, c0.y)));
+        ti = add_rn(ti, add_rn(mul_rn(br, c0.y), mul_rn(bi, c0.x)));
     }
-    *dst = make_double2(tr, ti);
+    typename Pair<R>::type o;
+    o.x = tr; o.y = ti;
+    *dst = o;
 }
 
 } // namespace
@@ -611,6 +627,65 @@ static int blas_entry(int f32, int layout, int transa, int transb, int64_t m, in
     return -(lay ? row[-rc] : col[-rc]);
 }
 
+static size_t complex_workspace_bytes(size_t esz, int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode)
+{
+    if (m < 0 || n < 0 || k < 0 || 2 * k > OZAKI2_MAX_K) return 0;
+    const size_t real_ws = ozaki2_workspace_bytes(2 * m, n, 2 * k, num_moduli, scaling_mode);
+    if (!real_ws && m && n && k) return 0;
+    return align_up(real_ws) + align_up(esz * (size_t)(2 * m) * (2 * k)) + align_up(esz * (size_t)(2 * k) * n) + align_up(esz * (size_t)(2 * m) * n);
+}
+
+// ozaki2_zgemm (R = double) / ozaki2_cgemm (R = float): embed, run the real path, combine
+template <typename R>
+static int complex_entry(int64_t m, int64_t n, int64_t k, R alpha_re, R alpha_im, const R *A, int64_t lda, const R *B, int64_t ldb,
+                         R beta_re, R beta_im, R *C, int64_t ldc, int num_moduli, int scaling_mode, void *stream)
+{
+    typedef typename Pair<R>::type R2;
+    constexpr size_t esz = sizeof(R);
+    constexpr uintptr_t amask = 2 * sizeof(R) - 1;                     // interleaved pairs: 16-byte (FP64) / 8-byte (FP32) aligned
+    if (m < 0) return -1;
+    if (n < 0) return -2;
+    if (k < 0 || 2 * k > OZAKI2_MAX_K || (scaling_mode == OZAKI2_MODE_ACCURATE && 2 * k > OZAKI2_MAX_K_ACCURATE)) return -3;
+    if (m > 0 && k > 0 && (!A || (reinterpret_cast<uintptr_t>(A) & amask))) return -6;
+    if (lda < (m > 1 ? m : 1)) return -7;
+    if (n > 0 && k > 0 && (!B || (reinterpret_cast<uintptr_t>(B) & amask))) return -8;
+    if (ldb < (k > 1 ? k : 1)) return -9;
+    if (m > 0 && n > 0 && (!C || (reinterpret_cast<uintptr_t>(C) & amask))) return -12;
+    if (ldc < (m > 1 ? m : 1)) return -13;
+    if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return -14;
+    if (scaling_mode < 0 || scaling_mode > 2) return -15;
+    if (m > (0x7FFFFFFFll - 1024) / 2 || n > 0x7FFFFFFFll - 1024) return m > n ? -1 : -2;
+    if (m == 0 || n == 0) return 0;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    DeviceState *dev = nullptr;
+    int rc = ensure_device(&dev);
+    if (rc) return rc;
+    const dim3 gc((unsigned)((m + 255) / 256), (unsigned)n);
+    const bool have_c = k > 0 && !(alpha_re == (R)0 && alpha_im == (R)0);
+    if (!have_c) {
+        k_zcombine<R><<<gc, 256, 0, st>>>(m, n, alpha_re, alpha_im, nullptr, 0, beta_re, beta_im, reinterpret_cast<R2 *>(C), ldc);
+        oz2_count_launches(1);
+        OZ2_CUDA_TRY(cudaGetLastError());
+        return 0;
+    }
+    const size_t real_ws = align_up(make_layout(2 * m, n, 2 * k, num_moduli, scaling_mode).total);
+    if (!dev->ws || dev->ws_bytes < complex_workspace_bytes(esz, m, n, k, num_moduli, scaling_mode)) return OZAKI2_ERR_WORKSPACE;
+    uint8_t *ws = static_cast<uint8_t *>(dev->ws);
+    R *At = reinterpret_cast<R *>(ws + real_ws);
+    R *Bt = reinterpret_cast<R *>(ws + real_ws + align_up(esz * (size_t)(2 * m) * (2 * k)));
+    R *Ct = reinterpret_cast<R *>(ws + real_ws + align_up(esz * (size_t)(2 * m) * (2 * k)) + align_up(esz * (size_t)(2 * k) * n));
+    k_zembed_a<R><<<dim3((unsigned)((m + 255) / 256), (unsigned)k), 256, 0, st>>>(m, k, reinterpret_cast<const R2 *>(A), lda, At);
+    k_zembed_b<R><<<dim3((unsigned)((k + 255) / 256), (unsigned)n), 256, 0, st>>>(k, n, reinterpret_cast<const R2 *>(B), ldb, Bt);
+    oz2_count_launches(2);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    rc = run_path(esz == 4 ? 1 : 0, 2 * m, n, 2 * k, 1.0, At, 2 * m, Bt, 2 * k, 0.0, Ct, 2 * m, num_moduli, scaling_mode, st, nullptr);
+    if (rc) return rc < 0 && rc > -100 ? -100 - rc : rc;      // an argument error of the embedded call would be a bug here
+    k_zcombine<R><<<gc, 256, 0, st>>>(m, n, alpha_re, alpha_im, Ct, 1, beta_re, beta_im, reinterpret_cast<R2 *>(C), ldc);
+    oz2_count_launches(1);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    return 0;
+}
+
 extern "C" {
 
 int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
@@ -812,57 +887,25 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
 
 size_t ozaki2_zgemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode)
 {
-    if (m < 0 || n < 0 || k < 0 || 2 * k > OZAKI2_MAX_K) return 0;
-    const size_t real_ws = ozaki2_workspace_bytes(2 * m, n, 2 * k, num_moduli, scaling_mode);
-    if (!real_ws && m && n && k) return 0;
-    return align_up(real_ws) + align_up(8 * (size_t)(2 * m) * (2 * k)) + align_up(8 * (size_t)(2 * k) * n) + align_up(8 * (size_t)(2 * m) * n);
+    return complex_workspace_bytes(8, m, n, k, num_moduli, scaling_mode);
+}
+size_t ozaki2_cgemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode)
+{
+    return complex_workspace_bytes(4, m, n, k, num_moduli, scaling_mode);
 }
 
 int ozaki2_zgemm(int64_t m, int64_t n, int64_t k, double alpha_re, double alpha_im, const double *A, int64_t lda,
                  const double *B, int64_t ldb, double beta_re, double beta_im, double *C, int64_t ldc, int num_moduli,
                  int scaling_mode, void *stream)
 {
-    if (m < 0) return -1;
-    if (n < 0) return -2;
-    if (k < 0 || 2 * k > OZAKI2_MAX_K || (scaling_mode == OZAKI2_MODE_ACCURATE && 2 * k > OZAKI2_MAX_K_ACCURATE)) return -3;
-    if (m > 0 && k > 0 && (!A || (reinterpret_cast<uintptr_t>(A) & 15))) return -6;
-    if (lda < (m > 1 ? m : 1)) return -7;
-    if (n > 0 && k > 0 && (!B || (reinterpret_cast<uintptr_t>(B) & 15))) return -8;
-    if (ldb < (k > 1 ? k : 1)) return -9;
-    if (m > 0 && n > 0 && (!C || (reinterpret_cast<uintptr_t>(C) & 15))) return -12;
-    if (ldc < (m > 1 ? m : 1)) return -13;
-    if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return -14;
-    if (scaling_mode < 0 || scaling_mode > 2) return -15;
-    if (m > (0x7FFFFFFFll - 1024) / 2 || n > 0x7FFFFFFFll - 1024) return m > n ? -1 : -2;
-    if (m == 0 || n == 0) return 0;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    DeviceState *dev = nullptr;
-    int rc = ensure_device(&dev);
-    if (rc) return rc;
-    const dim3 gc((unsigned)((m + 255) / 256), (unsigned)n);
-    const bool have_c = k > 0 && !(alpha_re == 0.0 && alpha_im == 0.0);
-    if (!have_c) {
-        k_zcombine<<<gc, 256, 0, st>>>(m, n, alpha_re, alpha_im, nullptr, 0, beta_re, beta_im, reinterpret_cast<double2 *>(C), ldc);
-        oz2_count_launches(1);
-        OZ2_CUDA_TRY(cudaGetLastError());
-        return 0;
-    }
-    const size_t real_ws = align_up(make_layout(2 * m, n, 2 * k, num_moduli, scaling_mode).total);
-    if (!dev->ws || dev->ws_bytes < ozaki2_zgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode)) return OZAKI2_ERR_WORKSPACE;
-    uint8_t *ws = static_cast<uint8_t *>(dev->ws);
-    double *At = reinterpret_cast<double *>(ws + real_ws);
-    double *Bt = reinterpret_cast<double *>(ws + real_ws + align_up(8 * (size_t)(2 * m) * (2 * k)));
-    double *Ct = reinterpret_cast<double *>(ws + real_ws + align_up(8 * (size_t)(2 * m) * (2 * k)) + align_up(8 * (size_t)(2 * k) * n));
-    k_zembed_a<<<dim3((unsigned)((m + 255) / 256), (unsigned)k), 256, 0, st>>>(m, k, reinterpret_cast<const double2 *>(A), lda, At);
-    k_zembed_b<<<dim3((unsigned)((k + 255) / 256), (unsigned)n), 256, 0, st>>>(k, n, reinterpret_cast<const double2 *>(B), ldb, Bt);
-    oz2_count_launches(2);
-    OZ2_CUDA_TRY(cudaGetLastError());
-    rc = run_path(0, 2 * m, n, 2 * k, 1.0, At, 2 * m, Bt, 2 * k, 0.0, Ct, 2 * m, num_moduli, scaling_mode, st, nullptr);
-    if (rc) return rc < 0 && rc > -100 ? -100 - rc : rc;      // an argument error of the embedded call would be a bug here
-    k_zcombine<<<gc, 256, 0, st>>>(m, n, alpha_re, alpha_im, Ct, 1, beta_re, beta_im, reinterpret_cast<double2 *>(C), ldc);
-    oz2_count_launches(1);
-    OZ2_CUDA_TRY(cudaGetLastError());
-    return 0;
+    return complex_entry<double>(m, n, k, alpha_re, alpha_im, A, lda, B, ldb, beta_re, beta_im, C, ldc, num_moduli, scaling_mode, stream);
+}
+
+int ozaki2_cgemm(int64_t m, int64_t n, int64_t k, float alpha_re, float alpha_im, const float *A, int64_t lda,
+                 const float *B, int64_t ldb, float beta_re, float beta_im, float *C, int64_t ldc, int num_moduli,
+                 int scaling_mode, void *stream)
+{
+    return complex_entry<float>(m, n, k, alpha_re, alpha_im, A, lda, B, ldb, beta_re, beta_im, C, ldc, num_moduli, scaling_mode, stream);
 }
 
 int ozaki2_debug_crt(int num_moduli, int64_t m, int64_t n, const uint8_t *U, const int32_t *e, const int32_t *f, double alpha,

@@ -222,3 +222,55 @@ def test_zgemm_quick_returns_and_errors(B):
     assert B.ozaki2_zgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, 21, 2) == -14
     assert B.ozaki2_set_workspace(None, 0) == 0
     assert B.ozaki2_zgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == B.OZAKI2_ERR_WORKSPACE
+
+
+@pytest.mark.parametrize("m,n,k,N,mode,alpha,beta", [
+    (70, 50, 90, 8, 2, 1.0, 0.0), (129, 33, 257, 12, 2, 0.5 - 2.0j, -1.25 + 0.75j), (64, 64, 64, 6, 1, 1.0, 1.0),
+    (40, 130, 300, 10, 0, -1.0j, 0.0), (1, 1, 1, 2, 2, 1.0, 0.0), (200, 20, 1000, 9, 2, 2.0, 0.5j),
+])
+def test_cgemm_against_the_oracle_on_the_real_embedding(B, m, n, k, N, mode, alpha, beta):
+    # the single-precision complex variant: bit-exact against oz2o_sgemm on the embedding of the FP32 parts + the FP32 tail
+    import torch
+    A, Bm = _complex_inputs(m, n, k, 1.0, 900 + m + n + k)
+    A, Bm = np.asfortranarray(A.astype(np.complex64)), np.asfortranarray(Bm.astype(np.complex64))
+    lda, ldb, ldc = m + 3, k + 1, m + 2
+    Ap = np.zeros((lda, k), np.complex64, order="F"); Ap[:m] = A
+    Bp = np.zeros((ldb, n), np.complex64, order="F"); Bp[:k] = Bm
+    rng = np.random.Generator(np.random.PCG64(19))
+    Cin = np.asfortranarray((rng.standard_normal((ldc, n)) + 1j * rng.standard_normal((ldc, n))).astype(np.complex64))
+    Ad = torch.from_numpy(np.ascontiguousarray(Ap.T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray(Bp.T)).cuda()
+    Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+    B.ensure_zgemm_workspace(m, n, k, N, mode)
+    assert B.ozaki2_cgemm_workspace_bytes(m, n, k, N, mode) <= B.ozaki2_zgemm_workspace_bytes(m, n, k, N, mode)
+    assert B.ozaki2_cgemm(m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == 0
+    torch.cuda.synchronize()
+    got = np.asfortranarray(Cd.cpu().numpy().T)
+    want = O.cgemm(A, Bm, N, mode, alpha=alpha, beta=beta, C_in=Cin[:m])
+    assert got.dtype == np.complex64 and np.array_equal(got[:m], want)
+    assert np.array_equal(got[m:], Cin[m:])
+    if mode != 1 and N >= 9:
+        ref = A.astype(np.complex128) @ Bm.astype(np.complex128)
+        assert np.max(np.abs(O.cgemm(A, Bm, N, mode) - ref) / np.abs(ref)) < 1e-3
+
+
+def test_cgemm_quick_returns_and_errors(B):
+    import torch
+    m, n, k, N = 32, 16, 24, 8
+    A, Bm = _complex_inputs(m, n, k, 0.5, 5)
+    Ad = torch.from_numpy(np.ascontiguousarray(A.astype(np.complex64).T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray(Bm.astype(np.complex64).T)).cuda()
+    Cin = np.asfortranarray((np.arange(m * n).reshape(m, n) * (1.0 + 0.5j)).astype(np.complex64))
+    Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+    B.ensure_zgemm_workspace(m, n, k, N, 2)
+    assert B.ozaki2_cgemm(m, n, k, 0.0, Ad, m, Bd, k, 2.0j, Cd, m, N, 2) == 0        # alpha == 0: C := beta C
+    torch.cuda.synchronize()
+    assert np.array_equal(np.asfortranarray(Cd.cpu().numpy().T), (np.complex64(2.0j) * Cin).astype(np.complex64))
+    assert B.ozaki2_cgemm(m, n, 0, 1.0, Ad, m, Bd, 1, 0.0, Cd, m, N, 2) == 0          # k == 0, beta == 0: zeros
+    torch.cuda.synchronize()
+    assert not np.any(Cd.cpu().numpy())
+    assert B.ozaki2_cgemm(m, -1, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == -2
+    assert B.ozaki2_cgemm(m, n, k, 1.0, Ad, m, Bd, k - 1, 0.0, Cd, m, N, 2) == -9
+    assert B.ozaki2_cgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 5) == -15
+    assert B.ozaki2_set_workspace(None, 0) == 0
+    assert B.ozaki2_cgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == B.OZAKI2_ERR_WORKSPACE

@@ -76,3 +76,59 @@ def test_error_against_numpy_complex_product_and_alpha_beta():
     tr = alpha.real * C.real - alpha.imag * C.imag + (beta.real * Cin.real - beta.imag * Cin.imag)
     ti = alpha.real * C.imag + alpha.imag * C.real + (beta.real * Cin.imag + beta.imag * Cin.real)
     assert np.array_equal(out.real, tr) and np.array_equal(out.imag, ti)
+
+
+# ---- single-precision complex variant (cgemm): the same reading on FP32 parts -------------------------------------------
+def complex64_inputs(m, n, k, phi, seed):
+    A, B = complex_inputs(m, n, k, phi, seed)
+    return A.astype(np.complex64), B.astype(np.complex64)
+
+
+@pytest.mark.parametrize("mode", [ACCU, FAST, PROP])
+def test_cgemm_gaussian_integer_matrices_exact(mode):
+    rng = np.random.Generator(np.random.PCG64(15))
+    A = (rng.integers(-8, 9, (10, 20)) + 1j * rng.integers(-8, 9, (10, 20))).astype(np.complex64)
+    B = (rng.integers(-8, 9, (20, 7)) + 1j * rng.integers(-8, 9, (20, 7))).astype(np.complex64)
+    want = A.astype(np.complex128) @ B.astype(np.complex128)          # |entries| < 2^24: exact in FP32 as well
+    assert np.array_equal(O.cgemm(A, B, 8, mode).astype(np.complex128), want)
+
+
+@pytest.mark.parametrize("mode", [FAST, PROP])
+def test_cgemm_real_inputs_reduce_to_sgemm_bit_for_bit(mode):
+    A, B = W.eq15_matrices(18, 12, 50, 1.0, 9)
+    A, B = A.astype(np.float32), B.astype(np.float32)
+    C = O.cgemm(A.astype(np.complex64), B.astype(np.complex64), 9, mode)
+    assert np.array_equal(C.real, O.sgemm(A, B, 9, mode)) and not np.any(C.imag)
+
+
+def test_cgemm_is_the_single_rounding_of_zgemm_on_the_same_inputs():
+    # both run Steps 1-3 on the same (exactly promoted) embedding, so C'' is the same integer: cgemm's parts are RN_32 of it,
+    # zgemm's are RN_64 of it.  With enough moduli that the integer carries more than 53 significant bits nothing can be said
+    # in general (double rounding), but RN_32(x) and RN_32(RN_64(x)) differ only on a 2^-29 sliver: compare within 1 ulp32
+    # everywhere and bit for bit on all but a handful of entries
+    A, B = complex64_inputs(20, 16, 96, 0.5, 40)
+    c32 = O.cgemm(A, B, 10, PROP)
+    c64 = O.zgemm(A.astype(np.complex128), B.astype(np.complex128), 10, PROP)
+    for got, ref in ((c32.real, c64.real), (c32.imag, c64.imag)):
+        r32 = ref.astype(np.float32)
+        assert np.all(np.abs(got.astype(np.float64) - ref) <= np.spacing(np.abs(r32)).astype(np.float64))
+        assert np.mean(got == r32) > 0.99
+
+
+def test_cgemm_error_scale_invariance_and_tail_order():
+    A, B = complex64_inputs(24, 18, 128, 0.5, 31)
+    ref = A.astype(np.complex128) @ B.astype(np.complex128)
+    C = O.cgemm(A, B, 10, PROP)
+    assert np.max(np.abs(C - ref) / np.abs(ref)) < 1e-5
+    C2 = O.cgemm(A * np.float32(2.0 ** 20), B * np.complex64(2.0 ** -30 * 1j), 10, PROP)
+    assert np.array_equal(C2, C * np.complex64(2.0 ** -10 * 1j))
+    alpha, beta = 0.5 - 2.0j, -1.25 + 0.75j
+    rng = np.random.Generator(np.random.PCG64(4))
+    Cin = (rng.standard_normal((24, 18)) + 1j * rng.standard_normal((24, 18))).astype(np.complex64)
+    out = O.cgemm(A, B, 10, PROP, alpha=alpha, beta=beta, C_in=Cin)
+    f = np.float32
+    ar, ai, br, bi = f(alpha.real), f(alpha.imag), f(beta.real), f(beta.imag)
+    tr = (ar * C.real - ai * C.imag) + (br * Cin.real - bi * Cin.imag)        # float32 arrays: every operation rounds to FP32
+    ti = (ar * C.imag + ai * C.real) + (br * Cin.imag + bi * Cin.real)
+    assert out.dtype == np.complex64 and tr.dtype == np.float32
+    assert np.array_equal(out.real, tr) and np.array_equal(out.imag, ti)
