@@ -148,6 +148,20 @@ size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, i
 int ozaki2_set_workspace(void *device_ptr, size_t bytes);
 
 /*
+ * ozaki2_dgemm / ozaki2_sgemm with the workspace of THIS call passed in (device pointer, 256-byte aligned, at least
+ * ozaki2_workspace_bytes(m, n, k, num_moduli, scaling_mode) bytes; it must stay valid until the call's work on `stream`
+ * has finished): calls that use different workspaces are independent and may run concurrently on different streams or from
+ * different host threads.  The registered workspace of the device is not touched.  A missing, misaligned or too small
+ * workspace returns -14 (its argument number).  Everything else as ozaki2_dgemm / ozaki2_sgemm.
+ */
+int ozaki2_dgemm_ws(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
+                    int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode,
+                    void *workspace, size_t workspace_bytes, void *stream);
+int ozaki2_sgemm_ws(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda, const float *B,
+                    int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode,
+                    void *workspace, size_t workspace_bytes, void *stream);
+
+/*
  * The same call with HOST buffers: copies A and B to the device, runs ozaki2_dgemm, copies C
  * back (and C in first if beta != 0), then synchronises `stream`.  For the two fast modes and
  * n >= 512 the work is cut into column panels of B / C: the kernels stay on `stream`, the copies

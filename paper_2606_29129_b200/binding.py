@@ -51,6 +51,10 @@ def lib() -> C.CDLL:
         L.ozaki2_dgemm_t.restype = ci
         sgemm_args = [i64, i64, i64, C.c_float, vp, i64, vp, i64, C.c_float, vp, i64, ci, ci, vp]
         L.ozaki2_sgemm.argtypes = sgemm_args
+        L.ozaki2_dgemm_ws.argtypes = gemm_args[:-1] + [vp, C.c_size_t, vp]
+        L.ozaki2_dgemm_ws.restype = ci
+        L.ozaki2_sgemm_ws.argtypes = sgemm_args[:-1] + [vp, C.c_size_t, vp]
+        L.ozaki2_sgemm_ws.restype = ci
         L.ozaki2_sgemm.restype = ci
         L.ozaki2_sgemm_stages.argtypes = sgemm_args + [C.POINTER(ozaki2_stage_outputs)]
         L.ozaki2_sgemm_stages.restype = ci
@@ -147,6 +151,19 @@ def ozaki2_dgemm(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scal
     """Raw call: returns the library's status (0 = success).  A, B, Cm: device tensors or addresses."""
     return int(lib().ozaki2_dgemm(m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc, num_moduli,
                                   scaling_mode, _stream(stream)))
+
+
+def ozaki2_dgemm_ws(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, workspace, workspace_bytes,
+                    stream=None) -> int:
+    """ozaki2_dgemm with the workspace of this call passed in (device tensor or address): independent of other calls."""
+    return int(lib().ozaki2_dgemm_ws(m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc, num_moduli, scaling_mode,
+                                     _ptr(workspace), workspace_bytes, _stream(stream)))
+
+
+def ozaki2_sgemm_ws(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, workspace, workspace_bytes,
+                    stream=None) -> int:
+    return int(lib().ozaki2_sgemm_ws(m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(Cm), ldc, num_moduli, scaling_mode,
+                                     _ptr(workspace), workspace_bytes, _stream(stream)))
 
 
 def ozaki2_dgemm_stages(m, n, k, alpha, A, lda, B, ldb, beta, Cm, ldc, num_moduli, scaling_mode, stream=None,

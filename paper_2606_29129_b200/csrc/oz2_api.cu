@@ -359,7 +359,8 @@ __global__ void k_zcombine(int64_t m, int64_t n, R ar, R ai, const R *__restrict
 // B, i.e. the two movers / reductions simply swap sides.
 static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda, const void *B,
                     int64_t ldb, double beta, void *C, int64_t ldc, int N, int mode, cudaStream_t st,
-                    const ozaki2_stage_outputs *out, int transa = 0, int transb = 0)
+                    const ozaki2_stage_outputs *out, int transa = 0, int transb = 0, void *call_ws = nullptr, size_t call_ws_bytes = 0,
+                    bool use_call_ws = false)
 {
     int rc = check_args(m, n, k, A, lda, B, ldb, C, ldc, N, mode, transa, transb);
     const int strided_a = transa ? 0 : 1, strided_b = transb ? 1 : 0;
@@ -379,8 +380,11 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
         return 0;
     }
     const Layout L = make_layout(m, n, k, N, mode);
-    if (!dev->ws || dev->ws_bytes < L.total) return OZAKI2_ERR_WORKSPACE;
-    uint8_t *ws = static_cast<uint8_t *>(dev->ws);
+    // the workspace of this call: the caller's own (ozaki2_*gemm_ws) or the one registered for the device
+    void *ws_ptr = use_call_ws ? call_ws : dev->ws;
+    const size_t ws_have = use_call_ws ? call_ws_bytes : dev->ws_bytes;
+    if (!ws_ptr || ws_have < L.total || (reinterpret_cast<uintptr_t>(ws_ptr) & 255)) return OZAKI2_ERR_WORKSPACE;
+    uint8_t *ws = static_cast<uint8_t *>(ws_ptr);
     int32_t *e = reinterpret_cast<int32_t *>(ws + L.off_e), *f = reinterpret_cast<int32_t *>(ws + L.off_f);
     unsigned long long *amax = reinterpret_cast<unsigned long long *>(ws + L.off_amax);
     unsigned long long *ssq = reinterpret_cast<unsigned long long *>(ws + L.off_ssq);
@@ -693,6 +697,24 @@ int ozaki2_dgemm(int64_t m, int64_t n, int64_t k, double alpha, const double *A,
 {
     return run_path(0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
                     static_cast<cudaStream_t>(stream), nullptr);
+}
+
+int ozaki2_dgemm_ws(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,
+                    int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli, int scaling_mode, void *workspace,
+                    size_t workspace_bytes, void *stream)
+{
+    const int rc = run_path(0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, num_moduli, scaling_mode,
+                            static_cast<cudaStream_t>(stream), nullptr, 0, 0, workspace, workspace_bytes, true);
+    return rc == OZAKI2_ERR_WORKSPACE ? -14 : rc;          // here the workspace is the 14th argument
+}
+
+int ozaki2_sgemm_ws(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda, const float *B,
+                    int64_t ldb, float beta, float *C, int64_t ldc, int num_moduli, int scaling_mode, void *workspace,
+                    size_t workspace_bytes, void *stream)
+{
+    const int rc = run_path(1, m, n, k, (double)alpha, A, lda, B, ldb, (double)beta, C, ldc, num_moduli, scaling_mode,
+                            static_cast<cudaStream_t>(stream), nullptr, 0, 0, workspace, workspace_bytes, true);
+    return rc == OZAKI2_ERR_WORKSPACE ? -14 : rc;
 }
 
 int ozaki2_dgemm_stages(int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda, const double *B,

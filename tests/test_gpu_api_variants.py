@@ -274,3 +274,42 @@ def test_cgemm_quick_returns_and_errors(B):
     assert B.ozaki2_cgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 5) == -15
     assert B.ozaki2_set_workspace(None, 0) == 0
     assert B.ozaki2_cgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, 2) == B.OZAKI2_ERR_WORKSPACE
+
+
+def test_per_call_workspaces_on_concurrent_streams(B):
+    # ozaki2_dgemm_ws / ozaki2_sgemm_ws: each call brings its own workspace, so calls on different streams are independent
+    # (no registered workspace is needed or touched); several rounds enqueued without any synchronisation in between
+    import torch
+    assert B.ozaki2_set_workspace(None, 0) == 0
+    probs = [(200, 136, 520, 14, 2, False), (129, 257, 1000, 17, 1, False), (96, 80, 300, 8, 2, True), (260, 40, 2049, 16, 0, False)]
+    streams = [torch.cuda.Stream() for _ in probs]
+    state = []
+    for (m, n, k, N, mode, f32), st in zip(probs, streams):
+        A, Bm = W.eq15_matrices(m, n, k, 1.0, 4000 + m + k)
+        dt = np.float32 if f32 else np.float64
+        A, Bm = np.asfortranarray(A.astype(dt)), np.asfortranarray(Bm.astype(dt))
+        Ad = torch.from_numpy(np.ascontiguousarray(A.T)).cuda()
+        Bd = torch.from_numpy(np.ascontiguousarray(Bm.T)).cuda()
+        Cd = torch.full((n, m), float("nan"), dtype=Ad.dtype, device="cuda")
+        nbytes = B.ozaki2_workspace_bytes(m, n, k, N, mode)
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        off = (-ws.data_ptr()) % 256
+        state.append((A, Bm, Ad, Bd, Cd, ws, ws.data_ptr() + off, nbytes))
+    torch.cuda.synchronize()
+    for _ in range(3):
+        for (m, n, k, N, mode, f32), st, (A, Bm, Ad, Bd, Cd, ws, wp, nbytes) in zip(probs, streams, state):
+            fn = B.ozaki2_sgemm_ws if f32 else B.ozaki2_dgemm_ws
+            assert fn(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, wp, nbytes, stream=st.cuda_stream) == 0
+    torch.cuda.synchronize()
+    for (m, n, k, N, mode, f32), (A, Bm, Ad, Bd, Cd, ws, wp, nbytes) in zip(probs, state):
+        want = (O.sgemm if f32 else O.dgemm)(A, Bm, N, mode)
+        assert np.array_equal(Cd.cpu().numpy().T, want), (m, n, k, N, mode, f32)
+    # argument checks of the workspace itself: missing, too small, misaligned
+    m, n, k, N, mode, _ = probs[0]
+    A, Bm, Ad, Bd, Cd, ws, wp, nbytes = state[0]
+    assert B.ozaki2_dgemm_ws(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, None, nbytes) == -14
+    assert B.ozaki2_dgemm_ws(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, wp, nbytes - 1) == -14
+    assert B.ozaki2_dgemm_ws(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, wp + 8, nbytes) == -14
+    assert B.ozaki2_dgemm_ws(m, n, k, 1.0, Ad, m - 1, Bd, k, 0.0, Cd, m, N, mode, wp, nbytes) == -6
+    # the plain entry still reports the unregistered device workspace in its own way
+    assert B.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode) == B.OZAKI2_ERR_WORKSPACE
