@@ -173,6 +173,17 @@ def profiled_traffic(args, m, n, k, N, mode, f32):
     return None
 
 
+def traffic_capture_commit():
+    """The commit the ncu capture behind TRAFFIC_CSV was taken at, as the .md beside it states it."""
+    import re
+    try:
+        with open(os.path.join(ROOT, TRAFFIC_CSV[:-4] + ".md")) as fh:
+            mt = re.search(r"commit `([0-9a-f]{7,40})`", fh.read())
+        return mt.group(1) if mt else "unknown"
+    except OSError:
+        return "unknown"
+
+
 def cpu_slab_shape(m, n, k):
     """Bounded sample of the workload for the oracle: about 1.4e11 residue MACs at N = 16, i.e. 512 rows of A against
     4096 columns of B at k = 8192 (about 7 s on the GPU box's 16 host threads), fewer columns at longer k."""
@@ -386,7 +397,7 @@ def main():
                     int8_ceiling_tops=ceiling,
                     frac_of_ceiling_random=(achieved / ceiling["random"]["tops"]) if ceiling else None,
                     traffic=profiled_traffic(args, m, n, k, N, mode, f32),
-                    traffic_unit=f"bytes per launch (ncu dram read + write, {TRAFFIC_CSV})",
+                    traffic_unit=f"bytes per launch (ncu dram read + write, {TRAFFIC_CSV}, captured at commit {traffic_capture_commit()})",
                     algorithmic_bytes=N * X + N * Y)
     if roofline["frac"] > 1.0:
         roofline["note"] = "frac > 1: the kernel beats 2 x the cuBLAS bf16 burst figure; see int8_ceiling_tops"
