@@ -351,3 +351,39 @@ def test_int32_accumulator_wraps_at_k_2pow17(B):
         got = Ud.cpu().numpy()
         assert np.array_equal(got[:, :8, :8], want)
         assert np.all(got[1] == (127 * 127 * k) % 255)
+
+
+@pytest.mark.parametrize("m,n,k,N,mode,phi", [
+    (1500, 1301, 2101, 16, 2, 1.0),      # several waves of ragged tiles in every persistent kernel, k tail of 53
+    (1031, 1540, 1667, 18, 0, 2.0),      # wide conversion format (N >= 17), five words of P, accurate mode's auxiliary product
+    (2050, 515, 3073, 15, 1, 0.5),       # one row / column past a tile boundary, k = 24 x 128 + 1
+])
+def test_midsize_ragged_shapes_all_stages(B, m, n, k, N, mode, phi):
+    # between the small ragged cases above (at most a wave of tiles) and the sampled full-size tests (tile-aligned shapes):
+    # every stage compared in full on shapes whose persistent loops run many items with ragged edges in m, n and k
+    A, Bm = W.eq15_matrices(m, n, k, phi, 5000 + m + n + k)
+    o = O.stages(A, Bm, N, mode)
+    g = gpu_stages(B, A, Bm, N, mode)
+    assert_stage_parity(g, o, mode, f"{m}x{n}x{k} N{N} mode{mode}")
+    # and the plain call (product kernels: crt_fast + hand-over instead of crt_exact for every element)
+    import torch
+    Cd = B.dgemm(B.colmajor_to_device(A), B.colmajor_to_device(Bm), N, mode)
+    torch.cuda.synchronize()
+    assert np.array_equal(B.device_to_colmajor(Cd), o["C"])
+
+
+def test_random_shapes_fuzz(B):
+    # 40 seeded random problems: shapes 1 .. 400 (k up to 3000), every N and mode, eq. (15) data with phi in [0, 4] and a
+    # random power-of-two scale on each operand; all stages bit-exact
+    rng = np.random.Generator(np.random.PCG64(20261105))
+    for t in range(40):
+        m, n = int(rng.integers(1, 401)), int(rng.integers(1, 401))
+        k = int(rng.integers(1, 3001)) if t % 4 else int(rng.integers(1, 40))
+        N, mode = int(rng.integers(2, 21)), int(rng.integers(0, 3))
+        phi = float(rng.uniform(0.0, 4.0))
+        sa, sb = int(rng.integers(-300, 301)), int(rng.integers(-300, 301))
+        A, Bm = W.eq15_matrices(m, n, k, phi, 77000 + t)
+        A, Bm = np.ldexp(A, sa), np.ldexp(Bm, sb)
+        o = O.stages(A, Bm, N, mode)
+        g = gpu_stages(B, A, Bm, N, mode)
+        assert_stage_parity(g, o, mode, f"fuzz {t}: {m}x{n}x{k} N{N} mode{mode} phi{phi:.2f} 2^{sa} 2^{sb}")
