@@ -606,7 +606,7 @@ k2_tc_rows(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
 // ---------------------------------------------------------------------------------------------
 // accurate mode: Abar / Bbar = ceil(|a| 2^(5-E)) in [0, 64], one INT8 plane, CUDA cores only
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t ceil_scaled(double a, int E)
+__device__ __noinline__ uint32_t ceil_scaled(double a, int E)
 {
     const unsigned long long b = (unsigned long long)__double_as_longlong(a) & 0x7FFFFFFFFFFFFFFFull;
     if (b == 0) return 0u;
@@ -623,8 +623,17 @@ __device__ __forceinline__ uint32_t ceil_scaled(double a, int E)
 __device__ __forceinline__ void quad_bar(const double (&a)[4], int E, int8_t *dst)
 {
     uint32_t o = 0;
+    const int g = E < -4096 ? 4096 : 5 - E;           // the all-zero marker takes the integer route (which returns zeros)
+    if (g >= -1022 && g <= 1023) {
+        // |a| 2^g is an exact FP64 multiply while it stays normal; if it underflows, rounding up keeps it in (0, 1) and the
+        // ceiling is 1 as it must be; 0 stays 0.  (E of an all-zero vector is a marker far outside this range.)
+        const double scale = __hiloint2double((g + 1023) << 20, 0);
 #pragma unroll
-    for (int u = 0; u < 4; u++) o |= ceil_scaled(a[u], E) << (8 * u);
+        for (int u = 0; u < 4; u++) o |= (uint32_t)__double2int_ru(__dmul_ru(fabs(a[u]), scale)) << (8 * u);
+    } else {
+#pragma unroll
+        for (int u = 0; u < 4; u++) o |= ceil_scaled(a[u], E) << (8 * u);
+    }
     *reinterpret_cast<uint32_t *>(dst) = o;
 }
 
