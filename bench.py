@@ -173,6 +173,44 @@ def profiled_traffic(args, m, n, k, N, mode, f32):
     return None
 
 
+NCU_SUMMARY_MD = os.path.join("profiles", "r02_ncu_summary.md")
+
+
+def profiled_issue_bounds(args, m, n, k, N, mode, f32, sm_count=148, sm_mhz=1965.0):
+    """Plain-ALU (instruction issue) bound of the streaming stages: warp instructions per launch from the
+    committed `ncu --set full` summary / (SMs x 4 schedulers x max SM clock), in ms per stage; only for the workload of
+    that capture (8192^3, N = 16, mode 2, FP64).  DESIGN.md section 6 derives the peak: one warp instruction per scheduler
+    and cycle, 4 schedulers per SM."""
+    import re
+    path = os.path.join(ROOT, NCU_SUMMARY_MD)
+    if not (os.path.exists(path) and (m, n, k) == (8192, 8192, 8192) and N == 16 and mode == 2 and not f32):
+        return None
+    insts = {}
+    with open(path) as fh:
+        lines = fh.read().splitlines()
+    hdr = next((ln for ln in lines if ln.startswith("| kernel |")), None)
+    if hdr is None:
+        return None
+    cols = [c.strip() for c in hdr.strip("|").split("|")]
+    if "warp insts" not in cols:
+        return None
+    iw = cols.index("warp insts")
+    for ln in lines:
+        mt = re.match(r"\| `(k\d_\w+)", ln)
+        if mt:
+            cells = [c.strip() for c in ln.strip("|").split("|")]
+            insts[mt.group(1)] = insts.get(mt.group(1), 0.0) + float(cells[iw])
+    rate = sm_count * 4 * sm_mhz * 1e6                      # warp instructions per second, whole chip
+    groups = {"S1_scaling": ("k1_rows", "k1_rows_finalize", "k1_cols"), "S2_conversion": ("k2_tc_rows", "k2_tc_cols"),
+              "S4S5_crt_unscale": ("k5_crt_tc",)}
+    out = {}
+    for st, ks in groups.items():
+        w = sum(insts.get(kk, 0.0) for kk in ks)
+        if w:
+            out[st] = dict(warp_instructions=w, issue_bound_ms=w / rate * 1e3)
+    return out or None
+
+
 def traffic_capture_commit():
     """The commit the ncu capture behind TRAFFIC_CSV was taken at, as the .md beside it states it."""
     import re
@@ -407,6 +445,12 @@ def main():
         stages[nm] = dict(ms=ms_, algorithmic_gb=by / 1e9, gbs=by / (ms_ * 1e-3) / 1e9,
                           hbm_frac=by / (ms_ * 1e-3) / 1e9 / peaks["hbm_gbs"])
     stages["S3_residue_gemm"]["int8_tops"] = achieved
+    alu = profiled_issue_bounds(args, m, n, k, N, mode, f32)
+    if alu:
+        for nm, v in alu.items():                           # the plain-ALU bound next to the HBM one
+            stages[nm].update(alu_bound_ms=v["issue_bound_ms"], alu_warp_instructions=v["warp_instructions"],
+                              hbm_bound_ms=stages[nm]["algorithmic_gb"] / peaks["hbm_gbs"] * 1e3,
+                              alu_bound_source=f"{NCU_SUMMARY_MD}: warp instructions / (148 SMs x 4 schedulers x 1965 MHz)")
     total_bytes = (2 * esz + 2 * N) * X + (2 * N + esz) * Y
     t_hbm_ms = total_bytes / (peaks["hbm_gbs"] * 1e9) * 1e3
     t_roof_ms = max(s3_ops / (int8_peak * 1e12) * 1e3, t_hbm_ms)
