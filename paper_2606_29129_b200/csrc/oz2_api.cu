@@ -13,6 +13,11 @@
 #include <vector>
 
 static std::atomic<uint64_t> g_launches{0};
+bool oz2_pdl_enabled()
+{
+    static const bool on = [] { const char *e = getenv("OZAKI2_PDL"); return !(e && e[0] == '0'); }();
+    return on;
+}
 void oz2_count_launches(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
 
 namespace {

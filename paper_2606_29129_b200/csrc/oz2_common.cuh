@@ -83,6 +83,33 @@ int oz2_launch_crt(int N, int f32, int64_t m, int64_t n, const uint8_t *U, int64
 // kernel-launch accounting behind ozaki2_kernel_launches()
 void oz2_count_launches(int n);
 
+// Programmatic dependent launch (PDL): every kernel of the path is launched with the programmatic-stream-serialization
+// attribute, signals at its entry that its dependents may be scheduled (pdl_launch_dependents) and waits for its predecessor
+// to complete and flush (pdl_wait) before it touches anything the predecessor wrote -- and in any case before it exits,
+// which keeps the dependency transitive along the chain.  What runs before the wait (barrier initialisation, tensor-memory
+// allocation, constant operand images) overlaps the predecessor's tail; at small sizes that is a good part of the call.
+// OZAKI2_PDL=0 in the environment (read once) launches everything the plain way.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+bool oz2_pdl_enabled();
+template <typename... KArgs, typename... Args>
+static inline cudaError_t oz2_launch(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = oz2_pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif
+
 #define OZ2_CUDA_TRY(expr)                                   \
     do {                                                     \
         cudaError_t _e = (expr);                             \

@@ -476,7 +476,9 @@ k2_tc_cols(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
     extern __shared__ uint8_t smem_raw[];
     ConvSmem<WIDE> *S = conv_smem<WIDE>(smem_raw);
     ConvCtx cx;
+    pdl_launch_dependents();
     conv_setup<WIDE>(S, cx, N);
+    pdl_wait();                                      // the exponents come from the scaling kernels
     const int tid = threadIdx.x;
     const int chunks = (int)((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);      // k <= 2^22: fits 32 bits
     const int64_t items = rows * chunks;
@@ -542,7 +544,9 @@ k2_tc_rows(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
     constexpr int PITCH = StageRow<T>::PITCH;
     T *stage = reinterpret_cast<T *>(S + 1);
     ConvCtx cx;
+    pdl_launch_dependents();
     conv_setup<WIDE>(S, cx, N);
+    pdl_wait();                                      // the exponents come from the scaling kernels
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nib = (int)((rows + ST_ROWS - 1) / ST_ROWS), nhb = (int)(kp / ST_H);
     const int64_t items = (int64_t)nib * nhb;
@@ -645,6 +649,8 @@ k2_bar_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, const in
             int64_t kp)
 {
     __shared__ __align__(16) double tile[BAR_TI * BAR_SROW];
+    pdl_launch_dependents();
+    pdl_wait();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t i0 = (int64_t)blockIdx.x * BAR_TI, h0 = (int64_t)blockIdx.y * BAR_TH;
     {
@@ -678,6 +684,8 @@ __global__ void __launch_bounds__(BAR_THREADS)
 k2_bar_cols(int64_t n, int64_t k, const T *__restrict__ B, int64_t ldb, const int32_t *__restrict__ E, int8_t *__restrict__ plane,
             int64_t kp)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     const int64_t quads = kp / 4;
     const int64_t t = (int64_t)blockIdx.x * BAR_THREADS + threadIdx.x;
     if (t >= n * quads) return;
@@ -722,14 +730,14 @@ int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *
             const int64_t items = ((rows + ST_ROWS - 1) / ST_ROWS) * (kp / ST_H);
             int64_t grid = (int64_t)num_sms() * per_sm;
             if (grid > items) grid = items;
-            if (wide) k2_tc_rows<1, T><<<(unsigned)grid, CV_THREADS, rows_smem<1, T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
-            else k2_tc_rows<0, T><<<(unsigned)grid, CV_THREADS, rows_smem<0, T>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            if (wide) OZ2_CUDA_TRY(oz2_launch(k2_tc_rows<1, T>, dim3((unsigned)grid), dim3(CV_THREADS), rows_smem<1, T>(), st, N, rows, k, X, ldx, ex, planes, kp));
+            else OZ2_CUDA_TRY(oz2_launch(k2_tc_rows<0, T>, dim3((unsigned)grid), dim3(CV_THREADS), rows_smem<0, T>(), st, N, rows, k, X, ldx, ex, planes, kp));
         } else {
             const int64_t items = rows * ((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);
             int64_t grid = (int64_t)num_sms() * per_sm;
             if (grid > items) grid = items;
-            if (wide) k2_tc_cols<1, T><<<(unsigned)grid, CV_THREADS, cols_smem<1>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
-            else k2_tc_cols<0, T><<<(unsigned)grid, CV_THREADS, cols_smem<0>(), st>>>(N, rows, k, X, ldx, ex, planes, kp);
+            if (wide) OZ2_CUDA_TRY(oz2_launch(k2_tc_cols<1, T>, dim3((unsigned)grid), dim3(CV_THREADS), cols_smem<1>(), st, N, rows, k, X, ldx, ex, planes, kp));
+            else OZ2_CUDA_TRY(oz2_launch(k2_tc_cols<0, T>, dim3((unsigned)grid), dim3(CV_THREADS), cols_smem<0>(), st, N, rows, k, X, ldx, ex, planes, kp));
         }
     }
     oz2_count_launches(1);

@@ -455,6 +455,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     uint8_t *gen0 = smem_raw + (smem0 - smem_u32(smem_raw));                // generic pointer to the aligned base
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_launch_dependents();
     // The grid is nib x gj CTAs: CTA b owns row block ib = ib0 + b % nib (512 rows: its exponents e_i stay in registers) and
     // walks the columns j = b / nib, + gj, + 2 gj, ...
     const int gj = (int)gridDim.x / nib;
@@ -485,6 +486,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     tc_fence_after();
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+    pdl_wait();                                   // the residue products come from the GEMM
 
     if (warp == 0) {
         if (lane == 0) {
@@ -598,8 +600,8 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
             const int64_t nib = tiles_i - ib0 < gmax ? tiles_i - ib0 : gmax;
             int64_t gj = gmax / nib;
             if (gj > n) gj = n;
-            kern<<<(unsigned)(nib * gj), K5_THREADS, K5_SMEM, st>>>(map, N, mi, ni, e, f, alpha, beta, C, ldi, cpp, U, mpi, h_k5[N], (int)ib0,
-                                                                  (int)nib);
+            OZ2_CUDA_TRY(oz2_launch(kern, dim3((unsigned)(nib * gj)), dim3(K5_THREADS), K5_SMEM, st, map, N, mi, ni, e, f, alpha, beta, C, ldi, cpp,
+                                    U, mpi, h_k5[N], (int)ib0, (int)nib));
             oz2_count_launches(1);
         }
         return 0;

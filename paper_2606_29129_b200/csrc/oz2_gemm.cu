@@ -215,6 +215,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tiles_m = (m + TILE_M - 1) / TILE_M, tiles_n = (n + TILE_N - 1) / TILE_N;
     const int64_t total = (int64_t)nplanes * tiles_m * tiles_n;
+    pdl_launch_dependents();
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; s++) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
@@ -231,6 +232,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    pdl_wait();                                   // the residue planes come from the conversion kernels
 
     if (warp == 0) {
         // ===================== TMA producer =====================
@@ -379,6 +381,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
     const int tiles_m = (m + P2_TILE_M - 1) / P2_TILE_M, tiles_n = (n + TILE_N - 1) / TILE_N;
     const int64_t total = (int64_t)nplanes * tiles_m * tiles_n;
     const int64_t cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+    pdl_launch_dependents();
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < P2_STAGES; s++) {
@@ -402,6 +405,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
     tc_fence_after();
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+    pdl_wait();                                   // the residue planes come from the conversion kernels
 
     if (warp == 0) {
         // ===================== TMA producer (both CTAs): own 128 rows of A, own half of the B tile =====================
@@ -555,14 +559,14 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
         if (tiles < clusters) clusters = tiles;
         const unsigned grid = (unsigned)(2 * clusters);
         if (rowmax)
-            k3_residue_gemm_pair<EPI_MAX><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
-                                                                         nullptr, mp, rowmax, colmax);
+            OZ2_CUDA_TRY(oz2_launch(k3_residue_gemm_pair<EPI_MAX>, dim3(grid), dim3(NUM_THREADS), P2_SMEM, st, mapA, mapB, nplanes, mod_base,
+                                    (int)m, (int)n, num_kb, (uint8_t *)nullptr, mp, rowmax, colmax));
         else if (variant == OZ2_GEMM_PAIR_MMA_ONLY)
             k3_residue_gemm_pair<EPI_NONE><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
                                                                           nullptr, mp, nullptr, nullptr);
         else
-            k3_residue_gemm_pair<EPI_MODP><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
-                                                                          U, mp, nullptr, nullptr);
+            OZ2_CUDA_TRY(oz2_launch(k3_residue_gemm_pair<EPI_MODP>, dim3(grid), dim3(NUM_THREADS), P2_SMEM, st, mapA, mapB, nplanes, mod_base,
+                                    (int)m, (int)n, num_kb, U, mp, (int32_t *)nullptr, (int32_t *)nullptr));
         oz2_count_launches(1);
         OZ2_CUDA_TRY(cudaGetLastError());
         return 0;

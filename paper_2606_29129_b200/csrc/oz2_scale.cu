@@ -148,6 +148,8 @@ __global__ void __launch_bounds__(ROWS_PER_BLOCK *KSLICES)
 k1_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, int64_t kchunk,
         unsigned long long *__restrict__ amax, unsigned long long *__restrict__ ssq, int SQ)
 {
+    pdl_launch_dependents();
+    pdl_wait();                                  // PASS 1 reads the maxima of PASS 0; every kernel of the chain waits (transitivity)
     int64_t i = (int64_t)blockIdx.x * ROWS_PER_BLOCK + threadIdx.x;
     int64_t h0 = (int64_t)blockIdx.y * kchunk;
     int64_t h1 = h0 + kchunk < k ? h0 + kchunk : k;
@@ -201,6 +203,8 @@ k1_rows(int64_t m, int64_t k, const T *__restrict__ A, int64_t lda, int64_t kchu
 __global__ void k1_rows_finalize(int mode, int N, int64_t m, const unsigned long long *__restrict__ amax,
                                  const unsigned long long *__restrict__ ssq, int32_t *__restrict__ e, int SQ)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < m) e[i] = exponent_fastprop(mode, c_crt[N], amax[i], ssq[i], SQ);
 }
@@ -239,6 +243,8 @@ k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_
         int32_t *__restrict__ EB, int SQ)
 {
     __shared__ unsigned long long sm[COL_THREADS / 32];
+    pdl_launch_dependents();
+    pdl_wait();
     const T *col = B + (int64_t)blockIdx.x * ldb;
     bool vec = ((((uintptr_t)col) & (2 * sizeof(T) - 1)) == 0);
     int64_t kv = vec ? (k & ~(int64_t)1) : 0;
@@ -287,6 +293,8 @@ k1_cols(int mode, int N, int64_t k, const T *__restrict__ B, int64_t ldb, int32_
 // ---------------------------------------------------------------------------------------------
 __global__ void k1_rows_E(int64_t m, const unsigned long long *__restrict__ amax, int32_t *__restrict__ EA)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < m) EA[i] = amax[i] ? floor_log2_bits(amax[i]) : OZ2_E_ZERO;
 }
@@ -294,6 +302,8 @@ __global__ void k1_rows_E(int64_t m, const unsigned long long *__restrict__ amax
 __global__ void k1_accu_finalize(int N, int64_t cnt, const int32_t *__restrict__ E, const int32_t *__restrict__ mx,
                                  int32_t *__restrict__ out)
 {
+    pdl_launch_dependents();
+    pdl_wait();
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= cnt) return;
     // a zero row / column (E == OZ2_E_ZERO) gets exponent 0 (reading R4)
@@ -355,13 +365,13 @@ int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const 
     int gy = rows_grid_y(m, k, &kchunk);
     dim3 grid((unsigned)((m + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
     if (f32) {
-        k1_rows<0, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA, sq_shift(k));
-        k1_rows<1, float><<<grid, block, 0, st>>>(m, k, Af, lda, kchunk, amaxA, ssqA, sq_shift(k));
+        OZ2_CUDA_TRY(oz2_launch(k1_rows<0, float>, grid, block, 0, st, m, k, Af, lda, kchunk, amaxA, ssqA, sq_shift(k)));
+        OZ2_CUDA_TRY(oz2_launch(k1_rows<1, float>, grid, block, 0, st, m, k, Af, lda, kchunk, amaxA, ssqA, sq_shift(k)));
     } else {
-        k1_rows<0, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA, sq_shift(k));
-        k1_rows<1, double><<<grid, block, 0, st>>>(m, k, A, lda, kchunk, amaxA, ssqA, sq_shift(k));
+        OZ2_CUDA_TRY(oz2_launch(k1_rows<0, double>, grid, block, 0, st, m, k, A, lda, kchunk, amaxA, ssqA, sq_shift(k)));
+        OZ2_CUDA_TRY(oz2_launch(k1_rows<1, double>, grid, block, 0, st, m, k, A, lda, kchunk, amaxA, ssqA, sq_shift(k)));
     }
-    k1_rows_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(mode, N, m, amaxA, ssqA, e, sq_shift(k));
+    OZ2_CUDA_TRY(oz2_launch(k1_rows_finalize, dim3((unsigned)((m + 255) / 256)), dim3(256), 0, st, mode, N, m, amaxA, ssqA, e, sq_shift(k)));
     oz2_count_launches(3);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
@@ -370,8 +380,8 @@ int oz2_launch_scale_rows(int mode, int N, int f32, int64_t m, int64_t k, const 
 int oz2_launch_scale_cols(int mode, int N, int f32, int64_t n, int64_t k, const void *B, int64_t ldb, int32_t *f, cudaStream_t st)
 {
     if (n <= 0) return 0;
-    if (f32) k1_cols<false, float><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const float *>(B), ldb, f, nullptr, sq_shift(k));
-    else k1_cols<false, double><<<(unsigned)n, COL_THREADS, 0, st>>>(mode, N, k, static_cast<const double *>(B), ldb, f, nullptr, sq_shift(k));
+    if (f32) OZ2_CUDA_TRY(oz2_launch(k1_cols<false, float>, dim3((unsigned)n), dim3(COL_THREADS), 0, st, mode, N, k, static_cast<const float *>(B), ldb, f, nullptr, sq_shift(k)));
+    else OZ2_CUDA_TRY(oz2_launch(k1_cols<false, double>, dim3((unsigned)n), dim3(COL_THREADS), 0, st, mode, N, k, static_cast<const double *>(B), ldb, f, nullptr, sq_shift(k)));
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
