@@ -719,10 +719,10 @@ int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *
     if (N == 0) {                                     // accurate mode's single plane
         if (op == 0) {
             dim3 grid((unsigned)((rows + BAR_TI - 1) / BAR_TI), (unsigned)(kp / BAR_TH));
-            k2_bar_rows<T><<<grid, BAR_THREADS, 0, st>>>(rows, k, X, ldx, ex, planes, kp);
+            OZ2_CUDA_TRY(oz2_launch(k2_bar_rows<T>, grid, dim3(BAR_THREADS), 0, st, rows, k, X, ldx, ex, planes, kp));
         } else {
             const int64_t total = rows * (kp / 4);
-            k2_bar_cols<T><<<(unsigned)((total + BAR_THREADS - 1) / BAR_THREADS), BAR_THREADS, 0, st>>>(rows, k, X, ldx, ex, planes, kp);
+            OZ2_CUDA_TRY(oz2_launch(k2_bar_cols<T>, dim3((unsigned)((total + BAR_THREADS - 1) / BAR_THREADS)), dim3(BAR_THREADS), 0, st, rows, k, X, ldx, ex, planes, kp));
         }
     } else {
         const int per_sm = wide ? 5 : 8;              // tensor memory: 64 (+ 32) columns per CTA

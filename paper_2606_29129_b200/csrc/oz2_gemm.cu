@@ -580,8 +580,8 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
     if (tiles < grid) grid = (int)tiles;
     if (rowmax) {
         // accurate mode's auxiliary product: entries <= 64, the API keeps k <= 2^18 so that 2^12 k fits INT32
-        k3_residue_gemm<EPI_MAX><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, 0, num_kb,
-                                                                      0, nullptr, mp, rowmax, colmax);
+        OZ2_CUDA_TRY(oz2_launch(k3_residue_gemm<EPI_MAX>, dim3(grid), dim3(NUM_THREADS), SMEM_BYTES, st, mapA, mapB, nplanes, mod_base, (int)m,
+                                (int)n, 0, num_kb, 0, (uint8_t *)nullptr, mp, rowmax, colmax));
         oz2_count_launches(1);
     } else {
         // the INT32 accumulator holds k <= 2^17; longer products are blocked and summed mod p_l in the epilogue
@@ -592,8 +592,8 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
                 k3_residue_gemm<EPI_NONE><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, kb0,
                                                                                nkb, 0, nullptr, mp, nullptr, nullptr);
             else
-                k3_residue_gemm<EPI_MODP><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, kb0,
-                                                                               nkb, kb0 > 0 ? 1 : 0, U, mp, nullptr, nullptr);
+                OZ2_CUDA_TRY(oz2_launch(k3_residue_gemm<EPI_MODP>, dim3(grid), dim3(NUM_THREADS), SMEM_BYTES, st, mapA, mapB, nplanes, mod_base,
+                                        (int)m, (int)n, kb0, nkb, kb0 > 0 ? 1 : 0, U, mp, (int32_t *)nullptr, (int32_t *)nullptr));
             oz2_count_launches(1);
         }
     }

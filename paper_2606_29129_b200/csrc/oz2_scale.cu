@@ -399,13 +399,13 @@ int oz2_launch_scale_accu_side(int f32, int strided, int64_t cnt, int64_t k, con
         int64_t kchunk;
         int gy = rows_grid_y(cnt, k, &kchunk);
         dim3 grid((unsigned)((cnt + ROWS_PER_BLOCK - 1) / ROWS_PER_BLOCK), (unsigned)gy), block(ROWS_PER_BLOCK, KSLICES);
-        if (f32) k1_rows<0, float><<<grid, block, 0, st>>>(cnt, k, static_cast<const float *>(X), ldx, kchunk, amax, nullptr, 44);
-        else k1_rows<0, double><<<grid, block, 0, st>>>(cnt, k, static_cast<const double *>(X), ldx, kchunk, amax, nullptr, 44);
-        k1_rows_E<<<(unsigned)((cnt + 255) / 256), 256, 0, st>>>(cnt, amax, E);
+        if (f32) OZ2_CUDA_TRY(oz2_launch(k1_rows<0, float>, grid, block, 0, st, cnt, k, static_cast<const float *>(X), ldx, kchunk, amax, (unsigned long long *)nullptr, 44));
+        else OZ2_CUDA_TRY(oz2_launch(k1_rows<0, double>, grid, block, 0, st, cnt, k, static_cast<const double *>(X), ldx, kchunk, amax, (unsigned long long *)nullptr, 44));
+        OZ2_CUDA_TRY(oz2_launch(k1_rows_E, dim3((unsigned)((cnt + 255) / 256)), dim3(256), 0, st, cnt, amax, E));
         oz2_count_launches(2);
     } else {
-        if (f32) k1_cols<true, float><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const float *>(X), ldx, nullptr, E, 44);
-        else k1_cols<true, double><<<(unsigned)cnt, COL_THREADS, 0, st>>>(0, 2, k, static_cast<const double *>(X), ldx, nullptr, E, 44);
+        if (f32) OZ2_CUDA_TRY(oz2_launch(k1_cols<true, float>, dim3((unsigned)cnt), dim3(COL_THREADS), 0, st, 0, 2, k, static_cast<const float *>(X), ldx, (int32_t *)nullptr, E, 44));
+        else OZ2_CUDA_TRY(oz2_launch(k1_cols<true, double>, dim3((unsigned)cnt), dim3(COL_THREADS), 0, st, 0, 2, k, static_cast<const double *>(X), ldx, (int32_t *)nullptr, E, 44));
         oz2_count_launches(1);
     }
     OZ2_CUDA_TRY(cudaGetLastError());
@@ -415,8 +415,8 @@ int oz2_launch_scale_accu_side(int f32, int strided, int64_t cnt, int64_t k, con
 int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA, const int32_t *EB,
                                  const int32_t *rowmax, const int32_t *colmax, int32_t *e, int32_t *f, cudaStream_t st)
 {
-    k1_accu_finalize<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(N, m, EA, rowmax, e);
-    k1_accu_finalize<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(N, n, EB, colmax, f);
+    OZ2_CUDA_TRY(oz2_launch(k1_accu_finalize, dim3((unsigned)((m + 255) / 256)), dim3(256), 0, st, N, m, EA, rowmax, e));
+    OZ2_CUDA_TRY(oz2_launch(k1_accu_finalize, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, st, N, n, EB, colmax, f));
     oz2_count_launches(2);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
