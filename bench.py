@@ -417,6 +417,22 @@ def main():
     value = world * flops / (med_ms * 1e-3) / 1e12
 
     stage_ms = [statistics.median(evs[s][t].elapsed_time(evs[s][t + 1]) for s in range(K)) for t in range(4)]
+    # the plain call, without the five stage-event records (which cut the programmatic-launch chain at the stage boundaries):
+    # K more calls between one event pair; matters below 4096^3, where launch and prologue latencies are a good part of a call
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    p0.record(stream)
+    for _ in range(K):
+        step()
+    p1.record(stream)
+    barrier()
+    plain_ms = p0.elapsed_time(p1) / K
+    if world > 1:
+        tp = torch.tensor([plain_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tp, op=dist.ReduceOp.MAX)
+        plain_ms = float(tp[0].item())
+    plain_call = dict(ms_per_call=plain_ms, value=world * flops / (plain_ms * 1e-3) / 1e12, unit="TFLOPS", calls=K,
+                      what="mean over K back-to-back plain ozaki2_dgemm calls after the timed region (no stage events)")
     X, Y = float(m) * k + float(k) * n, float(m) * n
     # algorithmic work per launch / stage
     s3_ops = N * flops + (flops if mode == 0 else 0.0)          # mode 0: the auxiliary GEMM sits in S1
@@ -543,7 +559,7 @@ def main():
                                 protocol=args.protocol,
                                 l2="inputs larger than L2 (A + B = %.2f GB per step, residue planes %.2f GB)" %
                                    (esz * X / 1e9, N * X / 1e9), parallelism="replicas" if world > 1 else "single GPU"),
-                    clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, stages=stages, path=path,
+                    clocks=clocks, e2e=e2e, plain_call=plain_call, gpu_launches=int(launches), roofline=roofline, stages=stages, path=path,
                     cpu_baseline=cpu, accuracy=accuracy,
                     peaks=dict(hbm_gbs=peaks["hbm_gbs"], bf16_tflops=peaks["bf16"],
                                bf16_tflops_sustained=peaks["bf16_sustained"], source=peaks["source"]),
