@@ -313,3 +313,16 @@ def test_per_call_workspaces_on_concurrent_streams(B):
     assert B.ozaki2_dgemm_ws(m, n, k, 1.0, Ad, m - 1, Bd, k, 0.0, Cd, m, N, mode, wp, nbytes) == -6
     # the plain entry still reports the unregistered device workspace in its own way
     assert B.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode) == B.OZAKI2_ERR_WORKSPACE
+
+
+def test_plain_launches_give_the_same_results(B):
+    # OZAKI2_PDL=0 (read once per process) launches every kernel without the programmatic-launch attribute: same results
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, OZAKI2_PDL="0")
+    r = subprocess.run([sys.executable, os.path.join(root, "__graft_entry__.py"), "--smoke"], env=env, capture_output=True, text=True,
+                       timeout=600, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    assert "smoke ok" in r.stdout
