@@ -239,9 +239,8 @@ int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64
  * 2: the cta_group::2 variant, CTA pairs on 256 x 256 tiles, a measured alternative; 3: the kernel
  * of 1 with its epilogue reduced to handing the accumulator back, U untouched -- the INT8 ceiling
  * of this loop that bench.py measures) or on a plain CUDA-core check kernel (0) that ozaki2_dgemm
- * never uses.  5 / 6 / 7: the CTA-pair kernel with resA / resB / both stored MN-major ([N][k][m] resp. [N][k][n],
- * the row index fastest: the layout the path uses for a strided operand; m > 128, n a multiple of 16).
- * k must be a multiple of 128 and m of 16 (the planes are used in place).  None needs a workspace. */
+ * never uses.  k must be a multiple of 128 and m of 16 (the planes are used in place).  None
+ * needs a workspace. */
 int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA,
                               const int8_t *resB, uint8_t *U, int use_tensor_cores, void *stream);
 

@@ -902,13 +902,7 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
     if (k <= 0 || k % 128 != 0 || k > OZAKI2_MAX_K) return -4;      // canonical planes are used in place: pitch = k
     if (m % 16 != 0) return -2;                                     // U pitch = m
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (use_tensor_cores < 0 || use_tensor_cores > 7) return -8;
-    if (use_tensor_cores >= 5) {
-        // 5 / 6 / 7: CTA pairs with resA / resB / both given MN-major ([N][k][m], [N][k][n]: row index fastest)
-        const int majA = use_tensor_cores != 6, majB = use_tensor_cores != 5;
-        if (n % 16 != 0 || !oz2_gemm_takes_mn_major(OZ2_GEMM_PAIR, m, k)) return -2;
-        return oz2_launch_gemm_tc(OZ2_GEMM_PAIR, num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st, majA, m, majB, n);
-    }
+    if (use_tensor_cores < 0 || use_tensor_cores > 4) return -8;
     if (use_tensor_cores) {
         // 1: one CTA per tile (the ozaki2_dgemm path), 2: CTA pairs, 3: the path kernel without its epilogue
         const int variant = use_tensor_cores == 2 ? OZ2_GEMM_PAIR : use_tensor_cores == 3 ? OZ2_GEMM_MMA_ONLY

@@ -69,13 +69,8 @@ int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k
 // U: [plane][n][mp].  If rowmax/colmax != NULL the epilogue keeps maxima instead (accurate mode).
 // variant: OZ2_GEMM_PATH (what ozaki2_dgemm runs), OZ2_GEMM_PAIR (cta_group::2 alternative), OZ2_GEMM_MMA_ONLY (no epilogue)
 enum { OZ2_GEMM_PATH = 0, OZ2_GEMM_PAIR = 1, OZ2_GEMM_MMA_ONLY = 2, OZ2_GEMM_PAIR_MMA_ONLY = 3 };
-// majA / majB != 0 (CTA-pair kernel only): that operand's planes are MN-major, [plane][kp][pitch] with the row index fastest
-// (pitchA / pitchB = round_up(rows, 16) bytes), instead of K-major [plane][rows][kp]
 int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA,
-                       const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st,
-                       int majA = 0, int64_t pitchA = 0, int majB = 0, int64_t pitchB = 0);
-// whether (m, kp) runs on the CTA-pair kernel, i.e. whether MN-major operand planes can be used
-bool oz2_gemm_takes_mn_major(int variant, int64_t m, int64_t kp);
+                       const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st);
 int oz2_launch_gemm_check(int nplanes, int64_t m, int64_t n, int64_t k, const int8_t *RA, const int8_t *RB, int64_t kp,
                           uint8_t *U, int64_t mp, cudaStream_t st);
 int oz2_launch_mod_p(int l, const int32_t *in, uint8_t *out, int64_t count, cudaStream_t st);

@@ -68,13 +68,6 @@ __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr)
     return d;
 }
 
-// the same for an MN-major operand (planes stored [k][row], row fastest): one 128-byte block of rows per K row, SWIZZLE_128B,
-// 8-row K groups 1024 B apart; a K step of 32 rows is 4096 B further on
-__device__ __forceinline__ uint64_t make_smem_desc_mn(uint32_t saddr)
-{
-    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024u >> 4) << 32) | (1ull << 46) | (2ull << 61);
-}
-
 // R mod p in [0, p) for any INT32 R (the GEMM epilogue and ozaki2_debug_mod_p share this routine):
 // R = hi 2^16 + lo, hi in [-2^15, 2^15), lo in [0, 2^16);  y = hi w16 + lo + bias with bias = 0 (mod p) making
 // y non-negative and y < 2^24 + 2^16, where umulhi(y, magic) is the exact quotient.
@@ -384,9 +377,8 @@ template <int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB, int nplanes,
                      int mod_base, int m, int n, int num_kb, uint8_t *__restrict__ U, int64_t mp,
-                     int32_t *__restrict__ rowmax, int32_t *__restrict__ colmax, int majA, int majB)
+                     int32_t *__restrict__ rowmax, int32_t *__restrict__ colmax)
 {
-    // majA / majB != 0: that operand's planes are MN-major ([k][row], row fastest) instead of K-major ([row][k])
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t full = smem0 + P2_STAGES * P2_STAGE_BYTES, empty = full + 8 * P2_STAGES, tfull = empty + 8 * P2_STAGES,
@@ -439,10 +431,8 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
                     const uint32_t sa = smem0 + stage * P2_STAGE_BYTES, sb = sa + P2_A_BYTES;
                     const uint32_t lbar = (full + 8 * stage) & PEER_MASK;
                     if (rank == 0) mbar_expect_tx_a(full + 8 * stage, 2 * P2_STAGE_BYTES);
-                    if (majA) tma_load_3d_pair_hint(&mapA, lbar, sa, c.m0 + (int)rank * 128, kb * TILE_K, c.plane, polA);
-                    else tma_load_3d_pair_hint(&mapA, lbar, sa, kb * TILE_K, c.m0 + (int)rank * 128, c.plane, polA);
-                    if (majB) tma_load_3d_pair(&mapB, lbar, sb, c.n0 + (int)rank * 128, kb * TILE_K, c.plane);
-                    else tma_load_3d_pair(&mapB, lbar, sb, kb * TILE_K, c.n0 + (int)rank * 128, c.plane);
+                    tma_load_3d_pair_hint(&mapA, lbar, sa, kb * TILE_K, c.m0 + (int)rank * 128, c.plane, polA);
+                    tma_load_3d_pair(&mapB, lbar, sb, kb * TILE_K, c.n0 + (int)rank * 128, c.plane);
                     if (++stage == P2_STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
@@ -454,9 +444,6 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
             uint32_t phase = 0;
             int as = 0;
             uint32_t aphase = 0;
-            // K step of 32: 32 bytes along a K-major row, 32 rows of 128 bytes in an MN-major tile (descriptor units of 16 bytes)
-            const uint64_t astep = majA ? 4096 / 16 : UMMA_K / 16, bstep = majB ? 4096 / 16 : UMMA_K / 16;
-            const uint32_t idesc = P2_IDESC | (majA ? 1u << 15 : 0u) | (majB ? 1u << 16 : 0u);
             for (int64_t t = cluster_id; t < total; t += num_clusters) {
                 mbar_wait_a(tempty + 8 * as, aphase ^ 1u);
                 tc_fence_after();
@@ -465,11 +452,11 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
                     mbar_wait_a(full + 8 * stage, phase);
                     tc_fence_after();
                     const uint32_t sa = smem0 + stage * P2_STAGE_BYTES, sb = sa + P2_A_BYTES;
-                    const uint64_t adesc = majA ? make_smem_desc_mn(sa) : make_smem_desc(sa);
-                    const uint64_t bdesc = majB ? make_smem_desc_mn(sb) : make_smem_desc(sb);
+                    const uint64_t adesc = make_smem_desc(sa), bdesc = make_smem_desc(sb);
 #pragma unroll
                     for (int ks = 0; ks < TILE_K / UMMA_K; ks++)
-                        tc_mma_i8_pair(d_tmem, adesc + (uint64_t)ks * astep, bdesc + (uint64_t)ks * bstep, idesc, (uint32_t)((kb | ks) != 0));
+                        tc_mma_i8_pair(d_tmem, adesc + (uint64_t)(ks * UMMA_K / 16), bdesc + (uint64_t)(ks * UMMA_K / 16), P2_IDESC,
+                                       (uint32_t)((kb | ks) != 0));
                     tc_commit_pair(empty + 8 * stage);         // frees this stage in BOTH CTAs
                     if (++stage == P2_STAGES) { stage = 0; phase ^= 1u; }
                 }
@@ -535,14 +522,6 @@ int make_plane_map(CUtensorMap *map, const int8_t *base, int64_t kp, int64_t row
     return encode_u8_3d_cached(map, key);
 }
 
-// MN-major planes [nplanes][kp][pitch] INT8 (row index fastest) -> 3-D map (row, k, plane), box (128, 128, 1), 128B swizzle
-int make_plane_map_mn(CUtensorMap *map, const int8_t *base, int64_t pitch, int64_t kp, int nplanes)
-{
-    const TensorMapKey key = { base, (uint64_t)pitch, (uint64_t)kp, (uint64_t)nplanes, (uint64_t)pitch, (uint64_t)(kp * pitch),
-                               128u, (uint32_t)TILE_K, 1u, (uint32_t)CU_TENSOR_MAP_SWIZZLE_128B };
-    return encode_u8_3d_cached(map, key);
-}
-
 int num_sms()
 {
     static int sms = 0;
@@ -575,24 +554,17 @@ int oz2_gemm_upload_tables(const Oz2HostTables &t)
 // 8192^3, N = 16, inside the step (profiles/r02_gemm_variants.md): pairs 5.54 - 5.66 ms, single 5.84 - 5.95 ms.
 // OZ2_GEMM_MMA_ONLY / OZ2_GEMM_PAIR_MMA_ONLY: the same kernels with the epilogue reduced to handing the accumulator
 // back (INT8 ceiling of the loop; U untouched).
-bool oz2_gemm_takes_mn_major(int variant, int64_t m, int64_t kp)
-{
-    return (variant == OZ2_GEMM_PAIR || variant == OZ2_GEMM_PAIR_MMA_ONLY) && m > TILE_M && kp <= (1 << 17);
-}
-
 int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA,
-                       const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st,
-                       int majA, int64_t pitchA, int majB, int64_t pitchB)
+                       const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st)
 {
     (void)k;
     if (m <= 0 || n <= 0 || nplanes <= 0) return 0;
     CUtensorMap mapA, mapB;
     const int num_kb = (int)(kp / TILE_K);
-    if (!oz2_gemm_takes_mn_major(variant, m, kp) && (majA || majB)) return (int)cudaErrorInvalidValue;
-    if (oz2_gemm_takes_mn_major(variant, m, kp)) {
-        int rc = majA ? make_plane_map_mn(&mapA, RA, pitchA, kp, nplanes) : make_plane_map(&mapA, RA, kp, m, nplanes, 128);
+    if ((variant == OZ2_GEMM_PAIR || variant == OZ2_GEMM_PAIR_MMA_ONLY) && m > TILE_M && kp <= (1 << 17)) {
+        int rc = make_plane_map(&mapA, RA, kp, m, nplanes, 128);
         if (rc) return rc;
-        rc = majB ? make_plane_map_mn(&mapB, RB, pitchB, kp, nplanes) : make_plane_map(&mapB, RB, kp, n, nplanes, 128);
+        rc = make_plane_map(&mapB, RB, kp, n, nplanes, 128);
         if (rc) return rc;
         const int64_t tiles = (int64_t)nplanes * ((m + P2_TILE_M - 1) / P2_TILE_M) * ((n + TILE_N - 1) / TILE_N);
         int64_t clusters = num_sms() / 2;
@@ -600,13 +572,13 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
         const unsigned grid = (unsigned)(2 * clusters);
         if (rowmax)
             OZ2_CUDA_TRY(oz2_launch(k3_residue_gemm_pair<EPI_MAX>, dim3(grid), dim3(NUM_THREADS), P2_SMEM, st, mapA, mapB, nplanes, mod_base,
-                                    (int)m, (int)n, num_kb, (uint8_t *)nullptr, mp, rowmax, colmax, majA, majB));
+                                    (int)m, (int)n, num_kb, (uint8_t *)nullptr, mp, rowmax, colmax));
         else if (variant == OZ2_GEMM_PAIR_MMA_ONLY)
             k3_residue_gemm_pair<EPI_NONE><<<grid, NUM_THREADS, P2_SMEM, st>>>(mapA, mapB, nplanes, mod_base, (int)m, (int)n, num_kb,
-                                                                          nullptr, mp, nullptr, nullptr, majA, majB);
+                                                                          nullptr, mp, nullptr, nullptr);
         else
             OZ2_CUDA_TRY(oz2_launch(k3_residue_gemm_pair<EPI_MODP>, dim3(grid), dim3(NUM_THREADS), P2_SMEM, st, mapA, mapB, nplanes, mod_base,
-                                    (int)m, (int)n, num_kb, U, mp, (int32_t *)nullptr, (int32_t *)nullptr, majA, majB));
+                                    (int)m, (int)n, num_kb, U, mp, (int32_t *)nullptr, (int32_t *)nullptr));
         oz2_count_launches(1);
         OZ2_CUDA_TRY(cudaGetLastError());
         return 0;

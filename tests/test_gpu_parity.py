@@ -296,26 +296,6 @@ def test_residue_gemm_tensor_core_vs_oracle_and_check_kernel(B, m, n, k, N):
         assert np.array_equal(Ud.cpu().numpy(), want), f"tensor_cores={tc}"
 
 
-@pytest.mark.parametrize("m,n,k,N", [(256, 256, 128, 2), (384, 272, 2048, 20), (1040, 528, 640, 5)])
-def test_residue_gemm_with_mn_major_planes(B, m, n, k, N):
-    # the layout the path uses for a strided operand: planes stored [N][k][rows] (row index fastest), taken by the CTA-pair kernel
-    # as an MN-major tcgen05 operand; A only, B only, both -- against the oracle's products
-    import torch
-    rng = np.random.Generator(np.random.PCG64(7 * k + N))
-    p = O.constants(20)["p"][:N]
-    RA = np.stack([rng.integers(-(q // 2), (q - 1) // 2 + 1, size=(m, k)) for q in p]).astype(np.int8)
-    RB = np.stack([rng.integers(-(q // 2), (q - 1) // 2 + 1, size=(n, k)) for q in p]).astype(np.int8)
-    want, _ = O.products(N, RA, RB)
-    RAd, RBd = torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda()
-    RAt = torch.from_numpy(np.ascontiguousarray(RA.transpose(0, 2, 1))).cuda()
-    RBt = torch.from_numpy(np.ascontiguousarray(RB.transpose(0, 2, 1))).cuda()
-    for tc, a, b in ((5, RAt, RBd), (6, RAd, RBt), (7, RAt, RBt)):
-        Ud = torch.zeros((N, n, m), dtype=torch.uint8, device="cuda")
-        assert B.ozaki2_debug_residue_gemm(N, m, n, k, a, b, Ud, tc) == 0
-        torch.cuda.synchronize()
-        assert np.array_equal(Ud.cpu().numpy(), want), f"variant {tc}"
-
-
 def test_mma_only_variants_leave_U_untouched(B):
     # variants 3 / 4 of ozaki2_debug_residue_gemm (the INT8 ceiling runs of bench.py) hand the accumulator back unread
     import torch
