@@ -326,3 +326,38 @@ def test_plain_launches_give_the_same_results(B):
                        timeout=600, cwd=root)
     assert r.returncode == 0, r.stderr[-2000:]
     assert "smoke ok" in r.stdout
+
+
+def test_blas_entry_fuzz(B):
+    # 36 seeded random problems through the BLAS-shaped entries: random layout, transposes, precision, shape (1 .. 300, k up
+    # to 1500), N, mode, alpha / beta, leading-dimension padding and operand scales -- bit-exact against the oracle on the
+    # logical matrices
+    import torch
+    rng = np.random.Generator(np.random.PCG64(20261106))
+    for t in range(36):
+        f32 = bool(rng.integers(0, 2))
+        dt = np.float32 if f32 else np.float64
+        m, n, k = int(rng.integers(1, 301)), int(rng.integers(1, 301)), int(rng.integers(1, 1501))
+        N = int(rng.integers(2, 13)) if f32 else int(rng.integers(2, 21))
+        mode = int(rng.integers(0, 3))
+        rm, tra, trb = bool(rng.integers(0, 2)), bool(rng.integers(0, 2)), bool(rng.integers(0, 2))
+        alpha = float(rng.choice([1.0, -1.0, 0.5, 3.0]))
+        beta = float(rng.choice([0.0, 1.0, -0.25]))
+        sa, sb = (int(rng.integers(-20, 21)), int(rng.integers(-20, 21))) if f32 else (int(rng.integers(-200, 201)), int(rng.integers(-200, 201)))
+        A, Bm = W.eq15_matrices(m, n, k, float(rng.uniform(0.0, 2.0)), 88000 + t)
+        A, Bm = np.asfortranarray(np.ldexp(A, sa).astype(dt)), np.asfortranarray(np.ldexp(Bm, sb).astype(dt))
+        Cin = rng.standard_normal((m, n)).astype(dt)
+        bufA, lda = _stored(A, tra, rm, int(rng.integers(0, 4)))
+        bufB, ldb = _stored(Bm, trb, rm, int(rng.integers(0, 4)))
+        bufC, ldc = _stored(Cin, False, rm, int(rng.integers(0, 4)))
+        Ad, Bd, Cd = torch.from_numpy(bufA).cuda(), torch.from_numpy(bufB).cuda(), torch.from_numpy(bufC.copy()).cuda()
+        B.ensure_workspace(max(m, n), max(m, n), k, N, mode)
+        call = B.ozaki2_sgemm_blas if f32 else B.ozaki2_dgemm_blas
+        tag = f"fuzz {t}: f32={f32} {m}x{n}x{k} N{N} mode{mode} rm={rm} ta={tra} tb={trb} alpha={alpha} beta={beta}"
+        assert call("R" if rm else "C", "T" if tra else "N", "T" if trb else "N", m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == 0, tag
+        torch.cuda.synchronize()
+        got = Cd.cpu().numpy()
+        got = got[:, :n] if rm else got[:, :m].T
+        with np.errstate(all="ignore"):
+            want = (O.sgemm if f32 else O.dgemm)(A, Bm, N, mode, alpha=alpha, beta=beta, C_in=Cin.copy())
+        assert np.array_equal(got, want, equal_nan=True), tag
