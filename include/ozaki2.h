@@ -183,6 +183,39 @@ int ozaki2_sgemm_host(int64_t m, int64_t n, int64_t k, float alpha, const float 
                       void *stream);
 size_t ozaki2_host_scratch_bytes(int64_t m, int64_t n, int64_t k);
 
+/*
+ * S1 for the rows of A without any memory from the caller beyond the input and the output: e[i] = log2 mu_i of
+ * Algorithm 1 (OZAKI2_MODE_FAST) or Algorithm 2 (OZAKI2_MODE_PROP) for the m rows of the
+ * column-major m x k matrix A -- the same kernels, and therefore the same integers, as the `e` that ozaki2_dgemm
+ * computes for its A.  (Accurate mode needs B and an auxiliary product; it is rejected with -6.)
+ *
+ * Who this is for.  Every other compute call of this library needs a workspace, which somebody has to cudaMalloc.
+ * Some callers may not, or cannot: a plug-in running under a host application that took all of the device memory
+ * for its own pool at start-up (a further cudaMalloc fails there, and the host's pool is not ours to carve); code
+ * in a latency-critical loop, where cudaMalloc / cudaFree stall the whole device, not one stream; a component
+ * whose rules simply forbid driver allocations after initialisation.  For them the row statistics of the two
+ * streaming passes (max |a_ih| and the integer sum of squares, 16 bytes per row) live in an array that is part of
+ * the library image itself: OZAKI2_NOALLOC_MAX_ROWS rows, 1 MiB, present on every GPU that loads the library from
+ * the moment it is loaded until the process exits, whether this call is used or not.  The call runs no cudaMalloc,
+ * cudaFree or any routine that allocates; it enqueues one memset and three kernels on `stream`.
+ *
+ * Limits and rules.
+ *   - m <= OZAKI2_NOALLOC_MAX_ROWS; a larger m returns OZAKI2_ERR_NOALLOC_LIMIT and enqueues nothing (split the rows:
+ *     e[i] depends on row i only).  k <= OZAKI2_MAX_K.  k == 0 gives e[i] = 0.
+ *   - The first call on each device looks up where that device keeps the array (and, like every entry point, uploads
+ *     the constant tables if no other call has yet).  Make that first call during initialisation, with the device
+ *     current and outside any stream capture.
+ *   - There is ONE array per device and every call uses it.  Each call zeroes the part it needs on `stream` before
+ *     its kernels, so what an earlier call left behind is harmless -- but two calls whose GPU work can overlap
+ *     (different streams without an event between them, or different host threads on different streams) read and
+ *     write the same statistics and both get wrong exponents.  Order them: one stream, or events.
+ * A: device pointer, lda >= max(1, m); e: device pointer to m int32.  Errors: -i for argument i of this prototype.
+ */
+#define OZAKI2_NOALLOC_MAX_ROWS 65536
+#define OZAKI2_ERR_NOALLOC_LIMIT (-102)
+int ozaki2_row_exponents_noalloc(int64_t m, int64_t k, const double *A, int64_t lda, int num_moduli, int scaling_mode,
+                                 int32_t *e, void *stream);
+
 /* Text for a return value of this library. */
 const char *ozaki2_status_string(int status);
 

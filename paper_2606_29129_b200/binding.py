@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libozaki2.so")
 
 OZAKI2_MODE_ACCURATE, OZAKI2_MODE_FAST, OZAKI2_MODE_PROP = 0, 1, 2
 OZAKI2_ERR_WORKSPACE, OZAKI2_ERR_DEVICE = -100, -101
+OZAKI2_NOALLOC_MAX_ROWS, OZAKI2_ERR_NOALLOC_LIMIT = 65536, -102
 OZAKI2_K_BLOCK, OZAKI2_MAX_K, OZAKI2_MAX_K_ACCURATE = 1 << 17, 1 << 22, 1 << 18
 
 _lib = None
@@ -96,6 +97,8 @@ def lib() -> C.CDLL:
         L.ozaki2_debug_mod_p.restype = ci
         L.ozaki2_debug_residue_gemm.argtypes = [ci, i64, i64, i64, vp, vp, vp, ci, vp]
         L.ozaki2_debug_residue_gemm.restype = ci
+        L.ozaki2_row_exponents_noalloc.argtypes = [i64, i64, vp, i64, ci, ci, vp, vp]
+        L.ozaki2_row_exponents_noalloc.restype = ci
         L.ozaki2_version.restype = C.c_char_p
         L.ozaki2_kernel_launches.argtypes = []
         L.ozaki2_kernel_launches.restype = C.c_uint64
@@ -264,6 +267,14 @@ def ensure_zgemm_workspace(m, n, k, num_moduli, scaling_mode):
 def ozaki2_debug_crt(num_moduli, m, n, U, e, f, alpha, beta, Cm, ldc, Cpp=None, is_f32=False, stream=None) -> int:
     return int(lib().ozaki2_debug_crt(num_moduli, m, n, _ptr(U), _ptr(e), _ptr(f), alpha, beta, _ptr(Cm), ldc, _ptr(Cpp),
                                       1 if is_f32 else 0, _stream(stream)))
+
+
+def ozaki2_row_exponents_noalloc(m, k, A, lda, num_moduli, scaling_mode, e, stream=None) -> int:
+    """e[i] = log2 mu_i for the m rows of the column-major device matrix A (fast / revised fast mode), computed with the
+    library's built-in scratch array instead of a workspace: the call for code that is not in a position to allocate
+    device memory (see include/ozaki2.h).  A, e: device tensors or addresses; at most OZAKI2_NOALLOC_MAX_ROWS rows;
+    calls on one device share the scratch and must not overlap on the GPU.  Returns the library's status."""
+    return int(lib().ozaki2_row_exponents_noalloc(m, k, _ptr(A), lda, num_moduli, scaling_mode, _ptr(e), _stream(stream)))
 
 
 def ozaki2_get_constants(num_moduli: int) -> dict:

@@ -836,6 +836,8 @@ const char *ozaki2_status_string(int status)
     if (status == 0) return "success";
     if (status == OZAKI2_ERR_WORKSPACE) return "workspace missing or too small (ozaki2_set_workspace)";
     if (status == OZAKI2_ERR_DEVICE) return "current device is not sm_100 (B200)";
+    if (status == OZAKI2_ERR_NOALLOC_LIMIT)
+        return "more rows than the built-in scratch of ozaki2_row_exponents_noalloc holds (OZAKI2_NOALLOC_MAX_ROWS = 65536): split the rows";
     if (status < 0 && status >= -14) {
         snprintf(buf, sizeof buf, "invalid argument %d (ozaki2_dgemm numbering: %s)", -status, arg_names[-status]);
         return buf;
@@ -952,6 +954,32 @@ int ozaki2_debug_crt(int num_moduli, int64_t m, int64_t n, const uint8_t *U, con
     if (!C) return -9;
     if (ldc < m) return -10;
     return oz2_launch_crt(num_moduli, is_f32 ? 1 : 0, m, n, U, m, e, f, alpha, beta, C, ldc, Cpp, static_cast<cudaStream_t>(stream));
+}
+
+// S1 for the rows of A with the row statistics in the library's own static device array (oz2_scale.cu): for callers
+// that have no way of allocating a workspace.  Checks first, so that an oversized problem touches nothing.
+int ozaki2_row_exponents_noalloc(int64_t m, int64_t k, const double *A, int64_t lda, int num_moduli, int scaling_mode,
+                                 int32_t *e, void *stream)
+{
+    static_assert(OZAKI2_NOALLOC_MAX_ROWS == OZ2_NOALLOC_MAX_ROWS, "header and kernel source disagree on the limit");
+    if (m < 0) return -1;
+    if (m > OZAKI2_NOALLOC_MAX_ROWS) return OZAKI2_ERR_NOALLOC_LIMIT;
+    if (k < 0 || k > OZAKI2_MAX_K) return -2;
+    if (m > 0 && k > 0 && !A) return -3;
+    if (lda < (m > 1 ? m : 1)) return -4;
+    if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return -5;
+    if (scaling_mode != OZAKI2_MODE_FAST && scaling_mode != OZAKI2_MODE_PROP) return -6;
+    if (m > 0 && !e) return -7;
+    if (m == 0) return 0;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    DeviceState *dev = nullptr;
+    int rc = ensure_device(&dev);
+    if (rc) return rc;
+    if (k == 0) {                                                   // empty rows are zero rows: exponent 0 (reading R4)
+        OZ2_CUDA_TRY(cudaMemsetAsync(e, 0, sizeof(int32_t) * (size_t)m, st));
+        return 0;
+    }
+    return oz2_launch_scale_rows_noalloc(scaling_mode, num_moduli, m, k, A, lda, e, st);
 }
 
 uint64_t ozaki2_kernel_launches(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -60,6 +60,10 @@ int oz2_launch_scale_accu_side(int f32, int strided, int64_t cnt, int64_t k, con
 int oz2_launch_scale_accu_finish(int N, int64_t m, int64_t n, const int32_t *EA, const int32_t *EB,
                                  const int32_t *rowmax, const int32_t *colmax, int32_t *e, int32_t *f, cudaStream_t st);
 int oz2_launch_log2f(const float *x, float *y, int64_t count, cudaStream_t st);
+// oz2_launch_scale_rows with amax / ssq in the library's own static device array (ozaki2_row_exponents_noalloc);
+// m <= OZ2_NOALLOC_MAX_ROWS is the caller's check
+#define OZ2_NOALLOC_MAX_ROWS 65536
+int oz2_launch_scale_rows_noalloc(int mode, int N, int64_t m, int64_t k, const double *A, int64_t lda, int32_t *e, cudaStream_t st);
 
 // S2: residues of op(X) for all N moduli in one pass.  planes: [N][rows][kp]
 int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k, const void *X, int64_t ldx,

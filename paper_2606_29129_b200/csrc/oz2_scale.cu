@@ -14,6 +14,8 @@
 // reduced by one block with warp shuffles.
 #include "oz2_common.cuh"
 
+#include <mutex>
+
 namespace {
 
 __constant__ Oz2CrtTab c_crt[OZ2_MAX_MODULI + 1];
@@ -429,4 +431,58 @@ int oz2_launch_log2f(const float *x, float *y, int64_t count, cudaStream_t st)
     oz2_count_launches(1);
     OZ2_CUDA_TRY(cudaGetLastError());
     return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// ozaki2_row_exponents_noalloc: the row kernels above with their statistics in memory the library brings along
+// ---------------------------------------------------------------------------------------------
+// For callers that cannot hand us a workspace because they cannot allocate one: a plug-in whose host application
+// owns all device memory, a control loop that must not stall the device in cudaMalloc, a component that may not touch
+// the driver's allocator after start-up.  k1_rows<0> / k1_rows<1> / k1_rows_finalize need 16 bytes of scratch per
+// row (amax[i], ssq[i]); here those come from a fixed array in the module's data segment: 2 x 65536 x 8 B = 1 MiB,
+// loaded with the library on every GPU that uses it and released only at process exit.
+//
+// The identifier below means two different things.  Inside a kernel it is the array.  In host code it is only the
+// handle the runtime registered for it -- not a device address -- so it must never be passed to a kernel or to
+// cudaMemsetAsync as it stands: the device address is asked for with cudaGetSymbolAddress, once per device (each
+// device has its own copy at its own address) while that device is current, and that address is what the kernels get.
+namespace {
+
+static __device__ __align__(256) unsigned long long g_noalloc_row_stats[2 * OZ2_NOALLOC_MAX_ROWS];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned long long *g_noalloc_addr[NOALLOC_MAX_DEVICES];   // device address of g_noalloc_row_stats, per device; null = not asked yet
+std::mutex g_noalloc_mu;
+
+// Set-up on first use per device.  No allocation: the array already exists on the device.
+int noalloc_row_stats(unsigned long long **out)
+{
+    int dev = -1;
+    OZ2_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return (int)cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_addr[dev]) {
+        void *p = nullptr;
+        const cudaError_t rc = cudaGetSymbolAddress(&p, g_noalloc_row_stats);    // address on the CURRENT device
+        if (rc != cudaSuccess) return (int)rc;
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255)) return (int)cudaErrorInvalidSymbol;
+        g_noalloc_addr[dev] = static_cast<unsigned long long *>(p);
+    }
+    *out = g_noalloc_addr[dev];
+    return 0;
+}
+
+} // namespace
+
+int oz2_launch_scale_rows_noalloc(int mode, int N, int64_t m, int64_t k, const double *A, int64_t lda, int32_t *e, cudaStream_t st)
+{
+    if (m <= 0) return 0;
+    if (m > OZ2_NOALLOC_MAX_ROWS) return (int)cudaErrorInvalidValue;           // the entry point has refused this already
+    unsigned long long *stats = nullptr;
+    const int rc = noalloc_row_stats(&stats);
+    if (rc) return rc;
+    // amax[0..m) and ssq[0..m) side by side (256-byte aligned), so that the launcher zeroes exactly the 16 m bytes this
+    // call uses with one stream-ordered memset: the array still holds the statistics of whichever call ran before
+    unsigned long long *amax = stats, *ssq = stats + oz2_round_up(m, 32);
+    return oz2_launch_scale_rows(mode, N, 0, m, k, A, lda, amax, ssq, e, st);
 }
