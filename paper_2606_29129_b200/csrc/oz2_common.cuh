@@ -71,7 +71,8 @@ int oz2_launch_convert(int op, int N, int wide, int f32, int64_t rows, int64_t k
 
 // S3: batched INT8 GEMM with mod-p epilogue (tcgen05).  nplanes GEMMs; modulus index of plane b is mod_base + b.
 // U: [plane][n][mp].  If rowmax/colmax != NULL the epilogue keeps maxima instead (accurate mode).
-// variant: OZ2_GEMM_PATH (what ozaki2_dgemm runs), OZ2_GEMM_PAIR (cta_group::2 alternative), OZ2_GEMM_MMA_ONLY (no epilogue)
+// variant: OZ2_GEMM_PAIR (cta_group::2, CTA pairs on 256 x 256 tiles: what ozaki2_dgemm runs), OZ2_GEMM_PATH (one CTA per
+// 128 x 256 tile: m <= 128, K-blocked products, OZAKI2_GEMM=single), OZ2_GEMM_MMA_ONLY / OZ2_GEMM_PAIR_MMA_ONLY (no epilogue)
 enum { OZ2_GEMM_PATH = 0, OZ2_GEMM_PAIR = 1, OZ2_GEMM_MMA_ONLY = 2, OZ2_GEMM_PAIR_MMA_ONLY = 3 };
 int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_t n, int64_t k, const int8_t *RA,
                        const int8_t *RB, int64_t kp, uint8_t *U, int64_t mp, int32_t *rowmax, int32_t *colmax, cudaStream_t st);
@@ -92,6 +93,10 @@ void oz2_count_launches(int n);
 // to complete and flush (pdl_wait) before it touches anything the predecessor wrote -- and in any case before it exits,
 // which keeps the dependency transitive along the chain.  What runs before the wait (barrier initialisation, tensor-memory
 // allocation, constant operand images) overlaps the predecessor's tail; at small sizes that is a good part of the call.
+// Invariant for kernels that allocate tensor memory: they signal only AFTER tcgen05.alloc has returned and the CTA (pair) has
+// synchronised on it.  Dependents become schedulable once every CTA of the predecessor has signalled, i.e. once all of them
+// own their columns -- a dependent CTA that became resident earlier, took its columns and sat in pdl_wait could otherwise
+// starve a predecessor CTA still blocked in tcgen05.alloc, which no time-out covers.
 // OZAKI2_PDL=0 in the environment (read once) launches everything the plain way.
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }

@@ -60,21 +60,6 @@ __device__ __forceinline__ uint64_t kmajor_desc(uint32_t saddr, uint32_t sbo)
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(128u >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
 }
 
-__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
-{
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
-          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
-          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr)
-        : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-
 // ---------------------------------------------------------------------------------------------
 // trunc(a 2^ex)
 // ---------------------------------------------------------------------------------------------
@@ -476,8 +461,8 @@ k2_tc_cols(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
     extern __shared__ uint8_t smem_raw[];
     ConvSmem<WIDE> *S = conv_smem<WIDE>(smem_raw);
     ConvCtx cx;
-    pdl_launch_dependents();
     conv_setup<WIDE>(S, cx, N);
+    pdl_launch_dependents();                         // after the tensor-memory allocation of conv_setup (oz2_common.cuh)
     pdl_wait();                                      // the exponents come from the scaling kernels
     const int tid = threadIdx.x;
     const int chunks = (int)((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);      // k <= 2^22: fits 32 bits
@@ -544,8 +529,8 @@ k2_tc_rows(int N, int64_t rows, int64_t k, const T *__restrict__ X, int64_t ldx,
     constexpr int PITCH = StageRow<T>::PITCH;
     T *stage = reinterpret_cast<T *>(S + 1);
     ConvCtx cx;
-    pdl_launch_dependents();
     conv_setup<WIDE>(S, cx, N);
+    pdl_launch_dependents();                         // after the tensor-memory allocation of conv_setup (oz2_common.cuh)
     pdl_wait();                                      // the exponents come from the scaling kernels
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nib = (int)((rows + ST_ROWS - 1) / ST_ROWS), nhb = (int)(kp / ST_H);
@@ -696,17 +681,6 @@ k2_bar_cols(int64_t n, int64_t k, const T *__restrict__ B, int64_t ldb, const in
     quad_bar(a, __ldg(E + j), plane + j * kp + h);
 }
 
-int num_sms()
-{
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    }
-    return sms;
-}
-
 template <int WIDE, typename T>
 constexpr size_t rows_smem() { return sizeof(ConvSmem<WIDE>) + 128 + (size_t)ST_ROWS * StageRow<T>::PITCH * sizeof(T); }
 template <int WIDE>
@@ -728,13 +702,13 @@ int launch_convert_t(int op, int N, int wide, int64_t rows, int64_t k, const T *
         const int per_sm = wide ? 5 : 8;              // tensor memory: 64 (+ 32) columns per CTA
         if (op == 0) {
             const int64_t items = ((rows + ST_ROWS - 1) / ST_ROWS) * (kp / ST_H);
-            int64_t grid = (int64_t)num_sms() * per_sm;
+            int64_t grid = (int64_t)oz2_num_sms() * per_sm;
             if (grid > items) grid = items;
             if (wide) OZ2_CUDA_TRY(oz2_launch(k2_tc_rows<1, T>, dim3((unsigned)grid), dim3(CV_THREADS), rows_smem<1, T>(), st, N, rows, k, X, ldx, ex, planes, kp));
             else OZ2_CUDA_TRY(oz2_launch(k2_tc_rows<0, T>, dim3((unsigned)grid), dim3(CV_THREADS), rows_smem<0, T>(), st, N, rows, k, X, ldx, ex, planes, kp));
         } else {
             const int64_t items = rows * ((kp + CV_CHUNK_H - 1) / CV_CHUNK_H);
-            int64_t grid = (int64_t)num_sms() * per_sm;
+            int64_t grid = (int64_t)oz2_num_sms() * per_sm;
             if (grid > items) grid = items;
             if (wide) OZ2_CUDA_TRY(oz2_launch(k2_tc_cols<1, T>, dim3((unsigned)grid), dim3(CV_THREADS), cols_smem<1>(), st, N, rows, k, X, ldx, ex, planes, kp));
             else OZ2_CUDA_TRY(oz2_launch(k2_tc_cols<0, T>, dim3((unsigned)grid), dim3(CV_THREADS), cols_smem<0>(), st, N, rows, k, X, ldx, ex, planes, kp));

@@ -360,20 +360,6 @@ constexpr int K5_SMEM = K5_STAGES * K5_STAGE_BYTES + 1024 /*B image*/ + 1024 /*a
 
 __device__ uint8_t g_wb_image[OZ2_MAX_MODULI + 1][1024];        // per N: B operand image (see upload)
 
-__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
-{
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
-          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
-          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr)
-        : "memory");
-}
-
 // fold the byte slices S[0 .. 4 NW) of one element into the words of C'
 template <int NW>
 __device__ __forceinline__ void k5_fold(const uint32_t *S, uint32_t (&c)[NW + 1])
@@ -455,7 +441,6 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     uint8_t *gen0 = smem_raw + (smem0 - smem_u32(smem_raw));                // generic pointer to the aligned base
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    pdl_launch_dependents();
     // The grid is nib x gj CTAs: CTA b owns row block ib = ib0 + b % nib (512 rows: its exponents e_i stay in registers) and
     // walks the columns j = b / nib, + gj, + 2 gj, ...
     const int gj = (int)gridDim.x / nib;
@@ -486,6 +471,7 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
     tc_fence_after();
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+    pdl_launch_dependents();                      // only now: this CTA owns its tensor-memory columns (oz2_common.cuh)
     pdl_wait();                                   // the residue products come from the GEMM
 
     if (warp == 0) {
@@ -549,8 +535,8 @@ k5_crt_tc(const __grid_constant__ CUtensorMap mapU, int N, int m, int n, const i
 #pragma unroll
             for (int pr = 0; pr < 2; pr++) {                 // elements (i + 256 pr, i + 256 pr + 128)
                 uint32_t S[2 * NS];
-                tc_ld32(taddr + (uint32_t)(pr * 2 * NS), *reinterpret_cast<uint32_t(*)[32]>(S));
-                if constexpr (NS == 32) tc_ld32(taddr + (uint32_t)(pr * 2 * NS + 32), *reinterpret_cast<uint32_t(*)[32]>(S + 32));
+                tc_ld32_nowait(taddr + (uint32_t)(pr * 2 * NS), *reinterpret_cast<uint32_t(*)[32]>(S));
+                if constexpr (NS == 32) tc_ld32_nowait(taddr + (uint32_t)(pr * 2 * NS + 32), *reinterpret_cast<uint32_t(*)[32]>(S + 32));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                 if (pr == 1) {                               // both pairs are out of tensor memory: hand the buffer back
                     tc_fence_before();
@@ -578,23 +564,14 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
                                128u, 1u, (uint32_t)K5_KPAD, (uint32_t)CU_TENSOR_MAP_SWIZZLE_128B };
     const int erc = encode_u8_3d_cached(&map, key);
     if (erc) return erc;
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    }
+    const int sms = oz2_num_sms();
     const int64_t tiles_i = (m + K5_TILE_I - 1) / K5_TILE_I;
     const int per_sm = NW <= 4 ? 3 : 2;                   // TMEM: 128 / 256 columns per CTA; 320 threads; 3 x 51 KB shared
     const int64_t gmax = (int64_t)sms * per_sm;
     if (ldc >= (int64_t)1 << 31 || mp >= (int64_t)1 << 31) return (int)cudaErrorInvalidValue;
     const int mi = (int)m, ni = (int)n, ldi = (int)ldc, mpi = (int)mp;
-    static bool attr_set[3] = { false, false, false };     // per kernel variant of this (NW, TO) instantiation
-    auto launch = [&](auto kern, int variant, uint64_t *cpp) -> int {
-        if (!attr_set[variant]) {
-            OZ2_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, K5_SMEM));
-            attr_set[variant] = true;
-        }
+    // (the > 48 KB dynamic shared memory opt-in of these kernels is per device: oz2_crt_upload_tables)
+    auto launch = [&](auto kern, uint64_t *cpp) -> int {
         // grid = (row blocks of the launch) x (columns in flight); more row blocks than resident CTAs: several launches
         for (int64_t ib0 = 0; ib0 < tiles_i; ib0 += gmax) {
             const int64_t nib = tiles_i - ib0 < gmax ? tiles_i - ib0 : gmax;
@@ -607,17 +584,41 @@ int launch_tc(int N, int64_t m, int64_t n, const uint8_t *U, int64_t mp, const i
         return 0;
     };
     int lrc;
-    if (Cpp) lrc = launch(k5_crt_tc<NW, true, false, TO>, 0, Cpp);
-    else if (beta == (TO)0) lrc = launch(k5_crt_tc<NW, false, true, TO>, 1, nullptr);
-    else lrc = launch(k5_crt_tc<NW, false, false, TO>, 2, nullptr);
+    if (Cpp) lrc = launch(k5_crt_tc<NW, true, false, TO>, Cpp);
+    else if (beta == (TO)0) lrc = launch(k5_crt_tc<NW, false, true, TO>, nullptr);
+    else lrc = launch(k5_crt_tc<NW, false, false, TO>, nullptr);
     if (lrc) return lrc;
     return (int)cudaGetLastError();
 }
 
+// k5_crt_tc needs more than 48 KB of dynamic shared memory; the opt-in is a per-device attribute of each instantiation
+template <int NW, typename TO>
+int k5_opt_in_smem()
+{
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k5_crt_tc<NW, true, false, TO>, cudaFuncAttributeMaxDynamicSharedMemorySize, K5_SMEM));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k5_crt_tc<NW, false, true, TO>, cudaFuncAttributeMaxDynamicSharedMemorySize, K5_SMEM));
+    OZ2_CUDA_TRY(cudaFuncSetAttribute(k5_crt_tc<NW, false, false, TO>, cudaFuncAttributeMaxDynamicSharedMemorySize, K5_SMEM));
+    return 0;
+}
+template <typename TO>
+int k5_opt_in_smem_all()
+{
+    int rc;
+    if ((rc = k5_opt_in_smem<1, TO>())) return rc;
+    if ((rc = k5_opt_in_smem<2, TO>())) return rc;
+    if ((rc = k5_opt_in_smem<3, TO>())) return rc;
+    if ((rc = k5_opt_in_smem<4, TO>())) return rc;
+    return k5_opt_in_smem<5, TO>();
+}
+
 } // namespace
 
+// runs once per device (ensure_device, under its lock) with that device current
 int oz2_crt_upload_tables(const Oz2HostTables &t)
 {
+    int arc;
+    if ((arc = k5_opt_in_smem_all<double>())) return arc;
+    if ((arc = k5_opt_in_smem_all<float>())) return arc;
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(c_crt, t.crt, sizeof(t.crt)));
     // B operand images of k5_crt_tc: element (slice s, modulus l) at (s/8) 256 + (l/16) 128 + (s%8) 16 + (l%16)
     static uint8_t img[OZ2_MAX_MODULI + 1][1024];
@@ -630,9 +631,10 @@ int oz2_crt_upload_tables(const Oz2HostTables &t)
             }
     OZ2_CUDA_TRY(cudaMemcpyToSymbol(g_wb_image, img, sizeof(img)));
     // constants of the common case: Pn = 2^(32 NW) - P, K0 = 2^(32 (NW - 1)) / P, K1 = K0 2^-32
+    // (host copy: written by the first device's set-up only -- a later device's must not disturb launches on the first)
+    static bool h_k5_ready = false;
     K5Consts *k5 = h_k5;
-    memset(h_k5, 0, sizeof(h_k5));
-    for (int N = 2; N <= OZ2_MAX_MODULI; N++) {
+    for (int N = 2; N <= OZ2_MAX_MODULI && !h_k5_ready; N++) {
         const int nw = words_of_P(N);
         unsigned long long borrow = 0;
         for (int w = 0; w < nw; w++) {                       // 0 - P over nw words
@@ -643,6 +645,7 @@ int oz2_crt_upload_tables(const Oz2HostTables &t)
         k5[N].K0 = t.crt[N].invP;
         k5[N].K1 = t.crt[N].invP * 2.3283064365386963e-10;
     }
+    h_k5_ready = true;
     return 0;
 }
 

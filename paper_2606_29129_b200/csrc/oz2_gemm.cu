@@ -40,22 +40,6 @@ constexpr int GROUP_M = 32;
 constexpr uint32_t IDESC = (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TILE_N >> 3) << 17) |
                            ((uint32_t)(TILE_M >> 4) << 24);
 
-// 32 lanes x 32 consecutive columns of 32-bit accumulators -> 32 registers per thread
-__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
-{
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
-          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
-          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
-          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr)
-        : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-
 // shared-memory matrix descriptor: K-major, SWIZZLE_128B, rows of 128 B, 8-row groups 1024 B apart
 __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr)
 {
@@ -215,7 +199,6 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tiles_m = (m + TILE_M - 1) / TILE_M, tiles_n = (n + TILE_N - 1) / TILE_N;
     const int64_t total = (int64_t)nplanes * tiles_m * tiles_n;
-    pdl_launch_dependents();
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; s++) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
@@ -232,6 +215,7 @@ k3_residue_gemm(const __grid_constant__ CUtensorMap mapA, const __grid_constant_
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    pdl_launch_dependents();                      // only now: this CTA owns its tensor-memory columns (oz2_common.cuh)
     pdl_wait();                                   // the residue planes come from the conversion kernels
 
     if (warp == 0) {
@@ -389,7 +373,6 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
     const int tiles_m = (m + P2_TILE_M - 1) / P2_TILE_M, tiles_n = (n + TILE_N - 1) / TILE_N;
     const int64_t total = (int64_t)nplanes * tiles_m * tiles_n;
     const int64_t cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
-    pdl_launch_dependents();
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < P2_STAGES; s++) {
@@ -413,6 +396,7 @@ k3_residue_gemm_pair(const __grid_constant__ CUtensorMap mapA, const __grid_cons
     tc_fence_after();
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+    pdl_launch_dependents();                      // only now: the pair owns its tensor-memory columns (oz2_common.cuh)
     pdl_wait();                                   // the residue planes come from the conversion kernels
 
     if (warp == 0) {
@@ -522,19 +506,6 @@ int make_plane_map(CUtensorMap *map, const int8_t *base, int64_t kp, int64_t row
     return encode_u8_3d_cached(map, key);
 }
 
-int num_sms()
-{
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        const char *e = getenv("OZAKI2_GEMM_SMS");        // experiment knob: SMs the persistent GEMM grid may use
-        if (e && atoi(e) > 1 && atoi(e) < sms) sms = atoi(e);
-    }
-    return sms;
-}
-
 } // namespace
 
 int oz2_gemm_upload_tables(const Oz2HostTables &t)
@@ -567,7 +538,7 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
         rc = make_plane_map(&mapB, RB, kp, n, nplanes, 128);
         if (rc) return rc;
         const int64_t tiles = (int64_t)nplanes * ((m + P2_TILE_M - 1) / P2_TILE_M) * ((n + TILE_N - 1) / TILE_N);
-        int64_t clusters = num_sms() / 2;
+        int64_t clusters = oz2_num_sms() / 2;
         if (tiles < clusters) clusters = tiles;
         const unsigned grid = (unsigned)(2 * clusters);
         if (rowmax)
@@ -588,7 +559,7 @@ int oz2_launch_gemm_tc(int variant, int nplanes, int mod_base, int64_t m, int64_
     rc = make_plane_map(&mapB, RB, kp, n, nplanes, TILE_N);
     if (rc) return rc;
     const int64_t tiles = (int64_t)nplanes * ((m + TILE_M - 1) / TILE_M) * ((n + TILE_N - 1) / TILE_N);
-    int grid = num_sms();
+    int grid = oz2_num_sms();
     if (tiles < grid) grid = (int)tiles;
     if (rowmax) {
         // accurate mode's auxiliary product: entries <= 64, the API keeps k <= 2^18 so that 2^12 k fits INT32
