@@ -90,6 +90,10 @@ int ozaki2_dgemm_t(int transa, int transb, int64_t m, int64_t n, int64_t k, doub
 int ozaki2_dgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha, const double *A,
                       int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int num_moduli,
                       int scaling_mode, void *stream);
+/* Workspace of an ozaki2_dgemm_blas / ozaki2_sgemm_blas call with this `layout` (same flag values; 0 for an invalid problem):
+ * ozaki2_workspace_bytes(m, n, k, ...) for column-major and ozaki2_workspace_bytes(n, m, k, ...) for row-major, because a
+ * row-major call runs internally with m and n exchanged (with m = 300, n = 1 the row-major call needs the larger figure). */
+size_t ozaki2_blas_workspace_bytes(int layout, int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 
 /*
  * SGEMM variant (Fig. 6): A, B, C are FP32 (4-byte aligned device pointers, same
@@ -116,7 +120,8 @@ int ozaki2_sgemm_blas(int layout, int transa, int transb, int64_t m, int64_t n, 
  * elements; 16-byte aligned device pointers), computed as ozaki2_dgemm on the real embedding
  * [C_r; C_i] = [[A_r, -A_i], [A_i, A_r]] [B_r; B_i]  (a (2m x 2k)(2k x n) product: one scaling exponent per complex row
  * of A / column of B, condition (1) holds for both parts), then out = alpha c + beta C in plain complex arithmetic with
- * every product and sum rounded on its own (alpha == 1 and beta == 0 are not multiplied; beta == 0 overwrites).  The
+ * every product and sum rounded on its own (alpha == 1, beta == 0 and beta == 1 are not multiplied: beta == 0 overwrites,
+ * beta == 1 adds C as it is, and with k == 0 or alpha == 0 leaves C untouched, as the real entry points do).  The
  * embedded operands are materialised in the workspace: register ozaki2_zgemm_workspace_bytes(...) bytes with
  * ozaki2_set_workspace.  2k <= OZAKI2_MAX_K (OZAKI2_MAX_K_ACCURATE in accurate mode).  Errors: -i for argument i.
  */
@@ -135,7 +140,8 @@ int ozaki2_cgemm(int64_t m, int64_t n, int64_t k, float alpha_re, float alpha_im
                  int num_moduli, int scaling_mode, void *stream);
 size_t ozaki2_cgemm_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 
-/* Bytes of device workspace ozaki2_dgemm / ozaki2_sgemm needs for this problem (0 for an invalid one). */
+/* Bytes of device workspace ozaki2_dgemm / ozaki2_sgemm (and their _t, _ws, _stages forms) need for this problem (0 for an
+ * invalid one).  The figure is NOT symmetric in m and n. */
 size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode);
 
 /*
@@ -216,6 +222,14 @@ size_t ozaki2_host_scratch_bytes(int64_t m, int64_t n, int64_t k);
 int ozaki2_row_exponents_noalloc(int64_t m, int64_t k, const double *A, int64_t lda, int num_moduli, int scaling_mode,
                                  int32_t *e, void *stream);
 
+/*
+ * Environment.  The library reads two variables, once, when it is first used; neither changes a result:
+ *   OZAKI2_PDL=0        launch every kernel the plain way instead of chaining the kernels of a call by programmatic
+ *                       dependent launch (a diagnostic switch: profilers and sanitizers see ordinary launches)
+ *   OZAKI2_GEMM=single  run S3 on the one-CTA-per-tile kernel instead of CTA pairs
+ * Everything else is an argument.
+ */
+
 /* Text for a return value of this library. */
 const char *ozaki2_status_string(int status);
 
@@ -267,13 +281,13 @@ int ozaki2_debug_log2f(const float *x, float *y, int64_t count, void *stream);
  * epilogue of the residue GEMM.  in, out: device pointers. */
 int ozaki2_debug_mod_p(int modulus_index, const int32_t *in, uint8_t *out, int64_t count, void *stream);
 
-/* One INT8 product resA_l resB_l^T mod p_l for canonical planes (same layouts as above) on the
- * tensor-core kernel (use_tensor_cores = 1: one CTA per 128 x 256 tile, what ozaki2_dgemm runs;
- * 2: the cta_group::2 variant, CTA pairs on 256 x 256 tiles, a measured alternative; 3: the kernel
- * of 1 with its epilogue reduced to handing the accumulator back, U untouched -- the INT8 ceiling
- * of this loop that bench.py measures) or on a plain CUDA-core check kernel (0) that ozaki2_dgemm
- * never uses.  k must be a multiple of 128 and m of 16 (the planes are used in place).  None
- * needs a workspace. */
+/* One INT8 product resA_l resB_l^T mod p_l for canonical planes (same layouts as above) on a
+ * tensor-core kernel -- use_tensor_cores = 2: the cta_group::2 kernel, CTA pairs on 256 x 256 tiles,
+ * what ozaki2_dgemm runs (for m > 128 and k <= OZAKI2_K_BLOCK); 1: one CTA per 128 x 256 tile, what
+ * it runs otherwise and the measured alternative; 3 / 4: the kernels of 1 / 2 with the epilogue
+ * reduced to handing the accumulator back, U untouched (the INT8 ceiling of each loop that bench.py
+ * measures) -- or on a plain CUDA-core check kernel (0) that ozaki2_dgemm never uses.  k must be a
+ * multiple of 128 and m of 16 (the planes are used in place).  None needs a workspace. */
 int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, const int8_t *resA,
                               const int8_t *resB, uint8_t *U, int use_tensor_cores, void *stream);
 

@@ -2,7 +2,8 @@
 
 TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
 cpu_baseline / --impl reference legs import this.  It never imports the CUDA package.
-Argument marshalling only; every number is computed by the C file.
+Argument marshalling only for the real entry points (every number is computed by the C file); the complex variants
+zgemm / cgemm are DEFINED here: numpy embedding, the C oracle on it, and the complex alpha / beta tail in numpy.
 """
 from __future__ import annotations
 
@@ -287,7 +288,9 @@ def zgemm_embedding(A, B):
 def zgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_in=None):
     """Complex variant (named as future work at P:58; reading in DESIGN.md 8b #4): oz2o_dgemm on the real embedding,
     then out = alpha c + beta C_in in plain complex arithmetic -- every product and every sum rounded on its own, in the
-    order written below; alpha == 1 and beta == 0 are not multiplied (BLAS rule: beta == 0 overwrites)."""
+    order written below; alpha == 1, beta == 0 and beta == 1 are not multiplied (BLAS rules: beta == 0 overwrites, beta == 1
+    adds C_in as it is -- for finite C_in the same bits as 1 * C_in, but an Inf or NaN in one part of an entry no longer
+    reaches the other part through 0 * Inf)."""
     A = np.asarray(A, dtype=np.complex128)
     B = np.asarray(B, dtype=np.complex128)
     m = A.shape[0]
@@ -301,7 +304,11 @@ def zgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_
             ti = alpha.real * ci + alpha.imag * cr
     else:
         tr, ti = cr, ci
-    if beta != 0.0:
+    if beta == 1.0:
+        Cin = np.asarray(C_in, dtype=np.complex128)
+        with np.errstate(all="ignore"):
+            tr, ti = tr + Cin.real, ti + Cin.imag
+    elif beta != 0.0:
         Cin = np.asarray(C_in, dtype=np.complex128)
         with np.errstate(all="ignore"):
             tr = tr + (beta.real * Cin.real - beta.imag * Cin.imag)
@@ -314,7 +321,7 @@ def zgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_
 def cgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_in=None):
     """Single-precision complex variant (same reading as zgemm, DESIGN.md 8b #4): oz2o_sgemm on the real embedding of the FP32
     parts, then out = alpha c + beta C_in in FP32 complex arithmetic -- every product and every sum rounded to FP32 on its own,
-    in the order written below; alpha == 1 and beta == 0 are not multiplied."""
+    in the order written below; alpha == 1, beta == 0 and beta == 1 are not multiplied."""
     A = np.asarray(A, dtype=np.complex64)
     B = np.asarray(B, dtype=np.complex64)
     m = A.shape[0]
@@ -331,7 +338,11 @@ def cgemm(A, B, N: int, mode: int, alpha: complex = 1.0, beta: complex = 0.0, C_
             ti = (ar * ci).astype(f) + (ai * cr).astype(f)
     else:
         tr, ti = cr, ci
-    if beta != 0.0:
+    if beta == 1.0:
+        Cin = np.asarray(C_in, dtype=np.complex64)
+        with np.errstate(all="ignore"):
+            tr, ti = tr + Cin.real, ti + Cin.imag
+    elif beta != 0.0:
         Cin = np.asarray(C_in, dtype=np.complex64)
         br, bi = f(beta.real), f(beta.imag)
         with np.errstate(all="ignore"):

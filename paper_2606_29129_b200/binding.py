@@ -82,6 +82,8 @@ def lib() -> C.CDLL:
         L.ozaki2_debug_crt.restype = ci
         L.ozaki2_workspace_bytes.argtypes = [i64, i64, i64, ci, ci]
         L.ozaki2_workspace_bytes.restype = C.c_size_t
+        L.ozaki2_blas_workspace_bytes.argtypes = [ci, i64, i64, i64, ci, ci]
+        L.ozaki2_blas_workspace_bytes.restype = C.c_size_t
         L.ozaki2_host_scratch_bytes.argtypes = [i64, i64, i64]
         L.ozaki2_host_scratch_bytes.restype = C.c_size_t
         L.ozaki2_set_workspace.argtypes = [vp, C.c_size_t]
@@ -224,6 +226,10 @@ def ozaki2_sgemm_blas(layout, transa, transb, m, n, k, alpha, A, lda, B, ldb, be
                       stream=None) -> int:
     return int(lib().ozaki2_sgemm_blas(_flag(layout), _flag(transa), _flag(transb), m, n, k, alpha, _ptr(A), lda, _ptr(B), ldb,
                                        beta, _ptr(Cm), ldc, num_moduli, scaling_mode, _stream(stream)))
+
+
+def ozaki2_blas_workspace_bytes(layout, m, n, k, num_moduli, scaling_mode) -> int:
+    return int(lib().ozaki2_blas_workspace_bytes(_flag(layout), m, n, k, num_moduli, scaling_mode))
 
 
 def ozaki2_zgemm_workspace_bytes(m, n, k, num_moduli, scaling_mode) -> int:

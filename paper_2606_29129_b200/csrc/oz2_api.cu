@@ -282,13 +282,18 @@ int check_args(int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, cons
 template <typename T>
 __global__ void k_scale_c(int64_t m, int64_t n, T beta, T *C, int64_t ldc)
 {
-    int64_t i = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
-    int64_t j = blockIdx.x;
+    // one-dimensional grid of (row blocks) x n blocks: neither extent is bounded by the 65535 of grid.y / grid.z
+    const int64_t nrb = (m + blockDim.x - 1) / blockDim.x;
+    const int64_t j = blockIdx.x / nrb, i = (blockIdx.x - j * nrb) * blockDim.x + threadIdx.x;
     if (i < m) {
         T *p = C + i + j * ldc;
         *p = beta == (T)0 ? (T)0 : beta * *p;
     }
 }
+
+// blocks of a one-dimensional grid over (ceil(rows / 256) row blocks) x cols; the product is below 2^31 for anything
+// that fits the device's memory (rows x cols elements are stored)
+unsigned flat_grid(int64_t rows, int64_t cols) { return (unsigned)(((rows + 255) / 256) * cols); }
 
 // ---- complex variants (DESIGN.md 8b #4): real embedding and the complex alpha / beta tail -----------
 // R = double (zgemm) or float (cgemm); R2 = the interleaved pair type
@@ -306,7 +311,8 @@ __device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, 
 template <typename R>
 __global__ void k_zembed_a(int64_t m, int64_t k, const typename Pair<R>::type *__restrict__ A, int64_t lda, R *__restrict__ At)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, h = blockIdx.y;
+    const int64_t nrb = (m + blockDim.x - 1) / blockDim.x;               // flat_grid(m, k)
+    const int64_t h = blockIdx.x / nrb, i = (blockIdx.x - h * nrb) * blockDim.x + threadIdx.x;
     if (i >= m) return;
     const typename Pair<R>::type v = A[i + h * lda];
     const int64_t ld = 2 * m;
@@ -319,19 +325,21 @@ __global__ void k_zembed_a(int64_t m, int64_t k, const typename Pair<R>::type *_
 template <typename R>
 __global__ void k_zembed_b(int64_t k, int64_t n, const typename Pair<R>::type *__restrict__ B, int64_t ldb, R *__restrict__ Bt)
 {
-    const int64_t h = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int64_t nrb = (k + blockDim.x - 1) / blockDim.x;               // flat_grid(k, n)
+    const int64_t j = blockIdx.x / nrb, h = (blockIdx.x - j * nrb) * blockDim.x + threadIdx.x;
     if (h >= k) return;
     const typename Pair<R>::type v = B[h + j * ldb];
     Bt[h + j * 2 * k] = v.x;
     Bt[k + h + j * 2 * k] = v.y;
 }
 // C := alpha (c_r + i c_i) + beta C with [c_r; c_i] = Ct (2m x n); every product and sum rounded on its own, in the order
-// of the oracle (oracle/ozaki2_oracle.py zgemm / cgemm); alpha == 1 and beta == 0 are not multiplied; have_c == 0: c = 0
+// stated in include/ozaki2.h; alpha == 1, beta == 0 and beta == 1 are not multiplied; have_c == 0: c = 0
 template <typename R>
 __global__ void k_zcombine(int64_t m, int64_t n, R ar, R ai, const R *__restrict__ Ct, int have_c, R br, R bi,
                            typename Pair<R>::type *__restrict__ C, int64_t ldc)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    const int64_t nrb = (m + blockDim.x - 1) / blockDim.x;               // flat_grid(m, n)
+    const int64_t j = blockIdx.x / nrb, i = (blockIdx.x - j * nrb) * blockDim.x + threadIdx.x;
     if (i >= m) return;
     R tr = 0, ti = 0;
     if (have_c) {
@@ -343,7 +351,11 @@ __global__ void k_zcombine(int64_t m, int64_t n, R ar, R ai, const R *__restrict
         }
     }
     typename Pair<R>::type *dst = C + i + j * ldc;
-    if (br != (R)0 || bi != (R)0) {
+    if (br == (R)1 && bi == (R)0) {                                    // beta == 1 is not multiplied: C is added as it is
+        const typename Pair<R>::type c0 = *dst;
+        tr = add_rn(tr, c0.x);
+        ti = add_rn(ti, c0.y);
+    } else if (br != (R)0 || bi != (R)0) {
         const typename Pair<R>::type c0 = *dst;
         tr = add_rn(tr, sub_rn(mul_rn(br, c0.x), mul_rn(bi, c0.y)));
         ti = add_rn(ti, add_rn(mul_rn(br, c0.y), mul_rn(bi, c0.x)));
@@ -376,7 +388,7 @@ static int run_path(int f32, int64_t m, int64_t n, int64_t k, double alpha, cons
     if (k == 0 || alpha == 0.0) {
         // C := beta C (zeros if beta == 0, BLAS rule)
         if (!(beta == 1.0)) {
-            const dim3 grid((unsigned)n, (unsigned)((m + 255) / 256));
+            const dim3 grid(flat_grid(m, n));
             if (f32) k_scale_c<float><<<grid, 256, 0, st>>>(m, n, (float)beta, static_cast<float *>(C), ldc);
             else k_scale_c<double><<<grid, 256, 0, st>>>(m, n, beta, static_cast<double *>(C), ldc);
             oz2_count_launches(1);
@@ -670,9 +682,10 @@ static int complex_entry(int64_t m, int64_t n, int64_t k, R alpha_re, R alpha_im
     DeviceState *dev = nullptr;
     int rc = ensure_device(&dev);
     if (rc) return rc;
-    const dim3 gc((unsigned)((m + 255) / 256), (unsigned)n);
+    const dim3 gc(flat_grid(m, n));
     const bool have_c = k > 0 && !(alpha_re == (R)0 && alpha_im == (R)0);
     if (!have_c) {
+        if (beta_re == (R)1 && beta_im == (R)0) return 0;               // C := C, the BLAS quick return: C is not touched
         k_zcombine<R><<<gc, 256, 0, st>>>(m, n, alpha_re, alpha_im, nullptr, 0, beta_re, beta_im, reinterpret_cast<R2 *>(C), ldc);
         oz2_count_launches(1);
         OZ2_CUDA_TRY(cudaGetLastError());
@@ -684,10 +697,11 @@ static int complex_entry(int64_t m, int64_t n, int64_t k, R alpha_re, R alpha_im
     R *At = reinterpret_cast<R *>(ws + real_ws);
     R *Bt = reinterpret_cast<R *>(ws + real_ws + align_up(esz * (size_t)(2 * m) * (2 * k)));
     R *Ct = reinterpret_cast<R *>(ws + real_ws + align_up(esz * (size_t)(2 * m) * (2 * k)) + align_up(esz * (size_t)(2 * k) * n));
-    k_zembed_a<R><<<dim3((unsigned)((m + 255) / 256), (unsigned)k), 256, 0, st>>>(m, k, reinterpret_cast<const R2 *>(A), lda, At);
-    k_zembed_b<R><<<dim3((unsigned)((k + 255) / 256), (unsigned)n), 256, 0, st>>>(k, n, reinterpret_cast<const R2 *>(B), ldb, Bt);
-    oz2_count_launches(2);
+    k_zembed_a<R><<<dim3(flat_grid(m, k)), 256, 0, st>>>(m, k, reinterpret_cast<const R2 *>(A), lda, At);
     OZ2_CUDA_TRY(cudaGetLastError());
+    k_zembed_b<R><<<dim3(flat_grid(k, n)), 256, 0, st>>>(k, n, reinterpret_cast<const R2 *>(B), ldb, Bt);
+    OZ2_CUDA_TRY(cudaGetLastError());
+    oz2_count_launches(2);
     rc = run_path(esz == 4 ? 1 : 0, 2 * m, n, 2 * k, 1.0, At, 2 * m, Bt, 2 * k, 0.0, Ct, 2 * m, num_moduli, scaling_mode, st, nullptr);
     if (rc) return rc < 0 && rc > -100 ? -100 - rc : rc;      // an argument error of the embedded call would be a bug here
     k_zcombine<R><<<gc, 256, 0, st>>>(m, n, alpha_re, alpha_im, Ct, 1, beta_re, beta_im, reinterpret_cast<R2 *>(C), ldc);
@@ -763,6 +777,15 @@ size_t ozaki2_workspace_bytes(int64_t m, int64_t n, int64_t k, int num_moduli, i
     if (num_moduli < OZAKI2_MIN_MODULI || num_moduli > OZAKI2_MAX_MODULI) return 0;
     if (scaling_mode < 0 || scaling_mode > 2) return 0;
     return make_layout(m, n, k, num_moduli, scaling_mode).total;
+}
+
+// a row-major ozaki2_*gemm_blas call runs as the (n, m, k) problem, and the layout is not symmetric in m and n
+// (U is N n round_up(m, 16) bytes)
+size_t ozaki2_blas_workspace_bytes(int layout, int64_t m, int64_t n, int64_t k, int num_moduli, int scaling_mode)
+{
+    const int lay = parse_layout(layout);
+    if (lay < 0) return 0;
+    return lay ? ozaki2_workspace_bytes(n, m, k, num_moduli, scaling_mode) : ozaki2_workspace_bytes(m, n, k, num_moduli, scaling_mode);
 }
 
 int ozaki2_set_workspace(void *device_ptr, size_t bytes)
@@ -907,7 +930,7 @@ int ozaki2_debug_residue_gemm(int num_moduli, int64_t m, int64_t n, int64_t k, c
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (use_tensor_cores < 0 || use_tensor_cores > 4) return -8;
     if (use_tensor_cores) {
-        // 1: one CTA per tile (the ozaki2_dgemm path), 2: CTA pairs, 3: the path kernel without its epilogue
+        // 1: one CTA per tile, 2: CTA pairs (the ozaki2_dgemm path), 3 / 4: the kernels of 1 / 2 without their epilogue
         const int variant = use_tensor_cores == 2 ? OZ2_GEMM_PAIR : use_tensor_cores == 3 ? OZ2_GEMM_MMA_ONLY
                             : use_tensor_cores == 4 ? OZ2_GEMM_PAIR_MMA_ONLY : OZ2_GEMM_PATH;
         return oz2_launch_gemm_tc(variant, num_moduli, 0, m, n, k, resA, resB, k, U, m, nullptr, nullptr, st);

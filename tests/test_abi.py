@@ -102,3 +102,12 @@ def test_library_constants_against_mpmath_and_theorem1(B, N, golden):
     assert c["Pprop"] == down(l2 / 2 - mpf("0.5"))
     assert c["Pfast"] == down(l2 / 2 - mpf("1.5"))
     assert float(c["delta"]) == float.fromhex("0x1.000006p-1")
+
+
+def test_blas_workspace_query_follows_the_layout(B):
+    # a row-major BLAS-shaped call runs as the (n, m, k) problem; ozaki2_blas_workspace_bytes reports that orientation
+    for m, n, k, N, mode in [(1, 300, 64, 14, 2), (300, 1, 64, 14, 2), (17, 4000, 129, 20, 0), (8192, 8192, 8192, 16, 2)]:
+        assert B.ozaki2_blas_workspace_bytes("C", m, n, k, N, mode) == B.ozaki2_workspace_bytes(m, n, k, N, mode) > 0
+        assert B.ozaki2_blas_workspace_bytes("r", m, n, k, N, mode) == B.ozaki2_workspace_bytes(n, m, k, N, mode) > 0
+    assert B.ozaki2_blas_workspace_bytes("X", 8, 8, 8, 14, 2) == 0
+    assert B.ozaki2_workspace_bytes(1, 300, 64, 14, 2) != B.ozaki2_workspace_bytes(300, 1, 64, 14, 2)

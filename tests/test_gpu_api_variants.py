@@ -202,6 +202,71 @@ def test_zgemm_against_the_oracle_on_the_real_embedding(B, m, n, k, N, mode, alp
         assert np.max(np.abs(O.zgemm(A, Bm, N, mode) - ref) / np.abs(ref)) < {10: 1e-2, 14: 1e-6, 16: 1e-8, 17: 1e-9, 20: 1e-13}.get(N, 1.0)
 
 
+@pytest.mark.parametrize("cplx,m,n,k,N,mode,alpha,beta", [
+    # several ragged waves of every persistent kernel on the embedded (2m x 2k)(2k x n) problem, complex alpha / beta
+    ("z", 1100, 700, 1500, 16, 2, 0.5 - 2.0j, -1.25 + 0.75j), ("z", 600, 520, 900, 16, 1, 1.0, 1.0), ("z", 600, 520, 900, 18, 0, -1.0j, 0.0),
+    ("c", 1100, 700, 1500, 9, 2, 0.5 - 2.0j, -1.25 + 0.75j), ("c", 600, 520, 900, 9, 1, 1.0, 1.0), ("c", 600, 520, 900, 10, 0, -1.0j, 0.0),
+    # n or k beyond 65535 (the grid.y limit the embed / combine kernels once had); 2k > 2^17 also takes the K-blocked GEMM
+    ("z", 3, 70000, 5, 8, 2, 1.0, 0.5j), ("z", 2, 3, 66000, 14, 2, 2.0, 0.0), ("c", 2, 66000, 3, 6, 1, 1.0j, 1.0), ("c", 3, 2, 65600, 8, 2, 1.0, 0.0),
+])
+def test_complex_entries_at_multi_wave_and_long_sizes(B, cplx, m, n, k, N, mode, alpha, beta):
+    # bit-exact against the oracle's definition, element by element
+    import torch
+    ct = np.complex128 if cplx == "z" else np.complex64
+    A, Bm = _complex_inputs(m, n, k, 1.0, 1700 + m + n + k)
+    A, Bm = np.asfortranarray(A.astype(ct)), np.asfortranarray(Bm.astype(ct))
+    lda, ldb, ldc = m + 5, k + 3, m + 1
+    Ap = np.zeros((lda, k), ct, order="F"); Ap[:m] = A
+    Bp = np.zeros((ldb, n), ct, order="F"); Bp[:k] = Bm
+    rng = np.random.Generator(np.random.PCG64(29))
+    Cin = np.asfortranarray((rng.standard_normal((ldc, n)) + 1j * rng.standard_normal((ldc, n))).astype(ct))
+    Ad = torch.from_numpy(np.ascontiguousarray(Ap.T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray(Bp.T)).cuda()
+    Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+    B.ensure_zgemm_workspace(m, n, k, N, mode)
+    call, oracle = (B.ozaki2_zgemm, O.zgemm) if cplx == "z" else (B.ozaki2_cgemm, O.cgemm)
+    assert call(m, n, k, alpha, Ad, lda, Bd, ldb, beta, Cd, ldc, N, mode) == 0
+    torch.cuda.synchronize()
+    got = np.asfortranarray(Cd.cpu().numpy().T)
+    want = oracle(A, Bm, N, mode, alpha=alpha, beta=beta, C_in=Cin[:m])
+    assert got.dtype == ct and np.array_equal(got[:m], want)
+    assert np.array_equal(got[m:], Cin[m:])
+
+
+@pytest.mark.parametrize("cplx", ["z", "c"])
+def test_complex_beta_one_adds_c_as_it_is_and_the_quick_return_leaves_it_alone(B, cplx):
+    import torch
+    ct, N = (np.complex128, 14) if cplx == "z" else (np.complex64, 8)
+    call, oracle = (B.ozaki2_zgemm, O.zgemm) if cplx == "z" else (B.ozaki2_cgemm, O.cgemm)
+    m, n, k = 40, 24, 70
+    A, Bm = _complex_inputs(m, n, k, 0.5, 77)
+    A, Bm = np.asfortranarray(A.astype(ct)), np.asfortranarray(Bm.astype(ct))
+    rng = np.random.Generator(np.random.PCG64(5))
+    Cin = np.asfortranarray((rng.standard_normal((m, n)) + 1j * rng.standard_normal((m, n))).astype(ct))
+    Cin[3, 4] = complex(np.inf, 2.0)                  # a non-finite part must stay in its own part
+    Cin[5, 6] = complex(-1.0, np.nan)
+    Cin[7, 8] = complex(-np.inf, -0.0)
+    Ad = torch.from_numpy(np.ascontiguousarray(A.T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray(Bm.T)).cuda()
+    B.ensure_zgemm_workspace(m, n, k, N, 2)
+    word = np.uint64 if cplx == "z" else np.uint32
+    for alpha, kk in ((0.0, k), (1.0, 0)):            # quick returns with beta == 1: C is not touched at all
+        Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+        before = B.ozaki2_kernel_launches()
+        assert call(m, n, kk, alpha, Ad, m, Bd, max(1, kk), 1.0, Cd, m, N, 2) == 0
+        torch.cuda.synchronize()
+        assert B.ozaki2_kernel_launches() == before
+        assert np.array_equal(Cd.cpu().numpy().view(word), np.ascontiguousarray(Cin.T).view(word))
+    Cd = torch.from_numpy(np.ascontiguousarray(Cin.T)).cuda()
+    assert call(m, n, k, 0.5 - 2.0j, Ad, m, Bd, k, 1.0, Cd, m, N, 2) == 0
+    torch.cuda.synchronize()
+    got = np.asfortranarray(Cd.cpu().numpy().T)
+    want = oracle(A, Bm, N, 2, alpha=0.5 - 2.0j, beta=1.0, C_in=Cin)
+    # (NaN payloads are not part of the contract: FP32 adds on the GPU return the canonical NaN)
+    assert np.array_equal(got.real, want.real, equal_nan=True) and np.array_equal(got.imag, want.imag, equal_nan=True)
+    assert np.isfinite(got[3, 4].imag) and np.isfinite(got[5, 6].real) and got[7, 8].real == -np.inf and np.isfinite(got[7, 8].imag)
+
+
 def test_zgemm_quick_returns_and_errors(B):
     import torch
     m, n, k, N = 32, 16, 24, 12
@@ -326,6 +391,35 @@ def test_plain_launches_give_the_same_results(B):
                        timeout=600, cwd=root)
     assert r.returncode == 0, r.stderr[-2000:]
     assert "smoke ok" in r.stdout
+
+
+def test_row_major_call_with_the_workspace_the_query_reports(B):
+    # the layout is not symmetric in m and n and a row-major call runs as the (n, m, k) problem: ozaki2_blas_workspace_bytes
+    # reports what the call with that layout needs, and a workspace of exactly that size serves it (m = 300, n = 1: a
+    # row-major call needs more than ozaki2_workspace_bytes(m, n, k) says)
+    import torch
+    m, n, k, N, mode = 300, 1, 64, 14, 2
+    A, Bm = W.eq15_matrices(m, n, k, 1.0, 31337)
+    assert B.ozaki2_blas_workspace_bytes("C", m, n, k, N, mode) == B.ozaki2_workspace_bytes(m, n, k, N, mode)
+    assert B.ozaki2_blas_workspace_bytes("R", m, n, k, N, mode) == B.ozaki2_workspace_bytes(n, m, k, N, mode)
+    assert B.ozaki2_blas_workspace_bytes(101, m, n, k, N, mode) > B.ozaki2_blas_workspace_bytes(102, m, n, k, N, mode)
+    want = O.dgemm(A, Bm, N, mode)
+    for layout in ("R", "C"):
+        need = B.ozaki2_blas_workspace_bytes(layout, m, n, k, N, mode)
+        ws = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+        off = (-ws.data_ptr()) % 256
+        assert B.ozaki2_set_workspace(ws.data_ptr() + off, need) == 0
+        a = np.ascontiguousarray(A) if layout == "R" else np.ascontiguousarray(A.T)      # stored buffers, row by row
+        b = np.ascontiguousarray(Bm) if layout == "R" else np.ascontiguousarray(Bm.T)
+        Ad, Bd = torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda()
+        Cd = torch.empty((m, n) if layout == "R" else (n, m), dtype=torch.float64, device="cuda")
+        lda, ldb, ldc = (k, n, n) if layout == "R" else (m, k, m)
+        assert B.ozaki2_dgemm_blas(layout, "N", "N", m, n, k, 1.0, Ad, lda, Bd, ldb, 0.0, Cd, ldc, N, mode) == 0
+        torch.cuda.synchronize()
+        got = Cd.cpu().numpy() if layout == "R" else Cd.cpu().numpy().T
+        assert np.array_equal(got, want), layout
+        assert B.ozaki2_set_workspace(None, 0) == 0
+        del ws
 
 
 def test_blas_entry_fuzz(B):

@@ -1,6 +1,8 @@
 """Pins for the oracle's complex variant (the paper names ZGEMM as future work without formulas, P:58, P:444;
 reading in DESIGN.md 8b #4: the product of the real embeddings).  What fixes it: the textbook identity between a complex
 product and its real embedding, exact integer cases, the real special case, and the paper's invariants carried over."""
+from fractions import Fraction
+
 import numpy as np
 import pytest
 
@@ -72,10 +74,33 @@ def test_error_against_numpy_complex_product_and_alpha_beta():
     out = O.zgemm(A, B, 18, PROP, alpha=alpha, beta=beta, C_in=Cin)
     want = alpha * C + beta * Cin
     assert np.max(np.abs(out - want)) <= 4 * np.finfo(float).eps * np.max(np.abs(want))
-    # the stated operation order, element by element
-    tr = alpha.real * C.real - alpha.imag * C.imag + (beta.real * Cin.real - beta.imag * Cin.imag)
-    ti = alpha.real * C.imag + alpha.imag * C.real + (beta.real * Cin.imag + beta.imag * Cin.real)
-    assert np.array_equal(out.real, tr) and np.array_equal(out.imag, ti)
+
+
+def test_beta_one_adds_c_as_it_is():
+    # beta == 1 is not multiplied (the BLAS rule the real entry points follow: fma(1, C, t) = C + t).  For finite C_in that
+    # is the single rounding of t + C_in per part; a non-finite part of an entry stays in its own part
+    A, B = complex_inputs(12, 9, 64, 0.5, 31)
+    rng = np.random.Generator(np.random.PCG64(3))
+    Cin = rng.standard_normal((12, 9)) + 1j * rng.standard_normal((12, 9))
+    for alpha in (1.0, 0.5 - 2.0j):
+        t = O.zgemm(A, B, 16, PROP, alpha=alpha)
+        out = O.zgemm(A, B, 16, PROP, alpha=alpha, beta=1.0, C_in=Cin)
+        for i in range(12):
+            for j in range(9):                   # RN(t + c) from the exact rational sum, part by part
+                for got, a, b in ((out[i, j].real, t[i, j].real, Cin[i, j].real), (out[i, j].imag, t[i, j].imag, Cin[i, j].imag)):
+                    assert got == float(Fraction(float(a)) + Fraction(float(b)))
+    bad = Cin.copy()
+    bad[3, 4] = complex(np.inf, 2.0)
+    bad[5, 6] = complex(-1.0, np.nan)
+    out = O.zgemm(A, B, 16, PROP, beta=1.0, C_in=bad)
+    t = O.zgemm(A, B, 16, PROP)
+    assert out[3, 4].real == np.inf and out[3, 4].imag == t[3, 4].imag + 2.0
+    assert out[5, 6].real == t[5, 6].real - 1.0 and np.isnan(out[5, 6].imag)
+    A32, B32 = A.astype(np.complex64), B.astype(np.complex64)
+    out32 = O.cgemm(A32, B32, 9, PROP, beta=1.0, C_in=bad.astype(np.complex64))
+    t32 = O.cgemm(A32, B32, 9, PROP)
+    assert out32.dtype == np.complex64 and out32[3, 4].real == np.inf
+    assert out32[3, 4].imag == np.float32(t32[3, 4].imag + np.float32(2.0)) and np.isnan(out32[5, 6].imag)
 
 
 # ---- single-precision complex variant (cgemm): the same reading on FP32 parts -------------------------------------------
