@@ -48,7 +48,7 @@ MODE_NAMES = {0: "accurate", 1: "fast", 2: "prop"}
 NOMINAL_INT8_TOPS = 4500.0          # P:30 (B200 spec sheet, dense)
 INT8_OVER_BF16 = 2.0                # guide's nominal ratio 4.5 / 2.25 PFLOP/s
 DEFAULT_MODULI = {2: 16, 3: 20, 4: 16}
-TRAFFIC_CSV = os.path.join("profiles", "r02_dram_traffic.csv")      # ncu dram bytes per launch, see the .md beside it
+TRAFFIC_CSV = os.path.join("profiles", "r03_dram_traffic.csv")      # ncu dram bytes per launch, see the .md beside it
 
 
 def parse_args():
@@ -65,6 +65,10 @@ def parse_args():
     ap.add_argument("--protocol", default="fixed", choices=["fixed", "paper"],
                     help="paper: P:387-392 iteration caps (warm-up 3 s / 100, timed 12 s / 100) instead of --steps / --warmup")
     ap.add_argument("--sgemm", action="store_true", help="SURVEY 8(f) #1: the FP32 in / FP32 out variant (paper: N = 3..12)")
+    ap.add_argument("--zgemm", action="store_true", help="SURVEY 8(f) #4: ozaki2_zgemm on complex FP64 matrices of the config's shape "
+                    "(emulated complex TFLOPS = 8mnk / t; no e2e, no stage breakdown)")
+    ap.add_argument("--cgemm", action="store_true", help="SURVEY 8(f) #4: ozaki2_cgemm (complex FP32; default N = 9)")
+    ap.add_argument("--skip-sweep", action="store_true", help="leave out the sweep over the config's other moduli counts")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="profiling runs only: leave out the oracle leg")
     ap.add_argument("--skip-ceiling", action="store_true", help="profiling runs only: leave out the MMA-only ceiling runs")
@@ -72,8 +76,9 @@ def parse_args():
     ap.add_argument("--accuracy", action="store_true", help="add max relative error vs the double-double reference "
                     "(P:268) on a sampled slab, and max |R_l| on it (INT32 headroom, P:113)")
     a = ap.parse_args()
+    a.moduli_defaulted = not a.moduli
     if not a.moduli:
-        a.moduli = DEFAULT_MODULI[a.config]
+        a.moduli = 9 if a.cgemm else DEFAULT_MODULI[a.config]
     return a
 
 
@@ -138,9 +143,15 @@ class ClockSampler:
         except subprocess.TimeoutExpired:
             self.proc.kill()
         self.thread.join(timeout=5)
+        return self.summarize(self.window)
+
+    def summarize(self, window):
+        """Clocks over [window[0], window[1]] (host time) from the samples taken so far; the sampler keeps running."""
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
         sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        inside = [ln for ts, ln in self.lines if self.window[0] <= ts <= self.window[1]]
+        inside = [ln for ts, ln in list(self.lines) if window[0] <= ts <= window[1]]
         # a timed region shorter than the sampling period: fall back to every sample taken since start()
         for line in (inside if inside else [ln for _, ln in self.lines]):
             f = [x.strip() for x in line.split(",")]
@@ -161,19 +172,21 @@ class ClockSampler:
 
 
 def profiled_traffic(args, m, n, k, N, mode, f32):
-    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture (TRAFFIC_CSV; the .md
-    beside it names the command and the commit it was taken at), only for the workload of that capture."""
+    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` captures (TRAFFIC_CSV; the .md
+    beside it names the commands and the commit they were taken at), for the workloads that were captured; a constant
+    from that file, not a measurement of this run (the figure moves from board to board)."""
     path = os.path.join(ROOT, TRAFFIC_CSV)
-    if not (os.path.exists(path) and (m, n, k) == (8192, 8192, 8192) and N == 16 and mode == 2 and not f32):
+    if not os.path.exists(path) or f32:
         return None
+    key = f"{m}x{n}x{k}_N{N}_mode{mode}"                       # rows: workload,"kernel",bytes
     with open(path) as fh:
         for line in fh:
-            if line.startswith('"k3_residue_gemm'):
+            if line.startswith(key + ',"k3_residue_gemm'):
                 return float(line.rsplit(",", 1)[1])
     return None
 
 
-NCU_SUMMARY_MD = os.path.join("profiles", "r02_ncu_summary.md")
+NCU_SUMMARY_MD = os.path.join("profiles", "r03_ncu_summary.md")
 
 
 def profiled_issue_bounds(args, m, n, k, N, mode, f32, sm_count=148, sm_mhz=1965.0):
@@ -324,6 +337,79 @@ def measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=20):
     return out
 
 
+def run_complex(args, pkg, torch, W, local, world, rank, m, n, k, phi, N, mode, K, Wm, peaks):
+    """--zgemm / --cgemm: ozaki2_zgemm / ozaki2_cgemm on complex matrices whose real and imaginary parts are
+    eq. (15) draws of the config; emulated complex TFLOPS = 8mnk / t (a complex multiply-add = 4 real ones), median of K
+    event-bracketed calls.  The call runs the real path on the (2m x 2k)(2k x n) embedding: 4 real products, so the INT8 work
+    is N 2 (2m) n (2k) = 4 N 2mnk."""
+    import torch.distributed as dist
+    cplx = np.complex64 if args.cgemm else np.complex128
+    Ar, Br = W.eq15_matrices(m, n, k, phi, W.seed_for(args.config, rank))
+    Ai, Bi = W.eq15_matrices(m, n, k, phi, W.seed_for(args.config, rank) + 5)
+    Ad = torch.from_numpy(np.ascontiguousarray((Ar + 1j * Ai).astype(cplx).T)).cuda()
+    Bd = torch.from_numpy(np.ascontiguousarray((Br + 1j * Bi).astype(cplx).T)).cuda()
+    del Ar, Br, Ai, Bi
+    Cd = torch.empty((n, m), dtype=Ad.dtype, device="cuda")
+    pkg.ensure_zgemm_workspace(m, n, k, N, mode)
+    call = pkg.ozaki2_cgemm if args.cgemm else pkg.ozaki2_zgemm
+    stream = torch.cuda.current_stream()
+
+    def step():
+        rc = call(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, N, mode, stream)
+        if rc:
+            raise pkg.Ozaki2Error(rc, "ozaki2_cgemm" if args.cgemm else "ozaki2_zgemm")
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    for _ in range(Wm):
+        step()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    sampler.wait_first_sample()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = pkg.ozaki2_kernel_launches()
+    sampler.window[0] = time.time()
+    evs[0].record(stream)
+    for s_ in range(K):
+        step()
+        evs[s_ + 1].record(stream)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.window[1] = time.time()
+    launches = pkg.ozaki2_kernel_launches() - launches0
+    clocks = sampler.stop()
+    step_ms = [evs[s_].elapsed_time(evs[s_ + 1]) for s_ in range(K)]
+    med_ms = statistics.median(step_ms)
+    if world > 1:
+        tt = torch.tensor([med_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        med_ms = float(tt[0].item())
+    cflops = 8.0 * m * n * k
+    int8_peak = INT8_OVER_BF16 * peaks["bf16"]
+    int8_ops = 4.0 * N * 2.0 * m * n * k
+    if rank == 0:
+        name = "cgemm" if args.cgemm else "zgemm"
+        print(json.dumps(dict(
+            metric="emulated_complex_fp32_tflops" if args.cgemm else "emulated_complex_fp64_tflops", value=world * cflops / (med_ms * 1e-3) / 1e12,
+            unit="TFLOPS", n_gpus=world, steps=K, warmup=Wm, ms_per_step=med_ms, ms_per_step_min=min(step_ms), ms_per_step_max=max(step_ms),
+            higher_is_better=True, scaling="weak", vs_baseline=None,
+            dtype="int8xint8->int32 (tcgen05 kind::i8), complex %s in/out" % ("fp32" if args.cgemm else "fp64"), data="synthetic",
+            config=dict(workload=f"ozaki2_{name} (SURVEY 8(f) #4) on BASELINE configs[{args.config}] shape m={m}, n={n}, k={k}, eq.(15) "
+                                 f"phi={phi} real and imaginary parts, N={N} moduli, mode={MODE_NAMES[mode]}", moduli=N,
+                        scaling_mode=MODE_NAMES[mode], l2="inputs larger than L2" if 2 * Ad.element_size() * m * k > 126e6 else "inputs fit L2",
+                        parallelism="replicas" if world > 1 else "single GPU"),
+            clocks=clocks, e2e=None, gpu_launches=int(launches),
+            roofline=dict(bound="tensor", kernel="k3_residue_gemm_pair<EPI_MODP> on the real embedding (2m x 2k)(2k x n): 4 real products",
+                          achieved=int8_ops / (med_ms * 1e-3) / 1e12, peak=int8_peak, unit="TFLOP/s", frac=int8_ops / (med_ms * 1e-3) / 1e12 / int8_peak,
+                          note="achieved = INT8 ops of the embedded product / WHOLE-call time (no stage events on this entry point)", traffic=None),
+            cpu_baseline=None, peaks=dict(hbm_gbs=peaks["hbm_gbs"], bf16_tflops=peaks["bf16"], source=peaks["source"]))))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -351,6 +437,8 @@ def main():
     N, mode = args.moduli, args.mode
     K, Wm = args.steps, max(args.warmup, 3)
     flops = 2.0 * m * n * k
+    if args.zgemm or args.cgemm:
+        return run_complex(args, pkg, torch, W, local, world, rank, m, n, k, phi, N, mode, K, Wm, peaks)
 
     # ---- inputs: eq. (15), seeded, one variant per rank (replicas)
     A, B = W.eq15_matrices(m, n, k, phi, W.seed_for(args.config, rank))
@@ -442,7 +530,10 @@ def main():
     ceiling = None
     if not args.skip_ceiling and not f32:
         ceiling = measure_int8_ceiling(pkg, torch, m, n, k, N, stream, reps=args.ceiling_reps)
-    roofline = dict(bound="tensor", kernel="k3_residue_gemm<EPI_MODP> (tcgen05.mma kind::i8, batched over N moduli)",
+    # the kernel oz2_launch_gemm_tc picks for this shape: CTA pairs (cta_group::2) for m > 128 and k <= 2^17, else one CTA per tile
+    pair = m > 128 and ((k + 127) // 128) * 128 <= (1 << 17) and os.environ.get("OZAKI2_GEMM", "") != "single"
+    s3_kernel = "k3_residue_gemm_pair<EPI_MODP> (cta_group::2" if pair else "k3_residue_gemm<EPI_MODP> (cta_group::1"
+    roofline = dict(bound="tensor", kernel=s3_kernel + " tcgen05.mma kind::i8, batched over N moduli)",
                     achieved=achieved, peak=int8_peak, unit="TFLOP/s", frac=achieved / int8_peak,
                     peak_source=f"2 x bf16_tflops burst ({peaks['source']}): another dtype's measured peak x the nominal "
                                 "ratio 4.5 / 2.25; MEASURED_PEAKS.json has no INT8 entry",
@@ -474,6 +565,54 @@ def main():
     path = dict(roofline_ms=t_roof_ms, frac=t_roof_ms / med_ms, peak_tops=int8_peak, roofline_ms_nominal_4500=t_roof_nominal_ms,
                 frac_nominal_4500=t_roof_nominal_ms / med_ms, hbm_ms=t_hbm_ms, total_algorithmic_gb=total_bytes / 1e9,
                 int8_ops=s3_ops, stage_sum_ms=sum(stage_ms))
+
+    # ---- sweep over the other moduli counts the config names (BASELINE metric: "TFLOPS ... vs moduli N"; north_star: ">= 70 % of the
+    # roofline at 8192^3 with 14-18 moduli"): the same matrices, same mode, 3 warm-up + 10 timed steps per N with stage events
+    sweep = None
+    if world == 1 and args.moduli_defaulted and not args.skip_sweep and not f32 and not args.size and args.protocol == "fixed":
+        sweep = []
+        sw = ClockSampler(local)
+        sw.start()
+        sw.wait_first_sample()
+        Ks = 10
+        for Ns in W.CONFIGS[args.config]["moduli"]:
+            if Ns == N:
+                continue
+            pkg.ensure_workspace(m, n, k, Ns, mode)
+            for _ in range(3):
+                rc = pkg.ozaki2_dgemm(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, Ns, mode, stream)
+                if rc:
+                    raise pkg.Ozaki2Error(rc, "ozaki2_dgemm")
+            sevs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(Ks)]
+            for row in sevs:
+                for ev in row:
+                    ev.record(stream)
+            torch.cuda.synchronize()
+            w0 = time.time()
+            for r in range(Ks):
+                rc = pkg.dgemm_with_stage_events(m, n, k, 1.0, Ad, m, Bd, k, 0.0, Cd, m, Ns, mode, sevs[r], stream)
+                if rc:
+                    raise pkg.Ozaki2Error(rc, "ozaki2_dgemm_stages")
+            torch.cuda.synchronize()
+            w1 = time.time()
+            ms_n = statistics.median(sevs[r][0].elapsed_time(sevs[r][4]) for r in range(Ks))
+            st_n = [statistics.median(sevs[r][t].elapsed_time(sevs[r][t + 1]) for r in range(Ks)) for t in range(4)]
+            bytes_n = (2 * esz + 2 * Ns) * X + (2 * Ns + esz) * Y
+            roof_n = max(Ns * flops / (int8_peak * 1e12) * 1e3, bytes_n / (peaks["hbm_gbs"] * 1e9) * 1e3)
+            ck = sw.summarize((w0, w1))
+            sweep.append(dict(moduli=Ns, ms_per_step=ms_n, value=flops / (ms_n * 1e-3) / 1e12, unit="TFLOPS", steps=Ks, warmup=3,
+                              stage_ms=dict(S1=st_n[0], S2=st_n[1], S3=st_n[2], S4S5=st_n[3]),
+                              k3_tops=Ns * flops / (st_n[2] * 1e-3) / 1e12, roofline_ms=roof_n, path_frac=roof_n / ms_n,
+                              clocks=dict(sm_mhz=ck.get("sm_mhz"), power_w_median=ck.get("power_w_median"), samples=ck.get("samples"),
+                                          reasons=ck.get("reasons"))))
+        sw.stop()
+        sweep.append(dict(moduli=N, ms_per_step=med_ms, value=value, unit="TFLOPS", steps=K, warmup=Wm,
+                          stage_ms=dict(S1=stage_ms[0], S2=stage_ms[1], S3=stage_ms[2], S4S5=stage_ms[3]), k3_tops=achieved,
+                          roofline_ms=t_roof_ms, path_frac=t_roof_ms / med_ms, note="the headline line above"))
+        sweep.sort(key=lambda d: d["moduli"])
+        pkg.ensure_workspace(m, n, k, N, mode)
+        step()                                  # C of the headline N again: the e2e and cpu_baseline legs compare against it
+        torch.cuda.synchronize()
 
     # ---- e2e: host buffers through ozaki2_dgemm_host / ozaki2_sgemm_host (pinned), copies inside the timed region
     e2e = None
@@ -560,7 +699,7 @@ def main():
                                 l2="inputs larger than L2 (A + B = %.2f GB per step, residue planes %.2f GB)" %
                                    (esz * X / 1e9, N * X / 1e9), parallelism="replicas" if world > 1 else "single GPU"),
                     clocks=clocks, e2e=e2e, plain_call=plain_call, gpu_launches=int(launches), roofline=roofline, stages=stages, path=path,
-                    cpu_baseline=cpu, accuracy=accuracy,
+                    cpu_baseline=cpu, accuracy=accuracy, sweep=sweep,
                     peaks=dict(hbm_gbs=peaks["hbm_gbs"], bf16_tflops=peaks["bf16"],
                                bf16_tflops_sustained=peaks["bf16_sustained"], source=peaks["source"]),
                     context="paper (GH200): cuBLAS DGEMM 60.9 TFLOPS, Ozaki-II DGEMM up to 80.2 TFLOPS (P:48); "

@@ -51,3 +51,18 @@ def test_gpu_arm_json_line():
     assert d["e2e"]["h2d_bytes_per_step"] == 2 * 8 * 1024 * 1024 and d["e2e"]["matches_device_path"] is True
     assert d["cpu_baseline"]["gpu_slab_bit_exact_vs_oracle"] is True
     assert "sm_mhz" in d["clocks"] and "reasons" in d["clocks"]
+
+
+@pytest.mark.gpu
+def test_gpu_arm_default_run_carries_the_moduli_sweep():
+    # the default workload (configs[2], N = 16) also times the config's other moduli counts; the legs after the sweep still
+    # see the headline N's result
+    lines = run([sys.executable, "bench.py", "--steps", "3", "--warmup", "3", "--skip-ceiling", "--skip-cpu-baseline"], timeout=900)
+    d = json.loads(lines[0])
+    sw = d["sweep"]
+    assert [r["moduli"] for r in sw] == [14, 15, 16, 17, 18] and d["config"]["moduli"] == 16
+    for r in sw:
+        assert r["ms_per_step"] > 0 and 0 < r["path_frac"] < 1.2 and set(r["stage_ms"]) == {"S1", "S2", "S3", "S4S5"}
+    assert d["e2e"]["matches_device_path"] is True
+    assert d["roofline"]["kernel"].startswith("k3_residue_gemm_pair")
+    assert d["gpu_launches"] == 3 * 8
